@@ -1,0 +1,154 @@
+"""Pins for the oracle's integer lists (O-LIST) and for the three renderers agreeing.
+
+* row scan (N-SCAN) against an independent exact test written here in fp64 numpy: a cell is hit
+  iff the minimum of the quadratic form over the (clipped) cell rectangle is <= tau;
+* conservativeness by brute force: every pixel centre with q <= tau lies in a listed macro-tile;
+* counts / offsets / sorted segments against numpy (bincount, cumsum, lexsort);
+* orc_render == orc_brute (bounding box logic) and == orc_render_batched (Eq. (1)),
+  with B_r = 16 forcing many batches per macro-tile.
+No GPU, no product code."""
+import math
+
+import numpy as np
+import pytest
+
+import higs_scenes as hs
+import oracle
+
+
+def _min_q_over_rect(mux, muy, A, B2, C, x0, x1, y0, y1):
+    """Exact minimum of q(dx,dy) = A dx^2 + B2 dx dy + C dy^2 over the rectangle, in fp64."""
+    if x0 <= mux <= x1 and y0 <= muy <= y1:
+        return 0.0
+    best = math.inf
+    for y in (y0, y1):                       # horizontal edges: minimise over x in [x0, x1]
+        dy = y - muy
+        dx = min(max(-B2 * dy / (2 * A), x0 - mux), x1 - mux)
+        best = min(best, A * dx * dx + B2 * dx * dy + C * dy * dy)
+    for x in (x0, x1):                       # vertical edges
+        dx = x - mux
+        dy = min(max(-B2 * dx / (2 * C), y0 - muy), y1 - muy)
+        best = min(best, A * dx * dx + B2 * dx * dy + C * dy * dy)
+    return best
+
+
+def _cells_by_rect_test(geo, W, H, cw, ch):
+    mux, muy, a, b, c, tau = (float(v) for v in geo[:6])
+    det = a * c - b * b
+    A, B2, C = c / det, -2 * b / det, a / det
+    ncx, ncy = (W + cw - 1) // cw, (H + ch - 1) // ch
+    hit, near = [], []
+    for r in range(ncy):
+        for m in range(ncx):
+            q = _min_q_over_rect(mux, muy, A, B2, C, m * cw, min((m + 1) * cw, W), r * ch, min((r + 1) * ch, H))
+            if q <= tau:
+                hit.append(r * ncx + m)
+            if abs(q - tau) <= 2e-3 * tau:  # too close to call across fp32 / fp64
+                near.append(r * ncx + m)
+    return set(hit), set(near)
+
+
+@pytest.mark.parametrize("W,H,cw,ch", [(640, 480, 64, 32), (100, 70, 64, 32), (129, 129, 8, 8), (640, 480, 8, 8)])
+def test_row_scan_equals_min_q_over_rectangle(W, H, cw, ch):
+    s = hs.scene_cfg1(N=6000)
+    rng = np.random.default_rng(5)
+    s.scales[:] = s.scales * np.exp(rng.normal(0.8, 0.8, s.scales.shape)).astype(np.float32)  # some big, skewed ones
+    cam = hs.make_camera(W, H, eye=(0.4, 0.2, -1.0), centre=(0.0, 0.0, 5.0))
+    pr = oracle.project(s, cam)
+    idx = np.nonzero(pr.valid)[0]
+    assert idx.size > 1500
+    checked = 0
+    for i in idx[:: max(1, idx.size // 700)]:
+        got = set(oracle.scan(pr.geo[i], W, H, cw, ch).tolist())
+        want, near = _cells_by_rect_test(pr.geo[i], W, H, cw, ch)
+        assert got - near == want - near, (i, sorted(got ^ want))
+        assert len(got) > 0
+        checked += 1
+    assert checked > 500
+
+
+def test_row_scan_is_conservative_for_pixel_centres():
+    s = hs.scene_cfg0()
+    cam = s.cameras[0]
+    pr = oracle.project(s, cam)
+    nmx, _ = oracle.grid_dims(cam.W, cam.H)
+    ys, xs = np.mgrid[0:cam.H, 0:cam.W]
+    for i in range(0, s.N, 3):
+        cells = set(oracle.scan(pr.geo[i], cam.W, cam.H).tolist())
+        mux, muy, _, _, _, tau = (np.float32(v) for v in pr.geo[i, :6])
+        A, B2, C = (np.float32(v) for v in pr.conic[i])
+        dx = (xs.astype(np.float32) + np.float32(0.5)) - mux
+        dy = (ys.astype(np.float32) + np.float32(0.5)) - muy
+        q = A.astype(np.float64) * dx * dx + B2.astype(np.float64) * dx * dy + C.astype(np.float64) * dy * dy
+        inside = q <= float(tau) * (1 + 1e-5)
+        need = set(((ys[inside] // 32) * nmx + xs[inside] // 64).tolist())
+        assert need <= cells, i
+
+
+@pytest.mark.parametrize("B_r", [1024, 16])
+def test_lists_against_numpy(B_r):
+    s = hs.scene_cfg1(N=30_000)
+    cam = s.cameras[0]
+    pr = oracle.project(s, cam)
+    ls = oracle.bin_lists(pr, B_r=B_r)
+    nmx, nmy = oracle.grid_dims(cam.W, cam.H)
+    NM = nmx * nmy
+    cell, gid = [], []
+    for i in np.nonzero(pr.valid)[0]:
+        c = oracle.scan(pr.geo[i], cam.W, cam.H)
+        cell.append(c); gid.append(np.full(c.size, i, np.int64))
+    cell = np.concatenate(cell); gid = np.concatenate(gid)
+    cnt = np.bincount(cell, minlength=NM)
+    assert (ls.mt_count == cnt).all()
+    assert (ls.mt_offset == np.concatenate([[0], np.cumsum(cnt)])).all()
+    assert ls.n_pairs == cell.size == int(ls.mt_count.sum())
+    order = np.lexsort((gid, pr.key[gid], cell))           # by cell, then key, then id
+    assert (ls.ids == gid[order]).all()
+    assert (ls.keys == pr.key[gid[order]]).all()
+    nb = -(-cnt // B_r)
+    assert (ls.batch_offset == np.concatenate([[0], np.cumsum(nb)])).all()
+    assert ls.n_units == int(nb.sum())
+    assert (cnt > 1024).any() or B_r == 16                 # at least one multi-batch macro-tile at the paper's B_r
+
+
+def test_render_equals_brute_equals_batched_cfg0():
+    s = hs.scene_cfg0()
+    cam = s.cameras[0]
+    pr = oracle.project(s, cam)
+    img = oracle.render(pr)
+    brute = oracle.brute(pr)
+    assert np.array_equal(img, brute)                      # same arithmetic, bbox only prunes
+    ls = oracle.bin_lists(pr)
+    full = oracle.render_batched(pr, ls, B_r=1 << 30, terminate=False)
+    np.testing.assert_allclose(full, oracle.render(pr, terminate=False), atol=1e-12)
+    for B_r in (1024, 16, 1):
+        split = oracle.render_batched(pr, oracle.bin_lists(pr, B_r=B_r), B_r=B_r, terminate=False)
+        np.testing.assert_allclose(split, full, atol=1e-12)            # Eq. (1) is associative
+        split_t = oracle.render_batched(pr, oracle.bin_lists(pr, B_r=B_r), B_r=B_r, terminate=True)
+        assert np.abs(split_t - img).max() < 1e-4 * float(pr.rgb.max())  # termination point is free (Q2)
+
+
+def test_render_equals_brute_on_a_window_of_cfg1():
+    s = hs.scene_cfg1(N=20_000)
+    cam = s.cameras[0]
+    pr = oracle.project(s, cam)
+    win = (300, 200, 340, 232)
+    assert np.array_equal(oracle.render(pr, window=win), oracle.brute(pr, window=win))
+    full = oracle.render(pr)
+    assert np.array_equal(full[200:232, 300:340], oracle.render(pr, window=win))
+    assert np.array_equal(oracle.render(pr, threads=1), oracle.render(pr, threads=3))
+
+
+def test_odd_sizes_empty_and_all_culled():
+    s = hs.scene_cfg0(N=300, W=100, H=70)
+    cam = s.cameras[0]
+    pr = oracle.project(s, cam)
+    ls = oracle.bin_lists(pr)
+    assert ls.mt_count.size == 2 * 3
+    np.testing.assert_allclose(oracle.render_batched(pr, ls, terminate=False), oracle.render(pr, terminate=False), atol=1e-12)
+    s.means[:, 2] = -1.0                                    # everything behind the camera
+    pr = oracle.project(s, cam)
+    assert pr.n_vis == 0
+    ls = oracle.bin_lists(pr)
+    assert ls.n_pairs == 0 and ls.n_units == 0
+    assert not oracle.render(pr).any()
