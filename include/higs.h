@@ -1,0 +1,171 @@
+/*
+ * higs.h -- C ABI of the B200-native HiGS forward render path
+ * (arxiv/paper_2606_00352, "HiGS: A Hierarchical Rendering Architecture for Real-Time 3D
+ * Gaussian Splatting"; citations are PAPER.md:<line> + section).
+ *
+ * One frame = the pipeline of PAPER.md:53 (Fig. 2) / PAPER.md:230-301 (section 4):
+ *   a1 projection + cull + SH colour          PAPER.md:241-245 (4.2)
+ *   a2 count   (gaussian x macro-tile hits)    PAPER.md:85-107 (3.2), 251 (4.3)
+ *   a3 scan    (segment bounds, write bases)
+ *   a4 fill    ((depth key, id) pairs)
+ *   a5 segmented depth sort                    PAPER.md:109-117 (3.3), 259-276 (4.4)
+ *   a6 batch schedule (units of <= B_r)        PAPER.md:81 (3.1)
+ *   a7 macro-tile rasterizer                   PAPER.md:119-170 (3.4, Alg. 1-2), 278-284 (4.5)
+ *   a8 post-blend merge, Eq. (1)
+ * Every step runs in hand-written sm_100a kernels inside libhigs.so; there is no CPU fallback.
+ *
+ * Conventions
+ *   - "device pointer" = memory of the CUDA device the context was created on, owned by the
+ *     caller, contiguous fp32, never retained past the stream work of the call that got it.
+ *   - "host pointer"  = ordinary (preferably pinned) host memory.
+ *   - Inputs are *activated* 3DGS parameters: linear scales (> 0), opacities in [0,1],
+ *     quaternions (w,x,y,z) not necessarily normalised, SH as [N][K][3], K = (degree+1)^2,
+ *     in the convention of the public 3DGS models the paper renders.
+ *   - Camera frame: +x right, +y down, +z forward; pixel (i,j) has its centre at (i+0.5,j+0.5).
+ *   - Two-level grid: render tile 8x8 px; macro-tile = 8x4 render tiles = 64x32 px;
+ *     macro-tile id m = my*ceil(W/64) + mx; tile in macro-tile t = ty*8 + tx.
+ *   - All functions return HIGS_OK (0) or a negative higs_status; nothing throws.
+ *   - A context is not thread-safe; use one context per host thread / stream.
+ */
+#ifndef HIGS_H
+#define HIGS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HIGS_ABI_VERSION 1
+
+#define HIGS_TILE        8      /* render tile edge, px  */
+#define HIGS_MT_W        64     /* macro-tile width,  px (8 tiles)  */
+#define HIGS_MT_H        32     /* macro-tile height, px (4 tiles)  */
+#define HIGS_MT_TILES    32     /* M: render tiles per macro-tile  */
+#define HIGS_BATCH_CAP   1024   /* B_r: gaussians per rasterizer work unit  */
+#define HIGS_PART_BATCH  8192   /* B_p: gaussians per partitioning batch  */
+#define HIGS_SORT_BLOCK  8192   /* largest segment sorted by one CTA */
+
+typedef enum {
+    HIGS_OK          = 0,
+    HIGS_E_ARG       = -1,  /* null pointer, degree not in [0,3], W/H <= 0 or > max, N < 0 or > max */
+    HIGS_E_CUDA      = -2,  /* a CUDA call failed; text via higs_last_error()                       */
+    HIGS_E_CAPACITY  = -3,  /* the frame produced more pairs / units than the context was sized for;
+                               detected on the device, nothing is written out of bounds, the frame's
+                               image is then all zeros; reported by higs_get_stats / higs_get_lists  */
+    HIGS_E_NOMEM     = -4   /* host or device allocation failed                                     */
+} higs_status;
+
+/* Pinhole camera.  HOST memory, copied at call time.  20 floats, no padding. */
+typedef struct {
+    float view[12];   /* row-major 3x4 world->camera [R|t]                                        */
+    float fx, fy;     /* focal lengths, px                                                         */
+    float cx, cy;     /* principal point, px                                                       */
+    float near_z;     /* gaussians with z_cam <= near_z are culled (default 0.2)                   */
+    float cam_pos[3]; /* world-space camera centre (= -R^T t), used only for the SH view direction */
+} higs_camera;
+
+typedef struct higs_ctx higs_ctx;
+
+/* Frame statistics.  HOST struct filled by higs_get_stats (synchronises the render stream). */
+typedef struct {
+    int64_t n_gaussians;     /* N of the last render                                              */
+    int64_t n_visible;       /* gaussians surviving the cull                                      */
+    int64_t n_pairs;         /* (gaussian, macro-tile) pairs                  PAPER.md:97 Table 1 */
+    int64_t n_units;         /* N_R = sum_m ceil(n_m / B_r) rasterizer units         */
+    int64_t max_segment;     /* largest per-macro-tile list                                       */
+    int64_t n_oversize;      /* segments longer than HIGS_SORT_BLOCK (overflow path)*/
+    int32_t n_mt_x, n_mt_y;  /* macro-tile grid                                                   */
+    int32_t batch_cap;       /* B_r in effect                                                     */
+    int32_t overflow;        /* 1 if the frame hit HIGS_E_CAPACITY                                */
+    int64_t n_evals;         /* pixel-gaussian evaluations executed by the rasterizer; only
+                                counted when HIGS_FLAG_COUNT_EVALS is set, else 0                 */
+    int64_t n_tile_pairs;    /* (gaussian, render tile) pairs that passed the inline visibility
+                                test; only with HIGS_FLAG_COUNT_EVALS                             */
+    /* per-stage device time of the last frame, ms; only with HIGS_FLAG_STAGE_TIMERS, else 0     */
+    float ms_project, ms_count, ms_scan, ms_fill, ms_sort, ms_raster, ms_merge, ms_total;
+} higs_stats;
+
+/* The integer lists of the last frame (O-LIST).  DEVICE pointers owned by the context, valid
+ * until the next render on it.  higs_get_lists synchronises the render stream. */
+typedef struct {
+    int64_t n_pairs, n_units;
+    int32_t n_mt;                    /* N_M                                                       */
+    const uint32_t* mt_count;        /* [N_M]     pairs per macro-tile                            */
+    const uint32_t* mt_offset;       /* [N_M+1]   exclusive prefix sum = segment bounds           */
+    const uint32_t* batch_offset;    /* [N_M+1]   exclusive prefix sum of ceil(n_m/B_r)           */
+    const uint64_t* pairs;           /* [n_pairs] (key << 32 | id), each segment ascending        */
+    const uint32_t* unit_active;     /* [n_units] 32-bit active-tile mask per unit */
+} higs_lists;
+
+/* Per-gaussian records of the last frame.  DEVICE pointers owned by the context. */
+typedef struct {
+    int64_t n;
+    const uint32_t* valid_bits;      /* [ceil(N/32)] bit (i & 31) of word i/32 = gaussian i kept  */
+    const float*    geo;             /* [N][8]  mux, muy, a, b, c, tau, bits(key), unused; rows of
+                                        culled gaussians are not written                           */
+    const float*    ras;             /* [N][12] mux, muy, A, B2, C, tau, log2(o), r, g, b, 0, 0    */
+} higs_records;
+
+#define HIGS_FLAG_STAGE_TIMERS  1u   /* record CUDA events around every stage                     */
+#define HIGS_FLAG_COUNT_EVALS   2u   /* rasterizer counts evaluations (slower; for the roofline)  */
+#define HIGS_FLAG_NO_XBATCH_CUT 4u   /* disable the cross-batch saturation cut-off:
+                                        every unit then rasterizes every tile it touches          */
+
+/* Create a context on CUDA device `device` and preallocate all scratch (PAPER.md:83, 284:
+ * "preallocated up front").  max_pairs bounds N_pairs (<= 2^31-1; 0 selects 4*max_gaussians + 65536).
+ * Device memory taken: ~80 B/gaussian + 16 B/pair + 32 KB per unit (units <= N_M + max_pairs/1024). */
+int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, int max_H, int64_t max_pairs);
+void higs_destroy(higs_ctx* ctx);
+
+/* Runtime knobs: flags (HIGS_FLAG_*) and the rasterizer batch cap B_r in [1, 1024]
+ * (tests use small B_r to force many batches per macro-tile; the paper's value is 1024). */
+int higs_set_flags(higs_ctx* ctx, uint32_t flags);
+int higs_set_batch_cap(higs_ctx* ctx, int batch_cap);
+
+/* Render one frame.  All array arguments are DEVICE pointers:
+ *   means [N][3], scales [N][3], quats [N][4], opacities [N], sh [N][(degree+1)^2][3],
+ *   out_rgb [H][W][3] fp32, black background, no clamp / gamma.
+ * cam is a HOST pointer.  cuda_stream is a cudaStream_t (NULL = legacy default stream).
+ * Only enqueues work: no host synchronisation, no allocation, so the call may
+ * be captured into a CUDA graph.  N = 0 is valid (image = 0). */
+int higs_render(higs_ctx* ctx, const float* means, const float* scales, const float* quats,
+                const float* opacities, const float* sh, int degree, int64_t N,
+                const higs_camera* cam, int W, int H, float* out_rgb, void* cuda_stream);
+
+/* Same frame with HOST buffers: uploads the five arrays, renders, downloads the image into the
+ * host buffer out_rgb and synchronises.  Staging device buffers are owned by the context. */
+int higs_render_host(higs_ctx* ctx, const float* means, const float* scales, const float* quats,
+                     const float* opacities, const float* sh, int degree, int64_t N,
+                     const higs_camera* cam, int W, int H, float* out_rgb);
+
+/* Resident-scene path for view loops: upload once (HOST pointers), then per view copy the camera
+ * in and the image out (HOST pointer out_rgb, pinned for full speed) and synchronise. */
+int higs_scene_upload(higs_ctx* ctx, const float* means, const float* scales, const float* quats,
+                      const float* opacities, const float* sh, int degree, int64_t N);
+int higs_render_view_host(higs_ctx* ctx, const higs_camera* cam, int W, int H, float* out_rgb);
+/* Resident-scene path with a DEVICE image (no download, no synchronisation). */
+int higs_render_view(higs_ctx* ctx, const higs_camera* cam, int W, int H, float* out_rgb, void* cuda_stream);
+
+int higs_get_stats(higs_ctx* ctx, higs_stats* out);
+int higs_get_lists(higs_ctx* ctx, higs_lists* out);
+int higs_get_records(higs_ctx* ctx, higs_records* out);
+
+/* Stage-isolation entry point for tests ("teacher forcing", a5 alone): sorts every segment
+ * [seg_offset[s], seg_offset[s+1]) of the DEVICE array pairs (n_seg segments, 64-bit
+ * (key << 32 | id) items) ascending, in place, with the frame's own sort kernels. */
+int higs_sort_segments(higs_ctx* ctx, uint64_t* pairs, const uint32_t* seg_offset, int32_t n_seg,
+                       void* cuda_stream);
+
+/* Utility: synchronise the last render stream and copy `bytes` from a DEVICE pointer handed out by
+ * higs_get_lists / higs_get_records into HOST memory. */
+int higs_download(higs_ctx* ctx, const void* device_src, void* host_dst, uint64_t bytes);
+
+const char* higs_strerror(int status);
+const char* higs_last_error(higs_ctx* ctx);   /* text of the last HIGS_E_CUDA on this context */
+int higs_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HIGS_H */

@@ -1,0 +1,359 @@
+// api.cu -- the C ABI of include/higs.h: context, frame orchestration, stats.  Host code only
+// enqueues kernels; every data-dependent size stays on the device.
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+#include "higs_internal.cuh"
+
+int higs_binning_smem_setup(higs_ctx*);
+int higs_sort_smem_setup(higs_ctx*);
+int higs_raster_setup(higs_ctx*);
+
+namespace {
+
+template <typename T>
+int dev_alloc(higs_ctx* ctx, T** p, size_t count)
+{
+    void* q = nullptr;
+    cudaError_t e = cudaMalloc(&q, (count ? count : 1) * sizeof(T));
+    if (e != cudaSuccess) {
+        snprintf(ctx->err, sizeof(ctx->err), "cudaMalloc(%zu B): %s", count * sizeof(T), cudaGetErrorString(e));
+        cudaGetLastError();
+        return HIGS_E_NOMEM;
+    }
+    *p = static_cast<T*>(q);
+    return HIGS_OK;
+}
+
+template <typename T> void dev_free(T*& p) { if (p) cudaFree(p); p = nullptr; }
+
+int alloc_unit_buffers(higs_ctx* ctx)
+{
+    dev_free(ctx->unit_mt); dev_free(ctx->unit_active); dev_free(ctx->partial); dev_free(ctx->tile_maxT);
+    ctx->max_units = ctx->max_nm + (ctx->max_pairs + ctx->batch_cap - 1) / ctx->batch_cap + 1;
+    int rc;
+    if ((rc = dev_alloc(ctx, &ctx->unit_mt, (size_t)ctx->max_units))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->unit_active, (size_t)ctx->max_units))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->partial, (size_t)ctx->max_units * HIGS_MT_TILES * 64))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->tile_maxT, (size_t)ctx->max_units * HIGS_MT_TILES))) return rc;
+    return HIGS_OK;
+}
+
+int check_frame_args(higs_ctx* ctx, int degree, int64_t N, const higs_camera* cam, int W, int H, const void* out)
+{
+    if (!ctx || !cam || !out) return HIGS_E_ARG;
+    if (degree < 0 || degree > 3) return HIGS_E_ARG;
+    if (N < 0 || N > ctx->max_gaussians) return HIGS_E_ARG;
+    if (W <= 0 || H <= 0 || W > ctx->max_W || H > ctx->max_H) return HIGS_E_ARG;
+    const int64_t nm = (int64_t)((W + HIGS_MT_W - 1) / HIGS_MT_W) * ((H + HIGS_MT_H - 1) / HIGS_MT_H);
+    if (nm > ctx->max_nm) return HIGS_E_ARG;
+    return HIGS_OK;
+}
+
+int render_impl(higs_ctx* ctx, const float* means, const float* scales, const float* quats, const float* opac,
+                const float* sh, int degree, int64_t N, const higs_camera* cam, int W, int H, float* out_rgb,
+                cudaStream_t st)
+{
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    FrameParams P;
+    memcpy(P.V, cam->view, sizeof(P.V));
+    P.fx = cam->fx; P.fy = cam->fy; P.cx = cam->cx; P.cy = cam->cy; P.near_z = cam->near_z;
+    memcpy(P.cam, cam->cam_pos, sizeof(P.cam));
+    P.W = W; P.H = H;
+    P.n_mx = (W + HIGS_MT_W - 1) / HIGS_MT_W; P.n_my = (H + HIGS_MT_H - 1) / HIGS_MT_H; P.n_m = P.n_mx * P.n_my;
+    P.degree = degree; P.batch_cap = ctx->batch_cap; P.flags = ctx->flags;
+    P.max_pairs = (uint32_t)ctx->max_pairs; P.max_units = (uint32_t)ctx->max_units;
+    const bool timers = (ctx->flags & HIGS_FLAG_STAGE_TIMERS) != 0;
+    cudaEvent_t* ev = ctx->ev;
+    int rc;
+
+    HIGS_CUDA(ctx, cudaMemsetAsync(ctx->hdr, 0, sizeof(FrameHeader), st));
+    if (!(ctx->flags & HIGS_FLAG_NO_XBATCH_CUT))
+        HIGS_CUDA(ctx, cudaMemsetAsync(ctx->tile_maxT, 0, sizeof(float) * (size_t)ctx->max_units * HIGS_MT_TILES, st));
+    if (timers) cudaEventRecord(ev[0], st);
+    if ((rc = launch_project(ctx, P, means, scales, quats, opac, sh, N, st))) return rc;
+    if (timers) cudaEventRecord(ev[1], st);
+    if ((rc = launch_binning(ctx, P, N, st, timers ? ev[2] : nullptr, timers ? ev[3] : nullptr))) return rc;
+    if (timers) cudaEventRecord(ev[4], st);
+    if ((rc = launch_sort(ctx, P, st))) return rc;
+    if (timers) cudaEventRecord(ev[5], st);
+    if ((rc = launch_raster(ctx, P, st))) return rc;
+    if (timers) cudaEventRecord(ev[6], st);
+    if ((rc = launch_merge(ctx, P, out_rgb, st))) return rc;
+    if (timers) cudaEventRecord(ev[7], st);
+    ctx->timers_valid = timers;
+    ctx->last_n = N; ctx->last_W = W; ctx->last_H = H; ctx->last_nm = P.n_m; ctx->last_mx = P.n_mx; ctx->last_my = P.n_my;
+    ctx->last_stream = st;
+    return HIGS_OK;
+}
+
+int fetch_header(higs_ctx* ctx)
+{
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    HIGS_CUDA(ctx, cudaStreamSynchronize(ctx->last_stream));
+    HIGS_CUDA(ctx, cudaMemcpy(ctx->hdr_host, ctx->hdr, sizeof(FrameHeader), cudaMemcpyDeviceToHost));
+    return HIGS_OK;
+}
+
+int ensure_scene_capacity(higs_ctx* ctx, int64_t N, int K)
+{
+    if (N <= ctx->s_cap_n && K <= ctx->s_cap_k) return HIGS_OK;
+    dev_free(ctx->s_means); dev_free(ctx->s_scales); dev_free(ctx->s_quats); dev_free(ctx->s_opac); dev_free(ctx->s_sh);
+    const int64_t cap = N > ctx->s_cap_n ? N : ctx->s_cap_n;
+    const int kk = K > ctx->s_cap_k ? K : ctx->s_cap_k;
+    ctx->s_cap_n = 0; ctx->s_cap_k = 0;
+    int rc;
+    if ((rc = dev_alloc(ctx, &ctx->s_means, (size_t)cap * 3))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->s_scales, (size_t)cap * 3))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->s_quats, (size_t)cap * 4))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->s_opac, (size_t)cap))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->s_sh, (size_t)cap * kk * 3))) return rc;
+    ctx->s_cap_n = cap; ctx->s_cap_k = kk;
+    return HIGS_OK;
+}
+
+int ensure_image_capacity(higs_ctx* ctx, int W, int H)
+{
+    const int64_t need = (int64_t)W * H * 3;
+    if (need <= ctx->s_img_cap) return HIGS_OK;
+    dev_free(ctx->s_img); ctx->s_img_cap = 0;
+    int rc;
+    if ((rc = dev_alloc(ctx, &ctx->s_img, (size_t)need))) return rc;
+    ctx->s_img_cap = need;
+    return HIGS_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int higs_abi_version(void) { return HIGS_ABI_VERSION; }
+
+const char* higs_strerror(int status)
+{
+    switch (status) {
+        case HIGS_OK: return "ok";
+        case HIGS_E_ARG: return "invalid argument";
+        case HIGS_E_CUDA: return "CUDA error (see higs_last_error)";
+        case HIGS_E_CAPACITY: return "frame exceeded the preallocated pair / unit capacity";
+        case HIGS_E_NOMEM: return "out of memory";
+        default: return "unknown status";
+    }
+}
+
+const char* higs_last_error(higs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, int max_H, int64_t max_pairs)
+{
+    if (!out) return HIGS_E_ARG;
+    *out = nullptr;
+    if (max_gaussians < 0 || max_gaussians > 0xfffffff0ll || max_W <= 0 || max_H <= 0) return HIGS_E_ARG;
+    if (max_pairs <= 0) max_pairs = 4 * max_gaussians + 65536;
+    if (max_pairs > 0x7fffffffll) return HIGS_E_ARG;
+    const int64_t nm = (int64_t)((max_W + HIGS_MT_W - 1) / HIGS_MT_W) * ((max_H + HIGS_MT_H - 1) / HIGS_MT_H);
+    if (nm > HIGS_MAX_NM) return HIGS_E_ARG;
+    higs_ctx* ctx = new (std::nothrow) higs_ctx();
+    if (!ctx) return HIGS_E_NOMEM;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->device = device; ctx->max_gaussians = max_gaussians; ctx->max_W = max_W; ctx->max_H = max_H;
+    ctx->max_nm = (int)nm; ctx->max_pairs = max_pairs; ctx->batch_cap = HIGS_BATCH_CAP; ctx->flags = 0;
+    int rc = HIGS_OK;
+    auto fail = [&](int code) { higs_destroy(ctx); return code; };
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return fail(HIGS_E_CUDA); }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(HIGS_E_CUDA);
+    ctx->n_sm = prop.multiProcessorCount;
+    const int64_t n = max_gaussians > 0 ? max_gaussians : 1;
+    ctx->n_part_batches_max = (int)((n + HIGS_PART_BATCH - 1) / HIGS_PART_BATCH);
+    const int n_groups_max = (ctx->n_part_batches_max + 31) / 32;
+    const size_t pitch = ((size_t)nm + 1) & ~(size_t)1;
+    if ((rc = dev_alloc(ctx, &ctx->valid_bits, (size_t)(n + 31) / 32 + 1))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->geo, (size_t)n * 2))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->ras, (size_t)n * 3))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->hist, (size_t)ctx->n_part_batches_max * pitch))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->base, (size_t)(ctx->n_part_batches_max + n_groups_max) * nm))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->mt_count, (size_t)nm + 1))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->mt_offset, (size_t)nm + 1))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->batch_offset, (size_t)nm + 1))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->pairs, (size_t)max_pairs))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->pairs_alt, (size_t)max_pairs))) return fail(rc);
+    ctx->max_jobs = nm + max_pairs / HIGS_SORT_BLOCK + 2;
+    ctx->max_over = max_pairs / HIGS_SORT_BLOCK + 1;
+    if ((rc = dev_alloc(ctx, &ctx->sort_jobs, (size_t)ctx->max_jobs * HIGS_N_TIERS))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->over_segs, (size_t)ctx->max_over))) return fail(rc);
+    if ((rc = alloc_unit_buffers(ctx))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->hdr, 1))) return fail(rc);
+    if (cudaMallocHost((void**)&ctx->hdr_host, sizeof(FrameHeader)) != cudaSuccess) return fail(HIGS_E_NOMEM);
+    if (cudaMemset(ctx->hdr, 0, sizeof(FrameHeader)) != cudaSuccess) return fail(HIGS_E_CUDA);
+    memset(ctx->hdr_host, 0, sizeof(FrameHeader));
+    if (cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(HIGS_E_CUDA);
+    for (int i = 0; i < 9; ++i) if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) return fail(HIGS_E_CUDA);
+    if ((rc = higs_binning_smem_setup(ctx))) return fail(rc);
+    if ((rc = higs_sort_smem_setup(ctx))) return fail(rc);
+    if ((rc = higs_raster_setup(ctx))) return fail(rc);
+    ctx->last_stream = ctx->own_stream;
+    *out = ctx;
+    return HIGS_OK;
+}
+
+void higs_destroy(higs_ctx* ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    dev_free(ctx->valid_bits); dev_free(ctx->geo); dev_free(ctx->ras); dev_free(ctx->hist); dev_free(ctx->base);
+    dev_free(ctx->mt_count); dev_free(ctx->mt_offset); dev_free(ctx->batch_offset); dev_free(ctx->unit_mt);
+    dev_free(ctx->unit_active); dev_free(ctx->pairs); dev_free(ctx->pairs_alt); dev_free(ctx->sort_jobs);
+    dev_free(ctx->over_segs); dev_free(ctx->partial); dev_free(ctx->tile_maxT); dev_free(ctx->hdr);
+    dev_free(ctx->s_means); dev_free(ctx->s_scales); dev_free(ctx->s_quats); dev_free(ctx->s_opac); dev_free(ctx->s_sh);
+    dev_free(ctx->s_img);
+    if (ctx->hdr_host) cudaFreeHost(ctx->hdr_host);
+    if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    for (int i = 0; i < 9; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    cudaGetLastError();
+    delete ctx;
+}
+
+int higs_set_flags(higs_ctx* ctx, uint32_t flags)
+{
+    if (!ctx) return HIGS_E_ARG;
+    ctx->flags = flags;
+    return HIGS_OK;
+}
+
+int higs_set_batch_cap(higs_ctx* ctx, int batch_cap)
+{
+    if (!ctx || batch_cap < 1 || batch_cap > HIGS_BATCH_CAP) return HIGS_E_ARG;
+    if (batch_cap == ctx->batch_cap) return HIGS_OK;
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    HIGS_CUDA(ctx, cudaDeviceSynchronize());
+    ctx->batch_cap = batch_cap;
+    return alloc_unit_buffers(ctx);
+}
+
+int higs_render(higs_ctx* ctx, const float* means, const float* scales, const float* quats, const float* opacities,
+                const float* sh, int degree, int64_t N, const higs_camera* cam, int W, int H, float* out_rgb,
+                void* cuda_stream)
+{
+    int rc = check_frame_args(ctx, degree, N, cam, W, H, out_rgb);
+    if (rc) return rc;
+    if (N > 0 && (!means || !scales || !quats || !opacities || !sh)) return HIGS_E_ARG;
+    return render_impl(ctx, means, scales, quats, opacities, sh, degree, N, cam, W, H, out_rgb, (cudaStream_t)cuda_stream);
+}
+
+int higs_scene_upload(higs_ctx* ctx, const float* means, const float* scales, const float* quats,
+                      const float* opacities, const float* sh, int degree, int64_t N)
+{
+    if (!ctx || degree < 0 || degree > 3 || N < 0 || N > ctx->max_gaussians) return HIGS_E_ARG;
+    if (N > 0 && (!means || !scales || !quats || !opacities || !sh)) return HIGS_E_ARG;
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    const int K = (degree + 1) * (degree + 1);
+    int rc = ensure_scene_capacity(ctx, N > 0 ? N : 1, K);
+    if (rc) return rc;
+    cudaStream_t st = ctx->own_stream;
+    if (N > 0) {
+        HIGS_CUDA(ctx, cudaMemcpyAsync(ctx->s_means, means, sizeof(float) * 3 * N, cudaMemcpyHostToDevice, st));
+        HIGS_CUDA(ctx, cudaMemcpyAsync(ctx->s_scales, scales, sizeof(float) * 3 * N, cudaMemcpyHostToDevice, st));
+        HIGS_CUDA(ctx, cudaMemcpyAsync(ctx->s_quats, quats, sizeof(float) * 4 * N, cudaMemcpyHostToDevice, st));
+        HIGS_CUDA(ctx, cudaMemcpyAsync(ctx->s_opac, opacities, sizeof(float) * N, cudaMemcpyHostToDevice, st));
+        HIGS_CUDA(ctx, cudaMemcpyAsync(ctx->s_sh, sh, sizeof(float) * 3 * K * N, cudaMemcpyHostToDevice, st));
+    }
+    HIGS_CUDA(ctx, cudaStreamSynchronize(st));
+    ctx->s_n = N; ctx->s_degree = degree;
+    return HIGS_OK;
+}
+
+int higs_render_view(higs_ctx* ctx, const higs_camera* cam, int W, int H, float* out_rgb, void* cuda_stream)
+{
+    if (!ctx) return HIGS_E_ARG;
+    int rc = check_frame_args(ctx, ctx->s_degree, ctx->s_n, cam, W, H, out_rgb);
+    if (rc) return rc;
+    return render_impl(ctx, ctx->s_means, ctx->s_scales, ctx->s_quats, ctx->s_opac, ctx->s_sh, ctx->s_degree, ctx->s_n,
+                       cam, W, H, out_rgb, (cudaStream_t)cuda_stream);
+}
+
+int higs_render_view_host(higs_ctx* ctx, const higs_camera* cam, int W, int H, float* out_rgb)
+{
+    if (!ctx) return HIGS_E_ARG;
+    int rc = check_frame_args(ctx, ctx->s_degree, ctx->s_n, cam, W, H, out_rgb);
+    if (rc) return rc;
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    if ((rc = ensure_image_capacity(ctx, W, H))) return rc;
+    cudaStream_t st = ctx->own_stream;
+    rc = render_impl(ctx, ctx->s_means, ctx->s_scales, ctx->s_quats, ctx->s_opac, ctx->s_sh, ctx->s_degree, ctx->s_n,
+                     cam, W, H, ctx->s_img, st);
+    if (rc) return rc;
+    HIGS_CUDA(ctx, cudaMemcpyAsync(out_rgb, ctx->s_img, sizeof(float) * 3 * (size_t)W * H, cudaMemcpyDeviceToHost, st));
+    HIGS_CUDA(ctx, cudaStreamSynchronize(st));
+    return HIGS_OK;
+}
+
+int higs_render_host(higs_ctx* ctx, const float* means, const float* scales, const float* quats, const float* opacities,
+                     const float* sh, int degree, int64_t N, const higs_camera* cam, int W, int H, float* out_rgb)
+{
+    int rc = check_frame_args(ctx, degree, N, cam, W, H, out_rgb);
+    if (rc) return rc;
+    if ((rc = higs_scene_upload(ctx, means, scales, quats, opacities, sh, degree, N))) return rc;
+    return higs_render_view_host(ctx, cam, W, H, out_rgb);
+}
+
+int higs_get_stats(higs_ctx* ctx, higs_stats* out)
+{
+    if (!ctx || !out) return HIGS_E_ARG;
+    int rc = fetch_header(ctx);
+    if (rc) return rc;
+    const FrameHeader& h = *ctx->hdr_host;
+    memset(out, 0, sizeof(*out));
+    out->n_gaussians = ctx->last_n; out->n_visible = h.n_visible; out->n_pairs = h.n_pairs; out->n_units = h.n_units;
+    out->max_segment = h.max_segment; out->n_oversize = h.n_oversize;
+    out->n_mt_x = ctx->last_mx; out->n_mt_y = ctx->last_my; out->batch_cap = ctx->batch_cap; out->overflow = (int32_t)h.overflow;
+    out->n_evals = (int64_t)h.n_evals; out->n_tile_pairs = (int64_t)h.n_tile_pairs;
+    if (ctx->timers_valid) {
+        float* dst[7] = { &out->ms_project, &out->ms_count, &out->ms_scan, &out->ms_fill, &out->ms_sort, &out->ms_raster, &out->ms_merge };
+        for (int i = 0; i < 7; ++i) HIGS_CUDA(ctx, cudaEventElapsedTime(dst[i], ctx->ev[i], ctx->ev[i + 1]));
+        HIGS_CUDA(ctx, cudaEventElapsedTime(&out->ms_total, ctx->ev[0], ctx->ev[7]));
+    }
+    return h.overflow ? HIGS_E_CAPACITY : HIGS_OK;
+}
+
+int higs_get_lists(higs_ctx* ctx, higs_lists* out)
+{
+    if (!ctx || !out) return HIGS_E_ARG;
+    int rc = fetch_header(ctx);
+    if (rc) return rc;
+    const FrameHeader& h = *ctx->hdr_host;
+    out->n_pairs = h.n_pairs; out->n_units = h.n_units; out->n_mt = ctx->last_nm;
+    out->mt_count = ctx->mt_count; out->mt_offset = ctx->mt_offset; out->batch_offset = ctx->batch_offset;
+    out->pairs = reinterpret_cast<const uint64_t*>(ctx->pairs); out->unit_active = ctx->unit_active;
+    return h.overflow ? HIGS_E_CAPACITY : HIGS_OK;
+}
+
+int higs_get_records(higs_ctx* ctx, higs_records* out)
+{
+    if (!ctx || !out) return HIGS_E_ARG;
+    int rc = fetch_header(ctx);
+    if (rc) return rc;
+    out->n = ctx->last_n; out->valid_bits = ctx->valid_bits;
+    out->geo = reinterpret_cast<const float*>(ctx->geo); out->ras = reinterpret_cast<const float*>(ctx->ras);
+    return HIGS_OK;
+}
+
+int higs_download(higs_ctx* ctx, const void* device_src, void* host_dst, uint64_t bytes)
+{
+    if (!ctx || (bytes && (!device_src || !host_dst))) return HIGS_E_ARG;
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    HIGS_CUDA(ctx, cudaStreamSynchronize(ctx->last_stream));
+    if (bytes) HIGS_CUDA(ctx, cudaMemcpy(host_dst, device_src, (size_t)bytes, cudaMemcpyDeviceToHost));
+    return HIGS_OK;
+}
+
+int higs_sort_segments(higs_ctx* ctx, uint64_t* pairs, const uint32_t* seg_offset, int32_t n_seg, void* cuda_stream)
+{
+    if (!ctx || !pairs || !seg_offset || n_seg < 0 || n_seg > ctx->max_nm) return HIGS_E_ARG;
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    ctx->last_stream = (cudaStream_t)cuda_stream;
+    return launch_sort_only(ctx, reinterpret_cast<unsigned long long*>(pairs), seg_offset, n_seg, (cudaStream_t)cuda_stream);
+}
+
+} // extern "C"

@@ -1,0 +1,234 @@
+// binning.cu -- steps a2 count, a3 scan, a4 fill, a6 batch schedule (section 3.2,
+// PAPER.md:247-257 section 4.3, section 3.1).
+//
+// Count and fill each run one CTA per partitioning batch of B_p = 8192 consecutive gaussian ids
+// (PAPER.md:89, 251); both consume the per-warp visibility bitfield of a1, so culled gaussians never
+// reach the intersection test.  The count CTA keeps a private shared-memory histogram
+// with one counter per macro-tile and flushes it as uint16 (a cell holds <= 8192) into the
+// N_B x N_M matrix; the scan widens it to 32-bit write bases in two levels (groups of 32 batches);
+// the fill CTA replays the intersection and drops (depth key << 32 | id) at base + local rank.
+// The intersection is the row scan N-SCAN: bit-exact with the oracle.
+#include <stdio.h>
+#include "higs_internal.cuh"
+
+namespace {
+
+constexpr int BIN_THREADS = 512;
+constexpr int SCAN_GROUP  = 32;      // batches per first-level scan group
+
+// visit every macro-tile the threshold ellipse of gaussian i touches
+template <typename F>
+__device__ __forceinline__ void for_each_macro_tile(const float4* __restrict__ geo, int64_t i, const FrameParams& P, F&& f)
+{
+    const float4 g0 = geo[2 * i], g1 = geo[2 * i + 1];
+    RowScan rs;
+    rs.init(g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, (float)HIGS_MT_H, P.n_my);
+    const float fW = (float)P.W, fH = (float)P.H;
+    for (int r = rs.r0; r <= rs.r1; ++r) {
+        int m0, m1;
+        if (!rs.row(r, (float)HIGS_MT_W, (float)HIGS_MT_H, fW, fH, P.n_mx, m0, m1)) continue;
+        for (int m = m0; m <= m1; ++m) f(r * P.n_mx + m, __float_as_uint(g1.z));
+    }
+}
+
+__global__ void __launch_bounds__(BIN_THREADS)
+k_count(const uint32_t* __restrict__ valid_bits, const float4* __restrict__ geo, int64_t N, const FrameParams P,
+        uint16_t* __restrict__ hist, int pitch, FrameHeader* __restrict__ hdr)
+{
+    extern __shared__ uint32_t s_hist[];
+    __shared__ uint32_t s_nvis;
+    for (int m = threadIdx.x; m < P.n_m; m += BIN_THREADS) s_hist[m] = 0;
+    if (threadIdx.x == 0) s_nvis = 0;
+    __syncthreads();
+    const int64_t i0 = (int64_t)blockIdx.x * HIGS_PART_BATCH;
+    uint32_t nvis = 0;
+    for (int k = 0; k < HIGS_PART_BATCH / BIN_THREADS; ++k) {
+        const int64_t i = i0 + k * BIN_THREADS + threadIdx.x;
+        if (i >= N) break;
+        if (!((valid_bits[i >> 5] >> (i & 31)) & 1u)) continue;
+        ++nvis;
+        for_each_macro_tile(geo, i, P, [&](int cell, uint32_t) { atomicAdd(&s_hist[cell], 1u); });
+    }
+    nvis = __reduce_add_sync(0xffffffffu, nvis);
+    if ((threadIdx.x & 31) == 0 && nvis) atomicAdd(&s_nvis, nvis);
+    __syncthreads();
+    uint32_t* row = reinterpret_cast<uint32_t*>(hist + (size_t)blockIdx.x * pitch);   // pitch is even
+    for (int m2 = threadIdx.x; m2 < pitch / 2; m2 += BIN_THREADS) {
+        const int m = 2 * m2;
+        const uint32_t lo = s_hist[m], hi = (m + 1 < P.n_m) ? s_hist[m + 1] : 0u;
+        row[m2] = lo | (hi << 16);
+    }
+    if (threadIdx.x == 0 && s_nvis) atomicAdd(&hdr->n_visible, s_nvis);
+}
+
+// First scan level: CTA (column chunk, group) walks its <= 32 batches; base[b][m] = pairs of
+// macro-tile m in the earlier batches of the same group; gsum[g][m] = total of the group.
+__global__ void __launch_bounds__(256)
+k_scan_groups(const uint16_t* __restrict__ hist, int pitch, int n_batches, int n_m,
+              uint32_t* __restrict__ base, uint32_t* __restrict__ gsum)
+{
+    const int m = blockIdx.x * 256 + threadIdx.x;
+    const int g = blockIdx.y;
+    if (m >= n_m) return;
+    const int b0 = g * SCAN_GROUP, b1 = min(n_batches, b0 + SCAN_GROUP);
+    uint32_t run = 0;
+#pragma unroll 8
+    for (int b = b0; b < b1; ++b) {
+        const uint32_t h = hist[(size_t)b * pitch + m];
+        base[(size_t)b * n_m + m] = run;
+        run += h;
+    }
+    gsum[(size_t)g * n_m + m] = run;
+}
+
+// exclusive block scan of NV values per thread position (1024 threads), with a running carry
+template <int NV>
+__device__ __forceinline__ void block_scan_excl(uint32_t (&v)[NV], uint32_t (&carry)[NV], uint32_t* s_warp /* [32*NV] */)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    uint32_t incl[NV];
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+        uint32_t x = v[q];
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
+        incl[q] = x;
+        if (lane == 31) s_warp[wid * NV + q] = x;
+    }
+    __syncthreads();
+    if (wid == 0) {
+#pragma unroll
+        for (int q = 0; q < NV; ++q) {
+            uint32_t x = s_warp[lane * NV + q];
+            uint32_t t = x;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, t, d); if (lane >= d) t += y; }
+            s_warp[lane * NV + q] = t - x;               // exclusive warp base
+            if (lane == 31) s_warp[32 * NV + q] = t;     // block total
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+        const uint32_t excl = carry[q] + s_warp[wid * NV + q] + incl[q] - v[q];
+        carry[q] += s_warp[32 * NV + q];
+        v[q] = excl;
+    }
+    __syncthreads();
+}
+
+// Second scan level + batch schedule (a6), one CTA of 1024 threads:
+//   gbase[g][m] = exclusive scan of gsum over g; mt_count[m]; mt_offset = exclusive scan over m;
+//   nb[m] = ceil(n_m / B_r); batch_offset = exclusive scan; unit_mt[u] = m.
+__global__ void __launch_bounds__(1024)
+k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, const FrameParams P,
+       uint32_t* __restrict__ mt_count, uint32_t* __restrict__ mt_offset, uint32_t* __restrict__ batch_offset,
+       uint32_t* __restrict__ unit_mt, FrameHeader* __restrict__ hdr)
+{
+    __shared__ uint32_t s_warp[33 * 2];
+    __shared__ uint32_t s_max;
+    if (threadIdx.x == 0) s_max = 0;
+    uint32_t carry[2] = {0, 0};
+    const uint32_t br = (uint32_t)P.batch_cap;
+    // pass 1: totals and offsets
+    for (int m0 = 0; m0 < P.n_m; m0 += 1024) {
+        const int m = m0 + threadIdx.x;
+        uint32_t n = 0;
+        if (m < P.n_m) {
+            for (int g = 0; g < n_groups; ++g) {
+                const uint32_t s = gsum[(size_t)g * P.n_m + m];
+                gsum[(size_t)g * P.n_m + m] = n;
+                n += s;
+            }
+            mt_count[m] = n;
+            if (n) atomicMax(&s_max, n);
+        }
+        uint32_t v[2] = { n, (n + br - 1) / br };
+        block_scan_excl<2>(v, carry, s_warp);
+        if (m < P.n_m) { mt_offset[m] = v[0]; batch_offset[m] = v[1]; }
+    }
+    __syncthreads();
+    const uint32_t n_pairs = carry[0], n_units = carry[1];
+    const bool overflow = n_pairs > P.max_pairs || n_units > P.max_units;
+    if (threadIdx.x == 0) {
+        mt_offset[P.n_m] = n_pairs; batch_offset[P.n_m] = n_units;
+        hdr->n_pairs = overflow ? 0u : n_pairs;
+        hdr->n_units = overflow ? 0u : n_units;
+        hdr->overflow = overflow ? 1u : 0u;
+        hdr->max_segment = s_max;
+    }
+    if (overflow) return;
+    // pass 2: unit table
+    for (int m = threadIdx.x; m < P.n_m; m += 1024) {
+        const uint32_t u0 = batch_offset[m], nb = (mt_count[m] + br - 1) / br;
+        for (uint32_t j = 0; j < nb; ++j) unit_mt[u0 + j] = (uint32_t)m;
+    }
+}
+
+__global__ void __launch_bounds__(BIN_THREADS)
+k_fill(const uint32_t* __restrict__ valid_bits, const float4* __restrict__ geo, int64_t N, const FrameParams P,
+       const uint32_t* __restrict__ base, const uint32_t* __restrict__ gbase, const uint32_t* __restrict__ mt_offset,
+       unsigned long long* __restrict__ pairs, const FrameHeader* __restrict__ hdr)
+{
+    extern __shared__ uint32_t s_cursor[];
+    if (hdr->overflow) return;                      // capacity exceeded: write nothing (HIGS_E_CAPACITY)
+    const int b = blockIdx.x, g = b / SCAN_GROUP;
+    for (int m = threadIdx.x; m < P.n_m; m += BIN_THREADS)
+        s_cursor[m] = mt_offset[m] + gbase[(size_t)g * P.n_m + m] + base[(size_t)b * P.n_m + m];
+    __syncthreads();
+    const int64_t i0 = (int64_t)b * HIGS_PART_BATCH;
+    for (int k = 0; k < HIGS_PART_BATCH / BIN_THREADS; ++k) {
+        const int64_t i = i0 + k * BIN_THREADS + threadIdx.x;
+        if (i >= N) break;
+        if (!((valid_bits[i >> 5] >> (i & 31)) & 1u)) continue;
+        for_each_macro_tile(geo, i, P, [&](int cell, uint32_t key) {
+            const uint32_t pos = atomicAdd(&s_cursor[cell], 1u);
+            pairs[pos] = ((unsigned long long)key << 32) | (unsigned long long)(uint32_t)i;
+        });
+    }
+}
+
+__global__ void k_zero_lists(uint32_t* mt_count, uint32_t* mt_offset, uint32_t* batch_offset, int n_m)
+{
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m < n_m) mt_count[m] = 0;
+    if (m <= n_m) { mt_offset[m] = 0; batch_offset[m] = 0; }
+}
+
+} // namespace
+
+int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t st, cudaEvent_t ev_count, cudaEvent_t ev_scan)
+{
+    const int n_b = (int)((N + HIGS_PART_BATCH - 1) / HIGS_PART_BATCH);
+    const int pitch = (P.n_m + 1) & ~1;
+    if (n_b == 0) {
+        k_zero_lists<<<(P.n_m + 256) / 256, 256, 0, st>>>(ctx->mt_count, ctx->mt_offset, ctx->batch_offset, P.n_m);
+        HIGS_CUDA(ctx, cudaGetLastError());
+        if (ev_count) { cudaEventRecord(ev_count, st); cudaEventRecord(ev_scan, st); }
+        return HIGS_OK;
+    }
+    const size_t smem = sizeof(uint32_t) * (size_t)P.n_m;
+    k_count<<<n_b, BIN_THREADS, smem, st>>>(ctx->valid_bits, ctx->geo, N, P, ctx->hist, pitch, ctx->hdr);
+    HIGS_CUDA(ctx, cudaGetLastError());
+    if (ev_count) cudaEventRecord(ev_count, st);
+    const int n_groups = (n_b + SCAN_GROUP - 1) / SCAN_GROUP;
+    uint32_t* gsum = ctx->base + (size_t)ctx->n_part_batches_max * ctx->max_nm;   // tail of the base allocation
+    k_scan_groups<<<dim3((P.n_m + 255) / 256, n_groups), 256, 0, st>>>(ctx->hist, pitch, n_b, P.n_m, ctx->base, gsum);
+    HIGS_CUDA(ctx, cudaGetLastError());
+    k_plan<<<1, 1024, 0, st>>>(gsum, n_groups, P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->unit_mt, ctx->hdr);
+    HIGS_CUDA(ctx, cudaGetLastError());
+    if (ev_scan) cudaEventRecord(ev_scan, st);
+    k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->valid_bits, ctx->geo, N, P, ctx->base, gsum, ctx->mt_offset, ctx->pairs, ctx->hdr);
+    HIGS_CUDA(ctx, cudaGetLastError());
+    return HIGS_OK;
+}
+
+int higs_binning_smem_setup(higs_ctx* ctx)
+{
+    const int bytes = (int)(sizeof(uint32_t) * (size_t)ctx->max_nm);
+    if (bytes > 48 * 1024) {
+        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_count, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    }
+    return HIGS_OK;
+}

@@ -1,0 +1,148 @@
+// higs_internal.cuh -- context layout, constants and small device helpers shared by the
+// kernels of libhigs.so.  Nothing here is visible through the C ABI (include/higs.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/higs.h"
+
+#define HIGS_EPS_T      1e-4f        // transmittance threshold, reading Q1
+#define HIGS_ALPHA_MAX  0.99f
+#define HIGS_MAX_NM     32768        // macro-tiles per frame the shared-memory histograms are sized for
+#define HIGS_N_TIERS    4            // block-sort tiers, capacities 1024 / 2048 / 4096 / 8192
+#define HIGS_MERGE_TILE 4096         // output items per merge-path tile (overflow path)
+
+// ---- per-frame device header: every data-dependent size lives here, never on the host ----------
+struct FrameHeader {
+    uint32_t n_pairs;          // sum of mt_count (0 when overflow)
+    uint32_t n_units;          // N_R (0 when overflow)
+    uint32_t overflow;         // pairs or units exceeded the preallocated capacity
+    uint32_t max_segment;
+    uint32_t n_oversize;       // segments > HIGS_SORT_BLOCK
+    uint32_t n_merge_tiles;    // sum over oversize segments of ceil(n / HIGS_MERGE_TILE)
+    uint32_t max_levels;       // merge levels needed by the longest oversize segment
+    uint32_t n_sort_jobs[HIGS_N_TIERS];
+    uint32_t sort_cursor[HIGS_N_TIERS];   // work counters (persistent kernels)
+    uint32_t raster_cursor;
+    uint32_t merge_barrier;    // software grid barrier of the merge kernel
+    uint32_t n_visible;
+    uint32_t pad0;
+    unsigned long long n_evals;
+    unsigned long long n_tile_pairs;
+};
+
+struct SortJob   { uint32_t start, len, dst_alt, pad; };           // dst_alt: write sorted chunk to the alternate buffer
+struct OverSeg   { uint32_t start, len, levels, tile_base; };     // an oversize segment and its merge plan
+
+// camera + frame constants handed to the kernels by value
+struct FrameParams {
+    float V[12];
+    float fx, fy, cx, cy, near_z;
+    float cam[3];
+    int   W, H;
+    int   n_mx, n_my, n_m;
+    int   degree;
+    int   batch_cap;
+    uint32_t flags;
+    uint32_t max_pairs, max_units;
+};
+
+struct higs_ctx {
+    int device;
+    int64_t max_gaussians;
+    int max_W, max_H, max_nm;
+    int64_t max_pairs, max_units;
+    int n_part_batches_max;
+    int n_sm;
+    uint32_t flags;
+    int batch_cap;
+    // scratch (device)
+    uint32_t* valid_bits;      // [ceil(maxN/32)]
+    float4*   geo;             // [maxN][2]  mux,muy,a,b | c,tau,bits(key),0
+    float4*   ras;             // [maxN][3]  mux,muy,A,B2 | C,tau,log2o,r | g,b,0,0
+    uint16_t* hist;            // [N_B][N_M]
+    uint32_t* base;            // [N_B][N_M] write base of (batch, macro-tile) relative to mt_offset[m]
+    uint32_t* mt_count;        // [max_nm]
+    uint32_t* mt_offset;       // [max_nm+1]
+    uint32_t* batch_offset;    // [max_nm+1]
+    uint32_t* unit_mt;         // [max_units] macro-tile of unit u
+    uint32_t* unit_active;     // [max_units]
+    unsigned long long* pairs; // [max_pairs]
+    unsigned long long* pairs_alt; // [max_pairs] ping-pong buffer of the overflow merge
+    SortJob*  sort_jobs;       // [HIGS_N_TIERS][max_jobs]
+    int64_t   max_jobs;
+    OverSeg*  over_segs;       // [max_over]
+    int64_t   max_over;
+    float4*   partial;         // [max_units][32 tiles][64 px] (r,g,b,T)
+    float*    tile_maxT;       // [max_units][32] largest transmittance left in (unit, tile); 1 = unknown
+    FrameHeader* hdr;          // device
+    FrameHeader* hdr_host;     // pinned
+    // resident scene / host staging
+    float *s_means, *s_scales, *s_quats, *s_opac, *s_sh, *s_img;
+    int64_t s_cap_n; int s_cap_k; int64_t s_img_cap;
+    int64_t s_n; int s_degree;
+    // last frame
+    int64_t last_n; int last_W, last_H, last_nm; int last_mx, last_my;
+    cudaStream_t last_stream;
+    cudaStream_t own_stream;
+    cudaEvent_t ev[9];
+    bool timers_valid;
+    char err[512];
+};
+
+#define HIGS_CUDA(ctx, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
+    snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+    return HIGS_E_CUDA; } } while (0)
+
+// ---- launch entry points, one per pipeline step (defined in the .cu files) ----------------------
+int launch_project(higs_ctx*, const FrameParams&, const float* means, const float* scales, const float* quats,
+                   const float* opac, const float* sh, int64_t N, cudaStream_t);
+int launch_binning(higs_ctx*, const FrameParams&, int64_t N, cudaStream_t, cudaEvent_t ev_count, cudaEvent_t ev_scan);
+int launch_sort(higs_ctx*, const FrameParams&, cudaStream_t);
+int launch_sort_only(higs_ctx*, unsigned long long* pairs, const uint32_t* seg_offset, int n_seg, cudaStream_t);
+int launch_raster(higs_ctx*, const FrameParams&, cudaStream_t);
+int launch_merge(higs_ctx*, const FrameParams&, float* out_rgb, cudaStream_t);
+
+// ---- device helpers ----------------------------------------------------------------------------
+__device__ __forceinline__ float clampf_(float v, float lo, float hi) { return fminf(fmaxf(v, lo), hi); }
+
+// The row scan of DESIGN.md section 3 (N-SCAN): exact x-extent of the threshold ellipse
+// {q <= tau} inside each row band of a grid of cw x ch cells, clipped to [0,W] x [0,H].
+// Every operation is a single correctly rounded fp32 op in the written order (no contraction):
+// the set of cells it yields is part of the bit-exact contract with the oracle.
+struct RowScan {
+    float mux, muy, tau, hx, hy, boc, rc, sdet, yR, nyR, ytop, ybot;
+    int r0, r1;
+    __device__ __forceinline__ void init(float mux_, float muy_, float a, float b, float c, float tau_,
+                                         float fch, int ncy)
+    {
+        mux = mux_; muy = muy_; tau = tau_;
+        hx = __fsqrt_rn(__fmul_rn(tau, a));
+        hy = __fsqrt_rn(__fmul_rn(tau, c));
+        ytop = __fsub_rn(muy, hy); ybot = __fadd_rn(muy, hy);
+        r0 = (int)clampf_(floorf(__fdiv_rn(ytop, fch)), 0.0f, (float)(ncy - 1));
+        r1 = (int)clampf_(floorf(__fdiv_rn(ybot, fch)), 0.0f, (float)(ncy - 1));
+        boc = __fdiv_rn(b, c);
+        rc = __fdiv_rn(1.0f, c);
+        sdet = fmaxf(0.0f, __fmaf_rn(-b, boc, a));
+        yR = __fmul_rn(b, __fsqrt_rn(__fdiv_rn(tau, a)));
+        nyR = -yR;
+    }
+    // columns [m0, m1] of row r; returns false when the row is not touched
+    __device__ __forceinline__ bool row(int r, float fcw, float fch, float fW, float fH, int ncx, int& m0, int& m1) const
+    {
+        float y0 = __fmul_rn((float)r, fch);
+        float y1 = fminf(__fmul_rn((float)(r + 1), fch), fH);
+        float ylo = __fsub_rn(fmaxf(y0, ytop), muy);
+        float yhi = __fsub_rn(fminf(y1, ybot), muy);
+        if (!(yhi >= ylo)) return false;
+        float rlo = __fsqrt_rn(fmaxf(0.0f, __fmul_rn(sdet, __fmaf_rn(-__fmul_rn(ylo, ylo), rc, tau))));
+        float rhi = __fsqrt_rn(fmaxf(0.0f, __fmul_rn(sdet, __fmaf_rn(-__fmul_rn(yhi, yhi), rc, tau))));
+        float xmax = (ylo <= yR && yR <= yhi) ? hx : fmaxf(__fmaf_rn(boc, ylo, rlo), __fmaf_rn(boc, yhi, rhi));
+        float xmin = (ylo <= nyR && nyR <= yhi) ? -hx : fminf(__fmaf_rn(boc, ylo, -rlo), __fmaf_rn(boc, yhi, -rhi));
+        xmin = __fadd_rn(xmin, mux); xmax = __fadd_rn(xmax, mux);
+        if (!(xmax > 0.0f) || !(xmin < fW)) return false;
+        m0 = (int)clampf_(floorf(__fdiv_rn(xmin, fcw)), 0.0f, (float)(ncx - 1));
+        m1 = (int)clampf_(floorf(__fdiv_rn(xmax, fcw)), 0.0f, (float)(ncx - 1));
+        return true;
+    }
+};

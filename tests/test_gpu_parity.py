@@ -1,0 +1,249 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Integer / index outputs bit-exact; pixels within 2e-3 max abs per channel
+(BASELINE.json north_star).  Run on the B200 box: python -m pytest tests -m gpu."""
+import numpy as np
+import pytest
+
+import higs_scenes as hs
+import oracle
+
+pytestmark = pytest.mark.gpu
+
+PIX_TOL = 2e-3          # north_star: max abs per channel, fp32 image in [0,1]
+RGB_TOL = 2e-5          # per-gaussian SH colour, fp32 vs fp64
+
+
+@pytest.fixture(scope="module")
+def hg():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu test without a CUDA device: the CUDA path has no fallback")
+    import paper_2606_00352_b200 as hg
+    return hg
+
+
+def _render(hg, scene, cam, flags=0, batch_cap=1024, max_pairs=0):
+    import torch
+    r = hg.Renderer(max(scene.N, 1), cam.W, cam.H, max_pairs=max_pairs, flags=flags, batch_cap=batch_cap)
+    dev = hg.scene_to_device(scene)
+    img = r.render(*dev, scene.degree, cam)
+    torch.cuda.synchronize()
+    return r, img.cpu().numpy()
+
+
+def _check_records(rec, pr):
+    valid = rec["valid"]
+    assert np.array_equal(valid, pr.valid.astype(bool))
+    v = np.nonzero(valid)[0]
+    geo, ras = rec["geo"][v], rec["ras"][v]
+    # decision-feeding values: bit-exact
+    for col, ocol in [(0, 0), (1, 1), (2, 2), (3, 3), (4, 4), (5, 5)]:
+        assert np.array_equal(geo[:, col].view(np.uint32), pr.geo[v, ocol].view(np.uint32)), f"geo column {col}"
+    assert np.array_equal(geo[:, 6].view(np.uint32), pr.key[v])
+    assert np.array_equal(ras[:, 0].view(np.uint32), pr.geo[v, 0].view(np.uint32))
+    assert np.array_equal(ras[:, 1].view(np.uint32), pr.geo[v, 1].view(np.uint32))
+    for col in range(3):
+        assert np.array_equal(ras[:, 2 + col].view(np.uint32), pr.conic[v, col].view(np.uint32)), f"conic {col}"
+    assert np.array_equal(ras[:, 5].view(np.uint32), pr.geo[v, 5].view(np.uint32))
+    # smooth values
+    np.testing.assert_allclose(ras[:, 6], np.log2(pr.opac[v].astype(np.float64)), atol=2e-6, rtol=2e-6)
+    np.testing.assert_allclose(ras[:, 7:10], pr.rgb[v], atol=RGB_TOL, rtol=RGB_TOL)
+
+
+def _check_lists(ls, ols):
+    assert ls["n_pairs"] == ols.n_pairs and ls["n_units"] == ols.n_units
+    assert np.array_equal(ls["mt_count"], ols.mt_count)
+    assert np.array_equal(ls["mt_offset"], ols.mt_offset)
+    assert np.array_equal(ls["batch_offset"], ols.batch_offset)
+    assert np.array_equal(ls["keys"], ols.keys)
+    assert np.array_equal(ls["ids"], ols.ids)
+
+
+def _full_check(hg, scene, cam, flags=0, batch_cap=1024, image=True):
+    r, img = _render(hg, scene, cam, flags=flags, batch_cap=batch_cap)
+    pr = oracle.project(scene, cam)
+    ols = oracle.bin_lists(pr, B_r=batch_cap)
+    st = r.stats()
+    assert st["n_visible"] == pr.n_vis and st["n_pairs"] == ols.n_pairs and st["n_units"] == ols.n_units
+    assert st["overflow"] == 0 and st["batch_cap"] == batch_cap
+    _check_records(r.records(), pr)
+    _check_lists(r.lists(), ols)
+    if image:
+        ref = oracle.render(pr)
+        err = np.abs(img.astype(np.float64) - ref).max()
+        assert err <= PIX_TOL, f"max abs pixel error {err}"
+    r.close()
+    return img
+
+
+def test_cfg0_tiny_all_outputs(hg):
+    s = hs.scene_cfg0()
+    _full_check(hg, s, s.cameras[0])
+
+
+@pytest.mark.parametrize("batch_cap", [16, 100, 1])
+def test_cfg0_small_batches_force_merging(hg, batch_cap):
+    s = hs.scene_cfg0()
+    _full_check(hg, s, s.cameras[0], batch_cap=batch_cap)
+
+
+def test_cfg0_no_cross_batch_cut_matches_too(hg):
+    s = hs.scene_cfg0()
+    a = _full_check(hg, s, s.cameras[0], batch_cap=16, flags=hg.HIGS_FLAG_NO_XBATCH_CUT)
+    b = _full_check(hg, s, s.cameras[0], batch_cap=16)
+    assert np.abs(a - b).max() < 5e-4          # the cut only drops contributions behind T < 1e-4
+
+
+def test_cfg1_small_all_outputs(hg):
+    s = hs.scene_cfg1()
+    _full_check(hg, s, s.cameras[0])
+
+
+@pytest.mark.parametrize("W,H", [(100, 70), (129, 129), (64, 32), (1, 1), (65, 33)])
+def test_odd_image_sizes(hg, W, H):
+    s = hs.scene_cfg0(N=800, W=W, H=H)
+    _full_check(hg, s, s.cameras[0], batch_cap=64)
+
+
+@pytest.mark.parametrize("degree", [0, 1, 2, 3])
+def test_sh_degrees(hg, degree):
+    s = hs.scene_cfg1(N=5000)
+    K = (degree + 1) ** 2
+    s.sh = np.ascontiguousarray(s.sh[:, :K, :])
+    s.degree = degree
+    cam = hs.make_camera(320, 240, eye=(0.5, -0.3, -1.0), centre=(0.0, 0.0, 5.0))
+    _full_check(hg, s, cam)
+
+
+def test_posed_camera_cfg2_subset(hg):
+    s = hs.scene_cfg2(N=60_000, W=640, H=360)
+    for cam in (s.cameras[1], s.cameras[5]):
+        _full_check(hg, s, cam)
+
+
+def test_empty_and_all_culled(hg):
+    import torch
+    s = hs.scene_cfg0(N=50)
+    cam = s.cameras[0]
+    r = hg.Renderer(100, cam.W, cam.H)
+    z = lambda *shape: torch.zeros(shape, dtype=torch.float32, device="cuda")
+    img = r.render(z(0, 3), z(0, 3), z(0, 4), z(0), z(0, 1, 3), 0, cam)
+    torch.cuda.synchronize()
+    assert not img.cpu().numpy().any()
+    st = r.stats()
+    assert st["n_visible"] == 0 and st["n_pairs"] == 0 and st["n_units"] == 0
+    s.means[:, 2] = -1.0
+    img = r.render(*hg.scene_to_device(s), 0, cam)
+    assert not img.cpu().numpy().any()
+    assert r.stats()["n_visible"] == 0
+    r.close()
+
+
+def test_one_gaussian_covering_the_whole_image(hg):
+    s = hs.single_gaussian((0, 0, 1.0), 3.0, (1, 0, 0, 0), 0.9, (0.3, 0.6, 0.9), 200, 150)
+    img = _full_check(hg, s, s.cameras[0])
+    assert img.min() > 0.1
+
+
+def test_duplicate_depths_tie_break_by_id(hg):
+    # 3000 gaussians on 5 depth planes: long equal-key runs inside one macro-tile
+    rng = np.random.default_rng(3)
+    n = 3000
+    means = np.stack([rng.uniform(-0.05, 0.05, n), rng.uniform(-0.05, 0.05, n), 3.0 + 0.5 * rng.integers(0, 5, n)], axis=1)
+    s = hs.stack_gaussians(means, np.full(n, 0.01), [(1, 0, 0, 0)] * n, rng.uniform(0.02, 0.2, n), rng.uniform(0, 1, (n, 3)), 128, 96)
+    _full_check(hg, s, s.cameras[0])
+
+
+def test_deep_stack_oversize_segment(hg):
+    # 60k gaussians piled onto a few pixels: one macro-tile segment far above the 8192 block size
+    rng = np.random.default_rng(4)
+    n = 60_000
+    means = np.stack([rng.normal(0, 0.01, n), rng.normal(0, 0.01, n), rng.uniform(2, 6, n)], axis=1)
+    s = hs.stack_gaussians(means, np.full(n, 0.004), [(1, 0, 0, 0)] * n, rng.uniform(0.005, 0.05, n), rng.uniform(0, 1, (n, 3)), 128, 64)
+    r, img = _render(hg, s, s.cameras[0])
+    st = r.stats()
+    assert st["max_segment"] > 8192 and st["n_oversize"] >= 1
+    pr = oracle.project(s, s.cameras[0])
+    _check_lists(r.lists(), oracle.bin_lists(pr))
+    assert np.abs(img - oracle.render(pr)).max() <= PIX_TOL
+    r.close()
+
+
+def test_capacity_overflow_is_flagged_not_written(hg):
+    s = hs.scene_cfg0()
+    cam = s.cameras[0]
+    r, img = _render(hg, s, cam, max_pairs=1000)             # the frame has 1,476 pairs
+    st = r.stats(allow_overflow=True)
+    assert st["overflow"] == 1 and st["n_pairs"] == 0 and st["n_units"] == 0
+    assert not img.any()
+    with pytest.raises(hg.HigsError) as e:
+        r.stats()
+    assert e.value.status == hg.HIGS_E_CAPACITY
+    r.close()
+
+
+def test_argument_errors(hg):
+    import ctypes as C
+    L = hg.load()
+    ctx = C.c_void_p()
+    assert L.higs_create(C.byref(ctx), 0, -1, 64, 64, 0) == hg.HIGS_E_ARG
+    assert L.higs_create(None, 0, 10, 64, 64, 0) == hg.HIGS_E_ARG
+    ctx = hg.higs_create(0, 10, 64, 64)
+    cam = hg.make_camera(hs.make_camera(64, 64))
+    assert L.higs_render(ctx, None, None, None, None, None, 4, 0, C.byref(cam), 64, 64, None, None) == hg.HIGS_E_ARG
+    assert L.higs_set_batch_cap(ctx, 0) == hg.HIGS_E_ARG and L.higs_set_batch_cap(ctx, 2048) == hg.HIGS_E_ARG
+    hg.higs_destroy(ctx)
+
+
+def test_host_buffer_entry_points(hg):
+    s = hs.scene_cfg0()
+    cam = s.cameras[0]
+    ctx = hg.higs_create(0, s.N, cam.W, cam.H)
+    out = np.zeros((cam.H, cam.W, 3), np.float32)
+    hg.higs_render_host(ctx, s.means, s.scales, s.quats, s.opacities, s.sh, 0, hg.make_camera(cam), cam.W, cam.H, out)
+    ref = oracle.render(oracle.project(s, cam))
+    assert np.abs(out - ref).max() <= PIX_TOL
+    out2 = np.zeros_like(out)
+    hg.higs_render_view_host(ctx, hg.make_camera(cam), cam.W, cam.H, out2)
+    assert np.array_equal(out, out2) or np.abs(out - out2).max() < 5e-4
+    hg.higs_destroy(ctx)
+
+
+def test_sort_segments_alone_against_numpy(hg):
+    """Teacher forcing of a5: random (key, id) pairs in segments of every tier size, incl. oversize and ties."""
+    import torch
+    rng = np.random.default_rng(9)
+    sizes = [0, 1, 2, 31, 32, 33, 1000, 1024, 1025, 2048, 3000, 4096, 5000, 8192, 8193, 20000, 70000, 7, 0, 500]
+    off = np.concatenate([[0], np.cumsum(sizes)]).astype(np.uint32)
+    n = int(off[-1])
+    keys = rng.integers(0, 2 ** 32, n, dtype=np.uint64)
+    keys[rng.random(n) < 0.3] = np.uint64(0x40400000)            # 30 % ties on one key
+    keys[:2000] &= np.uint64(0xff)                                 # a segment whose high digits are constant
+    ids = rng.permutation(n).astype(np.uint64)
+    pairs = (keys << np.uint64(32)) | ids
+    ctx = hg.higs_create(0, 1000, 1920, 1080, max_pairs=n + 10)
+    d_pairs = torch.from_numpy(pairs.view(np.int64)).cuda()
+    d_off = torch.from_numpy(off.view(np.int32)).cuda()
+    hg.higs_sort_segments(ctx, d_pairs, d_off)
+    torch.cuda.synchronize()
+    got = d_pairs.cpu().numpy().view(np.uint64)
+    for s in range(len(sizes)):
+        a, b = int(off[s]), int(off[s + 1])
+        assert np.array_equal(got[a:b], np.sort(pairs[a:b])), f"segment {s} of size {sizes[s]}"
+    hg.higs_destroy(ctx)
+
+
+def test_cfg3_shaped_reduced_scene_lists_and_sampled_pixels(hg):
+    """The large generator at 300k gaussians, 1080p: lists bit-exact, pixels checked on sampled windows."""
+    s = hs.scene_large(N=300_000, W=1920, H=1080)
+    cam = s.cameras[0]
+    r, img = _render(hg, s, cam)
+    pr = oracle.project(s, cam)
+    _check_lists(r.lists(), oracle.bin_lists(pr))
+    rng = np.random.default_rng(1)
+    for _ in range(12):
+        x0, y0 = int(rng.integers(0, 1920 - 64)), int(rng.integers(0, 1080 - 32))
+        win = (x0, y0, x0 + 64, y0 + 32)
+        ref = oracle.render(pr, window=win)
+        assert np.abs(img[y0:y0 + 32, x0:x0 + 64] - ref).max() <= PIX_TOL
+    r.close()
