@@ -1,0 +1,416 @@
+#!/usr/bin/env python
+"""bench.py -- frames/s of the HiGS forward render path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl higs|reference] [--n N_GAUSSIANS]
+
+A *step* is one frame: one pass of the whole hot path (a1 project+SH .. a8 merge, SURVEY.md section
+8a) over the seeded synthetic 5.8 M-gaussian scene (BASELINE.json configs[3], SH degree 3) at
+1920x1080; step i renders orbit view i % 32 (view 0 is configs[3]'s pose).  The scene arrays
+(1.37 GB) are resident in HBM before the timed region and are far larger than the 126 MB L2, so no
+L2 flush is needed between frames.  The 4K number (configs[4]: same scene, 3840x2160, 32 orbit
+views) is reported next to it under "fps_4k".
+
+Printed (rank 0, ONE JSON line): the base contract keys plus
+  roofline      dominant kernel, algorithmic work / CUDA-event time against the measured peak
+  stages        per-stage ms (CUDA events on the render stream) with each stage's own roofline
+  cpu_baseline  the oracle as it stands, timed on this host's cores (rank 0, N = 1 only)
+  e2e           same metric through higs_render_host: pinned HOST buffers in, HOST image out
+  fps_4k        configs[4] sweep: median / min / max FPS, stage means, unit-load statistics
+
+N > 1 (torchrun, one rank per GPU): frames are independent, so ranks render disjoint views of the
+replicated scene with no data-path collective ("replicas only"); value = frames
+of all ranks / max-over-ranks time.
+
+--impl reference times the CPU oracle (oracle/, plain C, untuned) on this host: the base
+contract's reference arm for this tier.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "frames_per_sec_1080p_5.8M_gaussians"
+UNIT = "frames/s"
+N_PAPER = 5_800_000
+FP32_LANES_PER_SM = 128          # ALU peak = SMs x 128 lanes x SM clock
+RASTER_FP32_INST_PER_EVAL = 13.0  # FP32-pipe instructions per pixel-gaussian evaluation (SASS count)
+
+
+def measured_peaks() -> dict:
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "which": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "which": "fallback"}
+
+
+# ---- rank plumbing (pure functions: covered by the gloo world_size-2 test) -------------------------
+def views_for_rank(step: int, rank: int, world: int, n_views: int) -> int:
+    """Orbit view rendered by `rank` at `step`: ranks walk disjoint, interleaved views."""
+    return (step * world + rank) % n_views
+
+
+def aggregate_fps(frames_per_rank: int, world: int, max_seconds: float) -> float:
+    return frames_per_rank * world / max_seconds if max_seconds > 0 else 0.0
+
+
+def dist_setup():
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, local, world
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled DURING a timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._pump, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def mark(self):
+        return time.time()
+
+    def stop(self):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self, t0: float, t1: float) -> dict:
+        sm, mx, reasons = [], [], set()
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.06] or [r for _, r in self.rows[-3:]]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def build_scene(n: int):
+    import higs_scenes as hs
+    return hs.scene_large(N=n, W=1920, H=1080)
+
+
+def subsample(scene, stride: int):
+    import higs_scenes as hs
+    if stride <= 1:
+        return scene
+    c = lambda a: np.ascontiguousarray(a[::stride])
+    return hs.Scene(scene.name + f"_every{stride}", c(scene.means), c(scene.scales), c(scene.quats), c(scene.opacities),
+                    c(scene.sh), scene.degree, scene.cameras)
+
+
+# ---- the CPU oracle, timed (cpu_baseline leg and --impl reference) ---------------------------------
+def oracle_frame_seconds(scene, cam) -> float:
+    import oracle
+    t0 = time.perf_counter()
+    oracle.render_scene(scene, cam)          # project -> global (key,id) sort -> O-IMG compositing
+    return time.perf_counter() - t0
+
+
+def run_reference(args) -> int:
+    rank, _, world = dist_setup()
+    if rank != 0:
+        return 0
+    import oracle
+    oracle.build()
+    scene = build_scene(args.n)
+    stride = args.ref_stride
+    sub = subsample(scene, stride)
+    cores = oracle.n_threads()
+    n_views = len(scene.cameras)
+    for i in range(args.warmup):
+        oracle_frame_seconds(sub, scene.cameras[i % n_views])
+    t = [oracle_frame_seconds(sub, scene.cameras[i % n_views]) for i in range(args.steps)]
+    total = float(np.sum(t))
+    fps = args.steps / (total * stride)       # a full frame costs ~stride x the sampled one (work is ~linear in N)
+    sample = (f"every {stride}th gaussian of the scene ({sub.N:,} of {scene.N:,}), full 1920x1080 frame, orbit views "
+              f"i%{n_views}; time scaled x{stride}")
+    line = {"impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1000.0 * total * stride / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64 (decisions f32)", "data": "synthetic",
+            "config": workload_config(scene, args, world),
+            "cpu_baseline": {"value": fps, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": fps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def workload_config(scene, args, world) -> dict:
+    return {"workload": "configs[3]: large scene, paper scale (heavy-tailed planes/shells + 20% background + 10% hot region)",
+            "n_gaussians": scene.N, "sh_degree": scene.degree, "image": "1920x1080", "fov_x_deg": 60,
+            "views": f"orbit of {len(scene.cameras)} poses, step i -> view (i*{world}+rank) % {len(scene.cameras)}; view 0 = configs[3]'s pose",
+            "tiles": "8x8 px render tiles, 8x4 macro-tiles (64x32 px), B_r=1024, B_p=8192",
+            "l2": "inputs (1.37 GB) and per-frame records (0.46 GB) exceed the 126 MB L2; no flush between frames",
+            "parallelism": f"replicas x{world} (views sharded, no collective)"}
+
+
+# ---- the CUDA path ------------------------------------------------------------------------------------
+def run_higs(args) -> int:
+    import torch
+    import torch.distributed as dist
+    import higs_scenes as hs
+    import paper_2606_00352_b200 as hg
+
+    rank, local, world = dist_setup()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the HiGS path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks = measured_peaks()
+    scene = build_scene(args.n)
+    n_views = len(scene.cameras)
+    cams_1080 = scene.cameras
+    cams_4k = hs.retarget(scene, 3840, 2160).cameras
+    dev = hg.scene_to_device(scene, f"cuda:{local}")
+    max_w, max_h = (3840, 2160) if not args.no_4k else (1920, 1080)
+    ctx = hg.higs_create(local, scene.N, max_w, max_h, 0)
+    ccams_1080 = [hg.make_camera(c) for c in cams_1080]
+    ccams_4k = [hg.make_camera(c) for c in cams_4k]
+    img = torch.empty((1080, 1920, 3), dtype=torch.float32, device=f"cuda:{local}")
+    stream = torch.cuda.current_stream()
+
+    def frame(i, cams=ccams_1080, W=1920, H=1080, out=img):
+        hg.higs_render(ctx, *dev, scene.degree, cams[views_for_rank(i, rank, world, n_views)], W, H, out, stream.cuda_stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # -- timed region: K frames, CUDA events on the render stream, clocks sampled meanwhile --
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    hg.higs_set_flags(ctx, 0)
+    for i in range(args.warmup):
+        frame(i)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_mark0 = sampler.mark()
+    e0.record(stream)
+    for i in range(args.steps):
+        frame(args.warmup + i)
+    e1.record(stream)
+    barrier()
+    t_mark1 = sampler.mark()
+    secs = e0.elapsed_time(e1) / 1000.0
+    st_last = hg.higs_get_stats(ctx)
+    launches_per_frame = int(st_last["n_launches"])
+    if world > 1:
+        t = torch.tensor([secs], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        secs = float(t.item())
+    fps = aggregate_fps(args.steps, world, secs)
+    clocks = sampler.summary(t_mark0, t_mark1) if rank == 0 else None
+
+    # -- per-stage pass: the same K views with stage events on, one sync per frame --
+    hg.higs_set_flags(ctx, hg.HIGS_FLAG_STAGE_TIMERS)
+    stage_names = ["project", "count", "scan", "fill", "sort", "raster", "merge", "total"]
+    rows, frames_stats = [], []
+    for i in range(args.steps):
+        frame(args.warmup + i)
+        s = hg.higs_get_stats(ctx)
+        rows.append([s["ms_" + k] for k in stage_names])
+        frames_stats.append(s)
+    stage_ms = dict(zip(stage_names, np.mean(np.array(rows), axis=0).tolist()))
+    stage_med = dict(zip(stage_names, np.median(np.array(rows), axis=0).tolist()))
+    mean_of = lambda k: float(np.mean([s[k] for s in frames_stats]))
+
+    # -- instrumented pass: evaluations actually executed by the rasterizer (same views) --
+    hg.higs_set_flags(ctx, hg.HIGS_FLAG_COUNT_EVALS)
+    evals, tile_pairs = [], []
+    for i in range(min(args.steps, 8)):
+        frame(args.warmup + i)
+        s = hg.higs_get_stats(ctx)
+        evals.append(s["n_evals"]); tile_pairs.append(s["n_tile_pairs"])
+    hg.higs_set_flags(ctx, 0)
+    n_evals, n_tile_pairs = float(np.mean(evals)), float(np.mean(tile_pairs))
+
+    # -- rooflines (algorithmic work per launch / mean CUDA-event duration of that stage) --
+    K = (scene.degree + 1) ** 2
+    N, n_vis, n_pairs, n_units = scene.N, mean_of("n_visible"), mean_of("n_pairs"), mean_of("n_units")
+    n_b, n_m = (N + 8191) // 8192, 30 * 34
+    hbm = peaks["hbm_gbs"]
+    alg_bytes = {
+        "project": 44.0 * N + (12.0 * K + 80.0) * n_vis,
+        "count": N / 8.0 + 32.0 * n_vis + 2.0 * n_b * n_m,
+        "fill": N / 8.0 + 32.0 * n_vis + 4.0 * n_b * n_m + 8.0 * n_pairs,
+        "sort": 16.0 * n_pairs,
+    }
+    def hbm_roof(stage, nbytes):
+        ms = stage_ms[stage]
+        ach = nbytes / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
+        return {"bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm, "traffic": None,
+                "peak_source": peaks["which"], "algorithmic_bytes": nbytes, "ms": ms}
+    sm_hz = peaks["sm_max_mhz"] * 1e6
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    alu_peak = n_sm * FP32_LANES_PER_SM * sm_hz / 1e9                      # G FP32-pipe thread-instructions / s
+    ras_ms = stage_ms["raster"]
+    ras_ach = n_evals * RASTER_FP32_INST_PER_EVAL / (ras_ms * 1e-3) / 1e9 if ras_ms > 0 else 0.0
+    roof = {k: hbm_roof(k, v) for k, v in alg_bytes.items()}
+    roof["raster"] = {"bound": "alu", "achieved": ras_ach, "peak": alu_peak, "unit": "G FP32 thread-inst/s",
+                      "frac": ras_ach / alu_peak, "traffic": None, "peak_source": f"{n_sm} SMs x {FP32_LANES_PER_SM} lanes x {peaks['sm_max_mhz']:.0f} MHz",
+                      "evals_per_frame": n_evals, "tile_pairs_per_frame": n_tile_pairs,
+                      "gevals_per_s": n_evals / (ras_ms * 1e-3) / 1e9 if ras_ms > 0 else 0.0,
+                      "fp32_inst_per_eval": RASTER_FP32_INST_PER_EVAL, "ms": ras_ms}
+    dominant = max(("project", "count", "fill", "sort", "raster"), key=lambda k: stage_ms[k])
+
+    # -- e2e: the same frames through higs_render_host (pinned host arrays in, host image out) --
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
+    host = [pin(scene.means), pin(scene.scales), pin(scene.quats), pin(scene.opacities), pin(scene.sh)]
+    host_img = torch.empty((1080, 1920, 3), dtype=torch.float32).pin_memory()
+    h2d = sum(int(t.numel()) * 4 for t in host) + 80
+    d2h = int(host_img.numel()) * 4
+    def e2e_frame(i):
+        hg.higs_render_host(ctx, *host, scene.degree, ccams_1080[views_for_rank(i, rank, world, n_views)], 1920, 1080, host_img)
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    for i in range(min(args.warmup, 3)):
+        e2e_frame(i)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(e2e_steps):
+        e2e_frame(args.warmup + i)
+    barrier()
+    e2e_secs = time.perf_counter() - t0
+    # resident-scene variant: per frame only the camera goes in and the image comes out
+    hg.higs_scene_upload(ctx, *host, scene.degree)
+    for i in range(3):
+        hg.higs_render_view_host(ctx, ccams_1080[i % n_views], 1920, 1080, host_img)
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        hg.higs_render_view_host(ctx, ccams_1080[views_for_rank(args.warmup + i, rank, world, n_views)], 1920, 1080, host_img)
+    barrier()
+    res_secs = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_secs, res_secs], dtype=torch.float64, device=f"cuda:{local}")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_secs, res_secs = (float(x) for x in t.tolist())
+    e2e = {"value": aggregate_fps(e2e_steps, world, e2e_secs), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+           "steps": e2e_steps, "api": "higs_render_host (all five arrays uploaded from pinned host memory every frame)",
+           "resident_scene": {"value": aggregate_fps(args.steps, world, res_secs), "unit": UNIT, "h2d_bytes_per_step": 80,
+                              "d2h_bytes_per_step": d2h, "api": "higs_scene_upload once, then higs_render_view_host per frame"}}
+
+    # -- 4K sweep (configs[4]): every orbit view, 1 warm + 3 timed frames each --
+    fps_4k = None
+    if not args.no_4k:
+        img4 = torch.empty((2160, 3840, 3), dtype=torch.float32, device=f"cuda:{local}")
+        hg.higs_set_flags(ctx, hg.HIGS_FLAG_STAGE_TIMERS)
+        per_view, st4 = [], []
+        my_views = [v for v in range(n_views) if v % world == rank]
+        for v in my_views:
+            ms = []
+            for rep in range(4):
+                hg.higs_render(ctx, *dev, scene.degree, ccams_4k[v], 3840, 2160, img4, stream.cuda_stream)
+                s = hg.higs_get_stats(ctx)
+                if rep:
+                    ms.append(s["ms_total"])
+            per_view.append(1000.0 / float(np.median(ms)))
+            st4.append(s)
+        hg.higs_set_flags(ctx, 0)
+        pv = np.array(per_view)
+        fps_4k = {"workload": "configs[4]: same scene at 3840x2160, 32 orbit views", "views": len(my_views),
+                  "median": float(np.median(pv)), "min": float(pv.min()), "max": float(pv.max()),
+                  "per_view": [round(float(x), 1) for x in pv],
+                  "stages_ms_mean": {k: float(np.mean([s["ms_" + k] for s in st4])) for k in stage_names},
+                  "n_pairs_mean": float(np.mean([s["n_pairs"] for s in st4])), "n_units_mean": float(np.mean([s["n_units"] for s in st4])),
+                  "unit_load_mean": float(np.mean([s["n_pairs"] / max(1, s["n_units"]) for s in st4])), "unit_load_max": 1024,
+                  "max_segment": int(max(s["max_segment"] for s in st4))}
+        del img4
+
+    hg.higs_destroy(ctx)
+    if rank == 0:
+        sampler.stop()
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        oracle.build()
+        stride = args.cpu_stride
+        sub = subsample(scene, stride)
+        secs_cpu = oracle_frame_seconds(sub, scene.cameras[0]) * stride
+        cpu_baseline = {"value": 1.0 / secs_cpu, "unit": UNIT, "cores": oracle.n_threads(), "kind": "oracle",
+                        "ms_per_frame": 1000.0 * secs_cpu,
+                        "sample": ("one whole frame, view 0, all gaussians" if stride == 1 else
+                                   f"every {stride}th gaussian ({sub.N:,} of {scene.N:,}), whole frame, view 0, time scaled x{stride}")}
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank != 0:
+        return 0
+    line = {"metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1000.0 * secs / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic", "config": workload_config(scene, args, world),
+            "clocks": clocks, "gpu_launches": launches_per_frame * args.steps, "gpu_launches_per_frame": launches_per_frame,
+            "roofline": dict(roof[dominant], kernel=dominant), "stages": {"ms_mean": stage_ms, "ms_median": stage_med, "roofline": roof},
+            "frame": {"n_visible": n_vis, "n_pairs": n_pairs, "n_units": n_units, "max_segment": mean_of("max_segment"),
+                      "n_oversize": mean_of("n_oversize"), "unit_load_mean": n_pairs / max(1.0, n_units), "unit_load_max": 1024},
+            "e2e": e2e, "fps_4k": fps_4k, "cpu_baseline": cpu_baseline,
+            "paper_context": "1,124 FPS at 1080p on a 5.8 M-gaussian scene, RTX PRO 6000 Blackwell, fp16 + 32-byte SH (PAPER.md:9): other hardware, other scene, not a target"}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def main() -> int:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=32)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="higs", choices=["higs", "reference"])
+    ap.add_argument("--n", type=int, default=N_PAPER, help="gaussians in the scene (default: the paper-scale 5.8 M)")
+    ap.add_argument("--no-4k", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=16)
+    ap.add_argument("--cpu-stride", type=int, default=1, help="cpu_baseline renders every k-th gaussian (1 = the whole frame)")
+    ap.add_argument("--ref-stride", type=int, default=16, help="--impl reference renders every k-th gaussian per step")
+    args = ap.parse_args()
+    if args.steps < 1 or args.warmup < 0:
+        ap.error("steps >= 1, warmup >= 0")
+    if args.impl == "higs" and args.warmup < 3:
+        args.warmup = 3                                  # timing rule: at least 3 warm-up frames
+    return run_reference(args) if args.impl == "reference" else run_higs(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -78,6 +78,8 @@ typedef struct {
     int32_t n_mt_x, n_mt_y;  /* macro-tile grid                                                   */
     int32_t batch_cap;       /* B_r in effect                                                     */
     int32_t overflow;        /* 1 if the frame hit HIGS_E_CAPACITY                                */
+    int32_t n_launches;      /* kernels the library enqueued for the last frame (memsets excluded) */
+    int32_t reserved0;
     int64_t n_evals;         /* pixel-gaussian evaluations executed by the rasterizer; only
                                 counted when HIGS_FLAG_COUNT_EVALS is set, else 0                 */
     int64_t n_tile_pairs;    /* (gaussian, render tile) pairs that passed the inline visibility

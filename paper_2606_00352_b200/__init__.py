@@ -35,7 +35,7 @@ class higs_camera(C.Structure):
 class higs_stats(C.Structure):
     _fields_ = [("n_gaussians", C.c_int64), ("n_visible", C.c_int64), ("n_pairs", C.c_int64), ("n_units", C.c_int64),
                 ("max_segment", C.c_int64), ("n_oversize", C.c_int64), ("n_mt_x", C.c_int32), ("n_mt_y", C.c_int32),
-                ("batch_cap", C.c_int32), ("overflow", C.c_int32), ("n_evals", C.c_int64), ("n_tile_pairs", C.c_int64),
+                ("batch_cap", C.c_int32), ("overflow", C.c_int32), ("n_launches", C.c_int32), ("reserved0", C.c_int32), ("n_evals", C.c_int64), ("n_tile_pairs", C.c_int64),
                 ("ms_project", C.c_float), ("ms_count", C.c_float), ("ms_scan", C.c_float), ("ms_fill", C.c_float),
                 ("ms_sort", C.c_float), ("ms_raster", C.c_float), ("ms_merge", C.c_float), ("ms_total", C.c_float)]
 

@@ -68,6 +68,7 @@ int render_impl(higs_ctx* ctx, const float* means, const float* scales, const fl
     cudaEvent_t* ev = ctx->ev;
     int rc;
 
+    ctx->n_launches = 0;
     HIGS_CUDA(ctx, cudaMemsetAsync(ctx->hdr, 0, sizeof(FrameHeader), st));
     if (!(ctx->flags & HIGS_FLAG_NO_XBATCH_CUT))
         HIGS_CUDA(ctx, cudaMemsetAsync(ctx->tile_maxT, 0, sizeof(float) * (size_t)ctx->max_units * HIGS_MT_TILES, st));
@@ -308,6 +309,7 @@ int higs_get_stats(higs_ctx* ctx, higs_stats* out)
     out->n_gaussians = ctx->last_n; out->n_visible = h.n_visible; out->n_pairs = h.n_pairs; out->n_units = h.n_units;
     out->max_segment = h.max_segment; out->n_oversize = h.n_oversize;
     out->n_mt_x = ctx->last_mx; out->n_mt_y = ctx->last_my; out->batch_cap = ctx->batch_cap; out->overflow = (int32_t)h.overflow;
+    out->n_launches = ctx->n_launches;
     out->n_evals = (int64_t)h.n_evals; out->n_tile_pairs = (int64_t)h.n_tile_pairs;
     if (ctx->timers_valid) {
         float* dst[7] = { &out->ms_project, &out->ms_count, &out->ms_scan, &out->ms_fill, &out->ms_sort, &out->ms_raster, &out->ms_merge };

@@ -203,23 +203,23 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
     const int pitch = (P.n_m + 1) & ~1;
     if (n_b == 0) {
         k_zero_lists<<<(P.n_m + 256) / 256, 256, 0, st>>>(ctx->mt_count, ctx->mt_offset, ctx->batch_offset, P.n_m);
-        HIGS_CUDA(ctx, cudaGetLastError());
+        HIGS_LAUNCHED(ctx);
         if (ev_count) { cudaEventRecord(ev_count, st); cudaEventRecord(ev_scan, st); }
         return HIGS_OK;
     }
     const size_t smem = sizeof(uint32_t) * (size_t)P.n_m;
     k_count<<<n_b, BIN_THREADS, smem, st>>>(ctx->valid_bits, ctx->geo, N, P, ctx->hist, pitch, ctx->hdr);
-    HIGS_CUDA(ctx, cudaGetLastError());
+    HIGS_LAUNCHED(ctx);
     if (ev_count) cudaEventRecord(ev_count, st);
     const int n_groups = (n_b + SCAN_GROUP - 1) / SCAN_GROUP;
     uint32_t* gsum = ctx->base + (size_t)ctx->n_part_batches_max * ctx->max_nm;   // tail of the base allocation
     k_scan_groups<<<dim3((P.n_m + 255) / 256, n_groups), 256, 0, st>>>(ctx->hist, pitch, n_b, P.n_m, ctx->base, gsum);
-    HIGS_CUDA(ctx, cudaGetLastError());
+    HIGS_LAUNCHED(ctx);
     k_plan<<<1, 1024, 0, st>>>(gsum, n_groups, P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->unit_mt, ctx->hdr);
-    HIGS_CUDA(ctx, cudaGetLastError());
+    HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
     k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->valid_bits, ctx->geo, N, P, ctx->base, gsum, ctx->mt_offset, ctx->pairs, ctx->hdr);
-    HIGS_CUDA(ctx, cudaGetLastError());
+    HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }
 

@@ -86,12 +86,16 @@ struct higs_ctx {
     cudaStream_t own_stream;
     cudaEvent_t ev[9];
     bool timers_valid;
+    int n_launches;            // kernels enqueued by the current / last frame
     char err[512];
 };
 
 #define HIGS_CUDA(ctx, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { \
     snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
     return HIGS_E_CUDA; } } while (0)
+
+// every kernel launch site of a frame calls this right after the <<<>>> (stats: n_launches)
+#define HIGS_LAUNCHED(ctx) do { HIGS_CUDA(ctx, cudaGetLastError()); ++(ctx)->n_launches; } while (0)
 
 // ---- launch entry points, one per pipeline step (defined in the .cu files) ----------------------
 int launch_project(higs_ctx*, const FrameParams&, const float* means, const float* scales, const float* quats,

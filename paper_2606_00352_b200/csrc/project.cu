@@ -217,6 +217,6 @@ int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, cons
         case 2: k_project<2><<<grid, 256, 0, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->geo, ctx->ras); break;
         default: k_project<3><<<grid, 256, 0, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->geo, ctx->ras); break;
     }
-    HIGS_CUDA(ctx, cudaGetLastError());
+    HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }

@@ -268,7 +268,7 @@ int launch_raster(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
     else
         k_raster<false><<<grid, RAS_THREADS, smem, st>>>(ctx->pairs, ctx->ras, ctx->mt_offset, ctx->mt_count, ctx->batch_offset,
                                                          ctx->unit_mt, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_maxT);
-    HIGS_CUDA(ctx, cudaGetLastError());
+    HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }
 
@@ -276,6 +276,6 @@ int launch_merge(higs_ctx* ctx, const FrameParams& P, float* out_rgb, cudaStream
 {
     const int warps = P.n_m * HIGS_MT_TILES;
     k_merge_image<<<(warps + 7) / 8, 256, 0, st>>>(ctx->partial, ctx->unit_active, ctx->batch_offset, P, ctx->hdr, out_rgb);
-    HIGS_CUDA(ctx, cudaGetLastError());
+    HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }

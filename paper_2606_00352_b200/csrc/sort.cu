@@ -282,14 +282,14 @@ int launch_tier(higs_ctx* ctx, int tier, int ctas, u64* pairs, cudaStream_t st)
 {
     k_block_sort<CAP, THREADS><<<ctas, THREADS, sort_smem<CAP, THREADS>(), st>>>(
         ctx->sort_jobs + (size_t)tier * ctx->max_jobs, ctx->hdr, tier, pairs, ctx->pairs_alt);
-    HIGS_CUDA(ctx, cudaGetLastError());
+    HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }
 
 int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, int honour_overflow, cudaStream_t st)
 {
     k_sort_plan<<<1, 1024, 0, st>>>(seg_offset, n_seg, honour_overflow, ctx->sort_jobs, (size_t)ctx->max_jobs, ctx->over_segs, ctx->hdr);
-    HIGS_CUDA(ctx, cudaGetLastError());
+    HIGS_LAUNCHED(ctx);
     int rc;
     if ((rc = launch_tier<1024, 128>(ctx, 0, ctx->n_sm * 8, pairs, st))) return rc;
     if ((rc = launch_tier<2048, 256>(ctx, 1, ctx->n_sm * 4, pairs, st))) return rc;
@@ -298,6 +298,7 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, i
     const OverSeg* over = ctx->over_segs; const FrameHeader* hdr = ctx->hdr; u64* alt = ctx->pairs_alt;
     void* args[] = { (void*)&over, (void*)&hdr, (void*)&pairs, (void*)&alt };
     HIGS_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)k_merge_levels, dim3(ctx->n_sm * g_merge_ctas_per_sm), dim3(MERGE_THREADS), args, 0, st));
+    ++ctx->n_launches;
     return HIGS_OK;
 }
 
