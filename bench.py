@@ -84,7 +84,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thr = threading.Thread(target=self._pump, daemon=True)
             self.thr.start()
@@ -161,9 +161,10 @@ def run_reference(args) -> int:
         oracle_frame_seconds(sub, scene.cameras[i % n_views])
     t = [oracle_frame_seconds(sub, scene.cameras[i % n_views]) for i in range(args.steps)]
     total = float(np.sum(t))
-    fps = args.steps / (total * stride)       # a full frame costs ~stride x the sampled one (work is ~linear in N)
-    sample = (f"every {stride}th gaussian of the scene ({sub.N:,} of {scene.N:,}), full 1920x1080 frame, orbit views "
-              f"i%{n_views}; time scaled x{stride}")
+    fps = args.steps / (total * stride)
+    sample = (f"whole frames (all {scene.N:,} gaussians, 1920x1080), orbit views i%{n_views}" if stride == 1 else
+              f"every {stride}th gaussian of the scene ({sub.N:,} of {scene.N:,}), full 1920x1080 frame, orbit views "
+              f"i%{n_views}; time scaled x{stride} (an over-estimate: occlusion makes the work sub-linear in N)")
     line = {"impl": "reference", "metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1000.0 * total * stride / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64 (decisions f32)", "data": "synthetic",
@@ -395,7 +396,7 @@ def run_higs(args) -> int:
 def main() -> int:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=32)
+    ap.add_argument("--steps", type=int, default=None, help="timed frames (default 100 for higs: the paper's protocol, PAPER.md:309; 10 for reference)")
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="higs", choices=["higs", "reference"])
     ap.add_argument("--n", type=int, default=N_PAPER, help="gaussians in the scene (default: the paper-scale 5.8 M)")
@@ -403,8 +404,10 @@ def main() -> int:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=16)
     ap.add_argument("--cpu-stride", type=int, default=1, help="cpu_baseline renders every k-th gaussian (1 = the whole frame)")
-    ap.add_argument("--ref-stride", type=int, default=16, help="--impl reference renders every k-th gaussian per step")
+    ap.add_argument("--ref-stride", type=int, default=1, help="--impl reference renders every k-th gaussian per step")
     args = ap.parse_args()
+    if args.steps is None:
+        args.steps = 100 if args.impl == "higs" else 10
     if args.steps < 1 or args.warmup < 0:
         ap.error("steps >= 1, warmup >= 0")
     if args.impl == "higs" and args.warmup < 3:
