@@ -104,9 +104,9 @@ typedef struct {
 typedef struct {
     int64_t n;
     const uint32_t* valid_bits;      /* [ceil(N/32)] bit (i & 31) of word i/32 = gaussian i kept  */
-    const float*    geo;             /* [N][8]  mux, muy, a, b, c, tau, bits(key), unused; rows of
-                                        culled gaussians are not written                           */
-    const float*    ras;             /* [N][12] mux, muy, A, B2, C, tau, log2(o), r, g, b, 0, 0    */
+    const float*    rec;             /* [N][16] mux, muy, A, B2, C, tau, log2(o), r, g, b, bits(key), (2 words
+                                        internal), a, b, c; rows of culled gaussians are not written
+                                        (a,b,c = 2D covariance, A,B2,C = conic)       */
 } higs_records;
 
 #define HIGS_FLAG_STAGE_TIMERS  1u   /* record CUDA events around every stage                     */
@@ -116,7 +116,7 @@ typedef struct {
 
 /* Create a context on CUDA device `device` and preallocate all scratch (PAPER.md:83, 284:
  * "preallocated up front").  max_pairs bounds N_pairs (<= 2^31-1; 0 selects 4*max_gaussians + 65536).
- * Device memory taken: ~80 B/gaussian + 16 B/pair + 32 KB per unit (units <= N_M + max_pairs/1024). */
+ * Device memory taken: ~64 B/gaussian + 16 B/pair + 32 KB per unit (units <= N_M + max_pairs/1024). */
 int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, int max_H, int64_t max_pairs);
 void higs_destroy(higs_ctx* ctx);
 

@@ -49,7 +49,7 @@ class higs_lists(C.Structure):
 
 
 class higs_records(C.Structure):
-    _fields_ = [("n", C.c_int64), ("valid_bits", C.c_void_p), ("geo", C.c_void_p), ("ras", C.c_void_p)]
+    _fields_ = [("n", C.c_int64), ("valid_bits", C.c_void_p), ("rec", C.c_void_p)]
 
 
 class HigsError(RuntimeError):
@@ -223,14 +223,13 @@ def higs_get_lists(ctx) -> dict:
 
 
 def higs_get_records(ctx) -> dict:
-    """Per-gaussian records of the last frame: valid (N,) bool, geo (N,8), ras (N,12) (rows of culled gaussians are stale)."""
+    """Per-gaussian records of the last frame: valid (N,) bool, rec (N,16) (rows of culled gaussians are stale)."""
     rc_ = higs_records()
     _check(load().higs_get_records(ctx, C.byref(rc_)), "higs_get_records", ctx)
     n = int(rc_.n)
     words = _dev_to_numpy(ctx, rc_.valid_bits, (n + 31) // 32, np.uint32)
     valid = ((words[:, None] >> np.arange(32, dtype=np.uint32)[None, :]) & 1).astype(bool).reshape(-1)[:n]
-    return {"n": n, "valid": valid, "geo": _dev_to_numpy(ctx, rc_.geo, n * 8, np.float32).reshape(n, 8),
-            "ras": _dev_to_numpy(ctx, rc_.ras, n * 12, np.float32).reshape(n, 12)}
+    return {"n": n, "valid": valid, "rec": _dev_to_numpy(ctx, rc_.rec, n * 16, np.float32).reshape(n, 16)}
 
 
 def higs_sort_segments(ctx, pairs, seg_offset, stream: Optional[int] = None) -> None:

@@ -7,6 +7,7 @@
 #include "higs_internal.cuh"
 
 int higs_binning_smem_setup(higs_ctx*);
+int higs_project_smem_setup(higs_ctx*);
 int higs_sort_smem_setup(higs_ctx*);
 int higs_raster_setup(higs_ctx*);
 
@@ -31,10 +32,14 @@ template <typename T> void dev_free(T*& p) { if (p) cudaFree(p); p = nullptr; }
 int alloc_unit_buffers(higs_ctx* ctx)
 {
     dev_free(ctx->unit_mt); dev_free(ctx->unit_active); dev_free(ctx->partial); dev_free(ctx->tile_maxT);
+    dev_free(ctx->unit_order); dev_free(ctx->level_hist); dev_free(ctx->level_cur);
     ctx->max_units = ctx->max_nm + (ctx->max_pairs + ctx->batch_cap - 1) / ctx->batch_cap + 1;
     int rc;
     if ((rc = dev_alloc(ctx, &ctx->unit_mt, (size_t)ctx->max_units))) return rc;
     if ((rc = dev_alloc(ctx, &ctx->unit_active, (size_t)ctx->max_units))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->unit_order, (size_t)ctx->max_units))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->level_hist, (size_t)ctx->max_units + 2))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->level_cur, (size_t)ctx->max_units + 2))) return rc;
     if ((rc = dev_alloc(ctx, &ctx->partial, (size_t)ctx->max_units * HIGS_MT_TILES * 64))) return rc;
     if ((rc = dev_alloc(ctx, &ctx->tile_maxT, (size_t)ctx->max_units * HIGS_MT_TILES))) return rc;
     return HIGS_OK;
@@ -170,8 +175,7 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     const int n_groups_max = (ctx->n_part_batches_max + 31) / 32;
     const size_t pitch = ((size_t)nm + 1) & ~(size_t)1;
     if ((rc = dev_alloc(ctx, &ctx->valid_bits, (size_t)(n + 31) / 32 + 1))) return fail(rc);
-    if ((rc = dev_alloc(ctx, &ctx->geo, (size_t)n * 2))) return fail(rc);
-    if ((rc = dev_alloc(ctx, &ctx->ras, (size_t)n * 3))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->rec, (size_t)n * 4))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->hist, (size_t)ctx->n_part_batches_max * pitch))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->base, (size_t)(ctx->n_part_batches_max + n_groups_max) * nm))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->mt_count, (size_t)nm + 1))) return fail(rc);
@@ -190,6 +194,7 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     memset(ctx->hdr_host, 0, sizeof(FrameHeader));
     if (cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(HIGS_E_CUDA);
     for (int i = 0; i < 9; ++i) if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) return fail(HIGS_E_CUDA);
+    if ((rc = higs_project_smem_setup(ctx))) return fail(rc);
     if ((rc = higs_binning_smem_setup(ctx))) return fail(rc);
     if ((rc = higs_sort_smem_setup(ctx))) return fail(rc);
     if ((rc = higs_raster_setup(ctx))) return fail(rc);
@@ -203,10 +208,11 @@ void higs_destroy(higs_ctx* ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
-    dev_free(ctx->valid_bits); dev_free(ctx->geo); dev_free(ctx->ras); dev_free(ctx->hist); dev_free(ctx->base);
+    dev_free(ctx->valid_bits); dev_free(ctx->rec); dev_free(ctx->hist); dev_free(ctx->base);
     dev_free(ctx->mt_count); dev_free(ctx->mt_offset); dev_free(ctx->batch_offset); dev_free(ctx->unit_mt);
     dev_free(ctx->unit_active); dev_free(ctx->pairs); dev_free(ctx->pairs_alt); dev_free(ctx->sort_jobs);
     dev_free(ctx->over_segs); dev_free(ctx->partial); dev_free(ctx->tile_maxT); dev_free(ctx->hdr);
+    dev_free(ctx->unit_order); dev_free(ctx->level_hist); dev_free(ctx->level_cur);
     dev_free(ctx->s_means); dev_free(ctx->s_scales); dev_free(ctx->s_quats); dev_free(ctx->s_opac); dev_free(ctx->s_sh);
     dev_free(ctx->s_img);
     if (ctx->hdr_host) cudaFreeHost(ctx->hdr_host);
@@ -337,7 +343,7 @@ int higs_get_records(higs_ctx* ctx, higs_records* out)
     int rc = fetch_header(ctx);
     if (rc) return rc;
     out->n = ctx->last_n; out->valid_bits = ctx->valid_bits;
-    out->geo = reinterpret_cast<const float*>(ctx->geo); out->ras = reinterpret_cast<const float*>(ctx->ras);
+    out->rec = reinterpret_cast<const float*>(ctx->rec);
     return HIGS_OK;
 }
 

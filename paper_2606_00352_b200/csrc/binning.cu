@@ -1,13 +1,13 @@
-// binning.cu -- steps a2 count, a3 scan, a4 fill, a6 batch schedule (section 3.2,
-// PAPER.md:247-257 section 4.3, section 3.1).
+// binning.cu -- steps a3 scan, a4 fill, a6 batch schedule (section 3.2,
+// PAPER.md:247-257 section 4.3, section 3.1).  The count pass (a2) lives in project.cu.
 //
 // Count and fill each run one CTA per partitioning batch of B_p = 8192 consecutive gaussian ids
-// (PAPER.md:89, 251); both consume the per-warp visibility bitfield of a1, so culled gaussians never
-// reach the intersection test.  The count CTA keeps a private shared-memory histogram
-// with one counter per macro-tile and flushes it as uint16 (a cell holds <= 8192) into the
+// (PAPER.md:89, 251); fill consumes the per-warp visibility bitfield of a1, so culled gaussians never
+// reach it.  The count CTA's histogram arrives as uint16 (a cell holds <= 8192) in the
 // N_B x N_M matrix; the scan widens it to 32-bit write bases in two levels (groups of 32 batches);
-// the fill CTA replays the intersection and drops (depth key << 32 | id) at base + local rank.
-// The intersection is the row scan N-SCAN: bit-exact with the oracle.
+// the fill CTA replays the intersection -- from the 64-bit span descriptor the count left in the
+// record, or by redoing the row scan N-SCAN when the span did not fit -- and drops
+// (depth key << 32 | id) at base + local rank.
 #include <stdio.h>
 #include "higs_internal.cuh"
 
@@ -15,51 +15,6 @@ namespace {
 
 constexpr int BIN_THREADS = 512;
 constexpr int SCAN_GROUP  = 32;      // batches per first-level scan group
-
-// visit every macro-tile the threshold ellipse of gaussian i touches
-template <typename F>
-__device__ __forceinline__ void for_each_macro_tile(const float4* __restrict__ geo, int64_t i, const FrameParams& P, F&& f)
-{
-    const float4 g0 = geo[2 * i], g1 = geo[2 * i + 1];
-    RowScan rs;
-    rs.init(g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, (float)HIGS_MT_H, P.n_my);
-    const float fW = (float)P.W, fH = (float)P.H;
-    for (int r = rs.r0; r <= rs.r1; ++r) {
-        int m0, m1;
-        if (!rs.row(r, (float)HIGS_MT_W, (float)HIGS_MT_H, fW, fH, P.n_mx, m0, m1)) continue;
-        for (int m = m0; m <= m1; ++m) f(r * P.n_mx + m, __float_as_uint(g1.z));
-    }
-}
-
-__global__ void __launch_bounds__(BIN_THREADS)
-k_count(const uint32_t* __restrict__ valid_bits, const float4* __restrict__ geo, int64_t N, const FrameParams P,
-        uint16_t* __restrict__ hist, int pitch, FrameHeader* __restrict__ hdr)
-{
-    extern __shared__ uint32_t s_hist[];
-    __shared__ uint32_t s_nvis;
-    for (int m = threadIdx.x; m < P.n_m; m += BIN_THREADS) s_hist[m] = 0;
-    if (threadIdx.x == 0) s_nvis = 0;
-    __syncthreads();
-    const int64_t i0 = (int64_t)blockIdx.x * HIGS_PART_BATCH;
-    uint32_t nvis = 0;
-    for (int k = 0; k < HIGS_PART_BATCH / BIN_THREADS; ++k) {
-        const int64_t i = i0 + k * BIN_THREADS + threadIdx.x;
-        if (i >= N) break;
-        if (!((valid_bits[i >> 5] >> (i & 31)) & 1u)) continue;
-        ++nvis;
-        for_each_macro_tile(geo, i, P, [&](int cell, uint32_t) { atomicAdd(&s_hist[cell], 1u); });
-    }
-    nvis = __reduce_add_sync(0xffffffffu, nvis);
-    if ((threadIdx.x & 31) == 0 && nvis) atomicAdd(&s_nvis, nvis);
-    __syncthreads();
-    uint32_t* row = reinterpret_cast<uint32_t*>(hist + (size_t)blockIdx.x * pitch);   // pitch is even
-    for (int m2 = threadIdx.x; m2 < pitch / 2; m2 += BIN_THREADS) {
-        const int m = 2 * m2;
-        const uint32_t lo = s_hist[m], hi = (m + 1 < P.n_m) ? s_hist[m + 1] : 0u;
-        row[m2] = lo | (hi << 16);
-    }
-    if (threadIdx.x == 0 && s_nvis) atomicAdd(&hdr->n_visible, s_nvis);
-}
 
 // First scan level: CTA (column chunk, group) walks its <= 32 batches; base[b][m] = pairs of
 // macro-tile m in the earlier batches of the same group; gsum[g][m] = total of the group.
@@ -123,7 +78,8 @@ __device__ __forceinline__ void block_scan_excl(uint32_t (&v)[NV], uint32_t (&ca
 __global__ void __launch_bounds__(1024)
 k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, const FrameParams P,
        uint32_t* __restrict__ mt_count, uint32_t* __restrict__ mt_offset, uint32_t* __restrict__ batch_offset,
-       uint32_t* __restrict__ unit_mt, FrameHeader* __restrict__ hdr)
+       uint32_t* __restrict__ unit_mt, uint32_t* __restrict__ unit_order, uint32_t* __restrict__ level_hist,
+       uint32_t* __restrict__ level_cur, FrameHeader* __restrict__ hdr)
 {
     __shared__ uint32_t s_warp[33 * 2];
     __shared__ uint32_t s_max;
@@ -158,15 +114,54 @@ k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, con
         hdr->max_segment = s_max;
     }
     if (overflow) return;
-    // pass 2: unit table
+    // pass 2: unit table, and the order the rasterizer claims units in: batch index j major ("level" j =
+    // the j-th batch of every macro-tile that has one), so that by the time a deep batch starts the batches
+    // in front of it have published their transmittance bounds (cross-batch cut).
+    const uint32_t max_nb = (s_max + br - 1) / br;
+    for (uint32_t v = threadIdx.x; v <= max_nb + 1; v += 1024) level_hist[v] = 0;
+    __syncthreads();
     for (int m = threadIdx.x; m < P.n_m; m += 1024) {
-        const uint32_t u0 = batch_offset[m], nb = (mt_count[m] + br - 1) / br;
-        for (uint32_t j = 0; j < nb; ++j) unit_mt[u0 + j] = (uint32_t)m;
+        const uint32_t nb = (mt_count[m] + br - 1) / br;
+        if (nb) atomicAdd(&level_hist[nb], 1u);               // macro-tiles with exactly nb batches
+    }
+    __syncthreads();
+    // units in level j = macro-tiles with more than j batches = n_nonempty - #{nb <= j}; level bases = exclusive
+    // prefix of that over j.  Two chained block scans over j in chunks of 1024.
+    {
+        uint32_t c_hist[1] = {0}, c_base[1] = {0};
+        __shared__ uint32_t s_nonempty;
+        if (threadIdx.x == 0) s_nonempty = 0;
+        __syncthreads();
+        uint32_t mine = 0;
+        for (uint32_t v = threadIdx.x; v <= max_nb; v += 1024) mine += level_hist[v];
+        mine = __reduce_add_sync(0xffffffffu, mine);
+        if ((threadIdx.x & 31) == 0 && mine) atomicAdd(&s_nonempty, mine);
+        __syncthreads();
+        const uint32_t n_nonempty = s_nonempty;
+        for (uint32_t j0 = 0; j0 < max_nb; j0 += 1024) {
+            const uint32_t j = j0 + threadIdx.x;
+            const uint32_t h = (j < max_nb) ? level_hist[j + 1] : 0u;       // hist[0] is unused (nb = 0 is never counted)
+            uint32_t v[1] = { h };
+            block_scan_excl<1>(v, c_hist, s_warp);                        // v = #{1 <= nb <= j}
+            const uint32_t cnt = (j < max_nb) ? n_nonempty - v[0] : 0u;     // macro-tiles with nb > j
+            uint32_t b[1] = { cnt };
+            block_scan_excl<1>(b, c_base, s_warp);
+            if (j < max_nb) level_cur[j] = b[0];
+        }
+    }
+    __syncthreads();
+    for (uint32_t u = threadIdx.x; u < n_units; u += 1024) {
+        int lo = 0, hi = P.n_m - 1;                                       // last m with batch_offset[m] <= u and a batch there
+        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (batch_offset[mid] <= u) lo = mid; else hi = mid - 1; }
+        unit_mt[u] = (uint32_t)lo;
+        unit_order[atomicAdd(&level_cur[u - batch_offset[lo]], 1u)] = u;
     }
 }
 
+#define HIGS_DESC_FALLBACK 0x8000000000000000ull   // see project.cu
+
 __global__ void __launch_bounds__(BIN_THREADS)
-k_fill(const uint32_t* __restrict__ valid_bits, const float4* __restrict__ geo, int64_t N, const FrameParams P,
+k_fill(const uint32_t* __restrict__ valid_bits, const float4* __restrict__ rec, int64_t N, const FrameParams P,
        const uint32_t* __restrict__ base, const uint32_t* __restrict__ gbase, const uint32_t* __restrict__ mt_offset,
        unsigned long long* __restrict__ pairs, const FrameHeader* __restrict__ hdr)
 {
@@ -181,10 +176,29 @@ k_fill(const uint32_t* __restrict__ valid_bits, const float4* __restrict__ geo, 
         const int64_t i = i0 + k * BIN_THREADS + threadIdx.x;
         if (i >= N) break;
         if (!((valid_bits[i >> 5] >> (i & 31)) & 1u)) continue;
-        for_each_macro_tile(geo, i, P, [&](int cell, uint32_t key) {
-            const uint32_t pos = atomicAdd(&s_cursor[cell], 1u);
-            pairs[pos] = ((unsigned long long)key << 32) | (unsigned long long)(uint32_t)i;
-        });
+        const float4 s2 = __ldcs(rec + 4 * i + 2), s3 = __ldcs(rec + 4 * i + 3);   // g, b, key, desc_lo | desc_hi, a, b, c
+        const unsigned long long item = ((unsigned long long)__float_as_uint(s2.z) << 32) | (unsigned long long)(uint32_t)i;
+        const unsigned long long desc = ((unsigned long long)__float_as_uint(s3.x) << 32) | __float_as_uint(s2.w);
+        if (!(desc & HIGS_DESC_FALLBACK)) {
+            const int r0 = (int)(desc & 511u), nr = (int)((desc >> 9) & 3u);
+            for (int rr = 0; rr <= nr; ++rr) {
+                const uint32_t f = (uint32_t)(desc >> (11 + 13 * rr)) & 0x1fffu;
+                const int m0 = (int)(f & 511u);
+                if (m0 == 511) continue;
+                const int cell0 = (r0 + rr) * P.n_mx + m0, w = (int)(f >> 9);
+                for (int m = 0; m <= w; ++m) pairs[atomicAdd(&s_cursor[cell0 + m], 1u)] = item;
+            }
+        } else {                                    // span too large for the descriptor: redo the row scan
+            const float4 s0 = __ldcs(rec + 4 * i), s1 = __ldcs(rec + 4 * i + 1);
+            RowScan rs;
+            rs.init(s0.x, s0.y, s3.y, s3.z, s3.w, s1.y, (float)HIGS_MT_H, P.n_my);
+            const float fW = (float)P.W, fH = (float)P.H;
+            for (int r = rs.r0; r <= rs.r1; ++r) {
+                int m0, m1;
+                if (!rs.row(r, (float)HIGS_MT_W, (float)HIGS_MT_H, fW, fH, P.n_mx, m0, m1)) continue;
+                for (int m = m0; m <= m1; ++m) pairs[atomicAdd(&s_cursor[r * P.n_mx + m], 1u)] = item;
+            }
+        }
     }
 }
 
@@ -208,17 +222,16 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
         return HIGS_OK;
     }
     const size_t smem = sizeof(uint32_t) * (size_t)P.n_m;
-    k_count<<<n_b, BIN_THREADS, smem, st>>>(ctx->valid_bits, ctx->geo, N, P, ctx->hist, pitch, ctx->hdr);
-    HIGS_LAUNCHED(ctx);
-    if (ev_count) cudaEventRecord(ev_count, st);
+    if (ev_count) cudaEventRecord(ev_count, st);    // the count pass ran inside k_project: this stage is empty
     const int n_groups = (n_b + SCAN_GROUP - 1) / SCAN_GROUP;
     uint32_t* gsum = ctx->base + (size_t)ctx->n_part_batches_max * ctx->max_nm;   // tail of the base allocation
     k_scan_groups<<<dim3((P.n_m + 255) / 256, n_groups), 256, 0, st>>>(ctx->hist, pitch, n_b, P.n_m, ctx->base, gsum);
     HIGS_LAUNCHED(ctx);
-    k_plan<<<1, 1024, 0, st>>>(gsum, n_groups, P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->unit_mt, ctx->hdr);
+    k_plan<<<1, 1024, 0, st>>>(gsum, n_groups, P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->unit_mt, ctx->unit_order,
+                               ctx->level_hist, ctx->level_cur, ctx->hdr);
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
-    k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->valid_bits, ctx->geo, N, P, ctx->base, gsum, ctx->mt_offset, ctx->pairs, ctx->hdr);
+    k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->valid_bits, ctx->rec, N, P, ctx->base, gsum, ctx->mt_offset, ctx->pairs, ctx->hdr);
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }
@@ -227,7 +240,6 @@ int higs_binning_smem_setup(higs_ctx* ctx)
 {
     const int bytes = (int)(sizeof(uint32_t) * (size_t)ctx->max_nm);
     if (bytes > 48 * 1024) {
-        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_count, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
         HIGS_CUDA(ctx, cudaFuncSetAttribute(k_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     }
     return HIGS_OK;

@@ -57,8 +57,8 @@ struct higs_ctx {
     int batch_cap;
     // scratch (device)
     uint32_t* valid_bits;      // [ceil(maxN/32)]
-    float4*   geo;             // [maxN][2]  mux,muy,a,b | c,tau,bits(key),0
-    float4*   ras;             // [maxN][3]  mux,muy,A,B2 | C,tau,log2o,r | g,b,0,0
+    float4*   rec;             // [maxN][4]  mux,muy,A,B2 | C,tau,log2o,r | g,b,bits(key),desc_lo | desc_hi,a,b,c  (64 B = two sectors:
+                               //            the rasterizer gathers the first 40 B, fill reads the second sector)
     uint16_t* hist;            // [N_B][N_M]
     uint32_t* base;            // [N_B][N_M] write base of (batch, macro-tile) relative to mt_offset[m]
     uint32_t* mt_count;        // [max_nm]
@@ -66,6 +66,9 @@ struct higs_ctx {
     uint32_t* batch_offset;    // [max_nm+1]
     uint32_t* unit_mt;         // [max_units] macro-tile of unit u
     uint32_t* unit_active;     // [max_units]
+    uint32_t* unit_order;      // [max_units] units in the order the rasterizer claims them: batch index j major
+    uint32_t* level_hist;      // [max_units+2] scratch of k_plan: macro-tiles per batch count, then level cursors
+    uint32_t* level_cur;       // [max_units+2]
     unsigned long long* pairs; // [max_pairs]
     unsigned long long* pairs_alt; // [max_pairs] ping-pong buffer of the overflow merge
     SortJob*  sort_jobs;       // [HIGS_N_TIERS][max_jobs]

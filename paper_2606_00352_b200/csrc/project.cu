@@ -1,10 +1,15 @@
-// project.cu -- step a1: fused EWA projection + cull + SH colour (section 4.2:
+// project.cu -- steps a1 + a2: fused EWA projection + cull + SH colour (section 4.2), with the
+// count pass of the partitioning folded in: one CTA per partition batch of B_p = 8192
+// consecutive ids keeps the private shared-memory histogram with one counter per macro-tile and flushes it as
+// packed uint16 into the N_B x N_M matrix.  The kernel is HBM-latency-bound, so the row scan runs in issue
+// slots that were idle; the macro-tile span it finds is also packed into a 64-bit descriptor in the record, so
+// the fill pass replays it without redoing the arithmetic.  (Section 4.2:
 // "Each thread processes one gaussian end-to-end: camera-space transformation, 2D covariance via
 // Jacobian projection, ... inline view-direction computation, and degree-3 spherical harmonics
 // evaluation.  The outputs -- 2D positions, ... conics, colors, and a compact per-warp visibility
 // bitfield -- are consumed by the partitioning and rasterization stages.")
 //
-// HBM-bound: 44 B read per gaussian + 12*K B of SH read and 80 B written per *visible* gaussian.
+// HBM-bound: 44 B read per gaussian + 12*K B of SH read and 64 B written per *visible* gaussian.
 // Everything that later decides an integer (cull, macro-tile set, depth key, the 1/255 skip) follows
 // the pinned fp32 sequence N-PROJ of DESIGN.md section 3, one correctly rounded op per written op:
 // the __f*_rn intrinsics are never contracted into FMAs by nvcc.
@@ -90,13 +95,30 @@ __device__ __forceinline__ void sh_accumulate(const float* __restrict__ shp, flo
     r = fmaxf(r, 0.0f); g = fmaxf(g, 0.0f); b = fmaxf(b, 0.0f);
 }
 
+constexpr int PROJ_THREADS = 512;
+
+// 64-bit macro-tile span descriptor (internal): bit 63 = "not representable, rerun the row scan";
+// bits 0-8 first macro-tile row r0, bits 9-10 rows-1 (<= 4 rows), then 13 bits per row:
+// first column m0 (9 bits, 511 = row not touched) and columns-1 (4 bits, <= 16 columns).
+#define HIGS_DESC_FALLBACK 0x8000000000000000ull
+
 template <int DEG>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(PROJ_THREADS, 2)
 k_project(const float* __restrict__ means, const float* __restrict__ scales, const float* __restrict__ quats,
           const float* __restrict__ opac, const float* __restrict__ sh, int64_t N, const FrameParams P,
-          uint32_t* __restrict__ valid_bits, float4* __restrict__ geo, float4* __restrict__ ras)
+          uint32_t* __restrict__ valid_bits, float4* __restrict__ rec, uint16_t* __restrict__ hist, int pitch,
+          FrameHeader* __restrict__ hdr)
 {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    extern __shared__ uint32_t s_hist[];
+    __shared__ uint32_t s_nvis;
+    for (int m = threadIdx.x; m < P.n_m; m += PROJ_THREADS) s_hist[m] = 0;
+    if (threadIdx.x == 0) s_nvis = 0;
+    __syncthreads();
+    const int64_t i0 = (int64_t)blockIdx.x * HIGS_PART_BATCH;
+    uint32_t nvis = 0;
+    for (int it = 0; it < HIGS_PART_BATCH / PROJ_THREADS; ++it) {
+    if (i0 + (int64_t)it * PROJ_THREADS >= N) break;                 // block-uniform
+    const int64_t i = i0 + (int64_t)it * PROJ_THREADS + threadIdx.x;
     bool ok = i < N;
     float mx = 0, my = 0, mz = 0;
     float mux = 0, muy = 0, a = 0, b = 0, c = 0, A = 0, B2 = 0, C = 0, tau = 0, zc = 0, o = 0;
@@ -187,21 +209,51 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
         }
     }
     const uint32_t vmask = __ballot_sync(0xffffffffu, ok);
-    if ((threadIdx.x & 31) == 0 && i < ((N + 31) / 32) * 32) valid_bits[i >> 5] = vmask;
-    if (!ok) return;
+    if ((threadIdx.x & 31) == 0 && (i < N)) valid_bits[i >> 5] = vmask;   // warp bases are multiples of 32
+    if (!ok) continue;
+    ++nvis;
+    // a2: macro-tile row scan (N-SCAN, pinned) -> private histogram + span descriptor
+    unsigned long long desc = 0;
+    {
+        RowScan rs;
+        rs.init(mux, muy, a, b, c, tau, (float)HIGS_MT_H, P.n_my);
+        const float fW = (float)P.W, fH = (float)P.H;
+        bool fits = (rs.r1 - rs.r0) <= 3 && P.n_mx <= 511 && rs.r0 <= 511;
+        desc = (unsigned long long)(uint32_t)rs.r0 | ((unsigned long long)(uint32_t)((rs.r1 - rs.r0) & 3) << 9);
+        for (int r = rs.r0; r <= rs.r1; ++r) {
+            int m0, m1;
+            uint32_t field = 511u;
+            if (rs.row(r, (float)HIGS_MT_W, (float)HIGS_MT_H, fW, fH, P.n_mx, m0, m1)) {
+                for (int m = m0; m <= m1; ++m) atomicAdd(&s_hist[r * P.n_mx + m], 1u);
+                fits = fits && (m1 - m0) <= 15;
+                field = (uint32_t)m0 | ((uint32_t)((m1 - m0) & 15) << 9);
+            }
+            if (r - rs.r0 <= 3) desc |= (unsigned long long)field << (11 + 13 * (r - rs.r0));
+        }
+        if (!fits) desc = HIGS_DESC_FALLBACK;
+    }
     // 11./12. depth key, colour
     float dx = mx - P.cam[0], dy = my - P.cam[1], dz = mz - P.cam[2];
     float len2 = dx * dx + dy * dy + dz * dz;
     float rl = len2 > 0.0f ? rsqrtf(len2) : 0.0f;
     float r, g, bl;
     sh_accumulate<DEG>(sh + i * (int64_t)((DEG + 1) * (DEG + 1) * 3), dx * rl, dy * rl, dz * rl, r, g, bl);
-    float4* gp = geo + 2 * i;
-    gp[0] = make_float4(mux, muy, a, b);
-    gp[1] = make_float4(c, tau, __uint_as_float(__float_as_uint(zc)), 0.0f);
-    float4* rp = ras + 3 * i;
+    float4* rp = rec + 4 * i;
     rp[0] = make_float4(mux, muy, A, B2);
     rp[1] = make_float4(C, tau, log2f(o), r);
-    rp[2] = make_float4(g, bl, 0.0f, 0.0f);
+    rp[2] = make_float4(g, bl, __uint_as_float(__float_as_uint(zc)), __uint_as_float((uint32_t)desc));
+    rp[3] = make_float4(__uint_as_float((uint32_t)(desc >> 32)), a, b, c);
+    }   // partition-batch loop
+    nvis = __reduce_add_sync(0xffffffffu, nvis);
+    if ((threadIdx.x & 31) == 0 && nvis) atomicAdd(&s_nvis, nvis);
+    __syncthreads();
+    uint32_t* row = reinterpret_cast<uint32_t*>(hist + (size_t)blockIdx.x * pitch);   // pitch is even
+    for (int m2 = threadIdx.x; m2 < pitch / 2; m2 += PROJ_THREADS) {
+        const int m = 2 * m2;
+        const uint32_t lo = s_hist[m], hi = (m + 1 < P.n_m) ? s_hist[m + 1] : 0u;
+        row[m2] = lo | (hi << 16);                                   // a cell holds <= 8192: uint16 is enough
+    }
+    if (threadIdx.x == 0 && s_nvis) atomicAdd(&hdr->n_visible, s_nvis);
 }
 
 } // namespace
@@ -210,13 +262,30 @@ int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, cons
                    const float* opac, const float* sh, int64_t N, cudaStream_t st)
 {
     if (N <= 0) return HIGS_OK;
-    const unsigned grid = (unsigned)((N + 255) / 256);
+    const unsigned grid = (unsigned)((N + HIGS_PART_BATCH - 1) / HIGS_PART_BATCH);
+    const size_t smem = sizeof(uint32_t) * (size_t)P.n_m;
+    const int pitch = (P.n_m + 1) & ~1;
+#define HIGS_PROJ(D) k_project<D><<<grid, PROJ_THREADS, smem, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
+                                                                   ctx->hist, pitch, ctx->hdr)
     switch (P.degree) {
-        case 0: k_project<0><<<grid, 256, 0, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->geo, ctx->ras); break;
-        case 1: k_project<1><<<grid, 256, 0, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->geo, ctx->ras); break;
-        case 2: k_project<2><<<grid, 256, 0, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->geo, ctx->ras); break;
-        default: k_project<3><<<grid, 256, 0, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->geo, ctx->ras); break;
+        case 0: HIGS_PROJ(0); break;
+        case 1: HIGS_PROJ(1); break;
+        case 2: HIGS_PROJ(2); break;
+        default: HIGS_PROJ(3); break;
     }
+#undef HIGS_PROJ
     HIGS_LAUNCHED(ctx);
+    return HIGS_OK;
+}
+
+int higs_project_smem_setup(higs_ctx* ctx)
+{
+    const int bytes = (int)(sizeof(uint32_t) * (size_t)ctx->max_nm);
+    if (bytes > 48 * 1024) {
+        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    }
     return HIGS_OK;
 }

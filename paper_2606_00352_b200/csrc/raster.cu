@@ -26,10 +26,16 @@ namespace {
 constexpr int RAS_THREADS = 256;
 constexpr int RAS_WARPS = RAS_THREADS / 32;
 constexpr int MASK_PITCH = 33;
+constexpr int RING = 64;                          // per-warp index ring (u16), drained 8 at a time (B_d, 8x unroll)
+constexpr int NULL_IDX = HIGS_BATCH_CAP;          // index of the "null" gaussian that pads the last drain
 
+// Shared-memory record of one staged gaussian, 64 B, laid out for packed f32x2 math: operands that multiply both
+// pixels of a lane sit duplicated in an aligned pair, so an LDS.128 lands them straight in an FFMA2 operand.
+//   f4[0] = mux, muy, A, B2      f4[1] = (C, C), (log2 o, log2 o)      f4[2] = (r, r), (g, g)      f4[3] = (b, b), tau, -
 struct __align__(16) RasSmem {
-    float4 rec[HIGS_BATCH_CAP * 3];               // 48 B per gaussian: mux,muy,A,B2 | C,tau,log2o,r | g,b,-,-
-    uint32_t masks[HIGS_MT_TILES * MASK_PITCH];   // [tile][mini-batch]
+    float4 rec[(HIGS_BATCH_CAP + 1) * 4];
+    uint32_t masks[HIGS_MT_TILES * MASK_PITCH];   // [tile][mini-batch]: bit j = gaussian k*32+j touches the tile
+    uint16_t ring[RAS_WARPS][RING];
     uint32_t unit, next_tile, active, cut;
 };
 
@@ -40,56 +46,80 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float sqrt_approx(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
-// Conservative render-tile overlap mask of one gaussian inside macro-tile (mtx, mty): the row scan
-// at 8-px cells on a threshold inflated by 1e-3 (internal; reading Q9 -- never compared
-// with the oracle, only required to keep every pixel centre with q <= tau).
-__device__ __forceinline__ uint32_t tile_mask(const float4 g0, const float4 g1, int mtx, int mty, const FrameParams& P)
+// Conservative render-tile overlap mask of one gaussian inside macro-tile (X0, Y0) (reading Q9:
+// internal, never compared with the oracle).  Row scan of the ellipse {q <= tau} written on the conic itself:
+//   dx(dy) = -h dy +- sqrt(tau/A - D dy^2),  h = B2/(2A),  D = det/A^2,  det = A C - B2^2/4,
+// with approximate rcp/sqrt; tau is inflated by 1e-3 and every pixel centre sits 0.5 px inside its tile, which
+// dwarfs the ~1e-6 relative error of the approximations.
+__device__ __forceinline__ uint32_t tile_mask_fast(float mux, float muy, float A, float B2, float C, float tau,
+                                                   float X0, float Y0, float fW, float fH)
 {
-    const float A = g0.z, B2 = g0.w, C = g1.x;
-    const float tau = g1.y * 1.001f;
     const float det = A * C - 0.25f * B2 * B2;
-    if (!(det > 0.0f)) return 0xffffffffu;
-    const float rd = 1.0f / det;
-    const float a = C * rd, b = -0.5f * B2 * rd, c = A * rd;
-    const int ncx = (P.W + HIGS_TILE - 1) / HIGS_TILE, ncy = (P.H + HIGS_TILE - 1) / HIGS_TILE;
-    RowScan rs;
-    rs.init(g0.x, g0.y, a, b, c, tau, (float)HIGS_TILE, ncy);
-    const int R0 = mty * 4, C0 = mtx * 8;
-    const int ra = max(rs.r0, R0), rb = min(rs.r1, R0 + 3);
+    if (!(det > 0.0f) || !(A > 0.0f)) return 0xffffffffu;
+    tau *= 1.001f;
+    const float rA = rcp_approx(A), rdet = rcp_approx(det);
+    const float h = 0.5f * B2 * rA;
+    const float D = det * rA * rA;
+    const float tA = tau * rA;
+    const float hx = sqrt_approx(tau * C * rdet), hy = sqrt_approx(tau * A * rdet);
+    const float yR = -0.5f * B2 * sqrt_approx(tau * rdet * rcp_approx(C));   // dy of the rightmost point
+    const float ytop = muy - hy, ybot = muy + hy;
     uint32_t mask = 0;
-    for (int r = ra; r <= rb; ++r) {
-        int m0, m1;
-        if (!rs.row(r, (float)HIGS_TILE, (float)HIGS_TILE, (float)P.W, (float)P.H, ncx, m0, m1)) continue;
-        m0 = max(m0, C0); m1 = min(m1, C0 + 7);
-        if (m0 > m1) continue;
-        const uint32_t bits = (2u << (m1 - C0)) - (1u << (m0 - C0));
-        mask |= bits << ((r - R0) * 8);
+#pragma unroll
+    for (int tr = 0; tr < 4; ++tr) {
+        const float y0 = Y0 + 8.0f * tr;
+        const float y1 = fminf(y0 + 8.0f, fH);
+        const float ylo = fmaxf(y0, ytop) - muy, yhi = fminf(y1, ybot) - muy;
+        if (!(yhi >= ylo)) continue;
+        const float rlo = sqrt_approx(fmaxf(0.0f, tA - D * ylo * ylo));
+        const float rhi = sqrt_approx(fmaxf(0.0f, tA - D * yhi * yhi));
+        float xmax = (ylo <= yR && yR <= yhi) ? hx : fmaxf(rlo - h * ylo, rhi - h * yhi);
+        float xmin = (ylo <= -yR && -yR <= yhi) ? -hx : fminf(-rlo - h * ylo, -rhi - h * yhi);
+        xmax = fminf(xmax + mux, fW) - X0; xmin = fmaxf(xmin + mux, 0.0f) - X0;
+        if (!(xmax >= 0.0f) || !(xmin < 64.0f) || !(xmax >= xmin)) continue;
+        const int c0 = max(0, (int)floorf(xmin * 0.125f)), c1 = min(7, (int)floorf(xmax * 0.125f));
+        if (c0 > c1) continue;
+        mask |= ((2u << c1) - (1u << c0)) << (tr * 8);
     }
     return mask;
 }
 
 template <bool COUNT>
-__global__ void __launch_bounds__(RAS_THREADS, 4)
-k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict__ ras,
+__global__ void __launch_bounds__(RAS_THREADS, 3)
+k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict__ rec,
          const uint32_t* __restrict__ mt_offset, const uint32_t* __restrict__ mt_count,
          const uint32_t* __restrict__ batch_offset, const uint32_t* __restrict__ unit_mt,
+         const uint32_t* __restrict__ unit_order,
          const FrameParams P, FrameHeader* __restrict__ hdr,
          float4* __restrict__ partial, uint32_t* __restrict__ unit_active, float* __restrict__ tile_maxT)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
     RasSmem& S = *reinterpret_cast<RasSmem*>(s_raw);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const uint32_t lt_mask = (1u << lane) - 1u;
     const uint32_t n_units = hdr->n_units;
     const bool use_cut = !(P.flags & HIGS_FLAG_NO_XBATCH_CUT);
+    const float fW = (float)P.W, fH = (float)P.H;
     unsigned long long n_eval_g = 0, n_tp = 0;
+    if (threadIdx.x == 0) {                                           // the null gaussian: tau < 0, never passes q <= tau
+        S.rec[NULL_IDX * 4] = make_float4(0.f, 0.f, 0.f, 0.f); S.rec[NULL_IDX * 4 + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+        S.rec[NULL_IDX * 4 + 2] = make_float4(0.f, 0.f, 0.f, 0.f); S.rec[NULL_IDX * 4 + 3] = make_float4(0.f, 0.f, -1.0f, 0.f);
+    }
+    uint16_t* ring = S.ring[w];
 
     for (;;) {
         __syncthreads();                                              // everyone is done with the previous unit's shared state
-        if (threadIdx.x == 0) { S.unit = atomicAdd(&hdr->raster_cursor, 1u); S.next_tile = 0; S.active = 0; S.cut = 0; }
+        if (threadIdx.x == 0) {
+            const uint32_t c = atomicAdd(&hdr->raster_cursor, 1u);
+            S.unit = c < n_units ? unit_order[c] : 0xffffffffu;
+            S.next_tile = 0; S.active = 0; S.cut = 0;
+        }
         __syncthreads();
         const uint32_t u = S.unit;
-        if (u >= n_units) break;
+        if (u == 0xffffffffu) break;
         const uint32_t m = unit_mt[u];
         const uint32_t u0 = batch_offset[m];
         const uint32_t j = u - u0;
@@ -97,24 +127,36 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
         const uint32_t start = mt_offset[m] + j * (uint32_t)P.batch_cap;
         const int len = (int)min((uint32_t)P.batch_cap, seg_n - j * (uint32_t)P.batch_cap);
         const int mtx = (int)(m % (uint32_t)P.n_mx), mty = (int)(m / (uint32_t)P.n_mx);
+        const float X0 = (float)(mtx * HIGS_MT_W), Y0 = (float)(mty * HIGS_MT_H);
 
-        // tiles wholly outside the image are never active (Alg. 1 line 11, InBounds)
-        const int tiles_x = min(8, (P.W - mtx * HIGS_MT_W + HIGS_TILE - 1) / HIGS_TILE);
-        const int tiles_y = min(4, (P.H - mty * HIGS_MT_H + HIGS_TILE - 1) / HIGS_TILE);
+        // ---- Phase 1a: start the gather of this unit's records (Alg. 1 line 4), first 48 B of each, by sorted id ----
+        for (int i = threadIdx.x; i < len; i += RAS_THREADS) {
+            const uint32_t id = (uint32_t)pairs[start + i];
+            const float4* src = rec + 4 * (size_t)id;
+            cp_async16(&S.rec[4 * i], src);
+            cp_async16(&S.rec[4 * i + 1], src + 1);
+            cp_async16(&S.rec[4 * i + 2], src + 2);
+        }
 
-        // cross-batch saturation cut-off: product over the earlier units of the largest transmittance
-        // they left in tile t bounds the transmittance in front of this unit
-        if (use_cut && j > 0 && w == 0) {
+        // tiles wholly outside the image are never active (Alg. 1 line 11, InBounds); cross-batch saturation
+        // cut-off: the product over the earlier units of this macro-tile of the largest transmittance they left
+        // in tile t bounds the transmittance in front of this unit
+        if (w == 0) {
+            const int tiles_x = min(8, (P.W - mtx * HIGS_MT_W + HIGS_TILE - 1) / HIGS_TILE);
+            const int tiles_y = min(4, (P.H - mty * HIGS_MT_H + HIGS_TILE - 1) / HIGS_TILE);
             float bound = 1.0f;
-            for (uint32_t jj = 0; jj < j; ++jj) {
-                const float v = __ldcg(tile_maxT + (size_t)(u0 + jj) * HIGS_MT_TILES + lane);
-                bound *= (v > 0.0f ? v : 1.0f);                       // 0 = not published yet
-                if (__all_sync(0xffffffffu, bound < HIGS_EPS_T)) break;
+            if (use_cut) {
+                for (uint32_t jj = 0; jj < j; ++jj) {
+                    const float v = __ldcg(tile_maxT + (size_t)(u0 + jj) * HIGS_MT_TILES + lane);
+                    bound *= (v > 0.0f ? v : 1.0f);                   // 0 = not published yet
+                    if (__all_sync(0xffffffffu, bound < HIGS_EPS_T)) break;
+                }
             }
             const bool inb = (lane & 7) < tiles_x && (lane >> 3) < tiles_y;
             const uint32_t cut = __ballot_sync(0xffffffffu, bound < HIGS_EPS_T || !inb);
             if (lane == 0) S.cut = cut;
         }
+        cp_async_wait_all();                                          // each thread waits for the records it asked for
         __syncthreads();
         const uint32_t cut = S.cut;
         if (cut == 0xffffffffu) {                                     // nothing left to see behind the earlier batches
@@ -122,79 +164,98 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             continue;
         }
 
-        // ---- Phase 1: gather records into shared memory ----
-        for (int i = threadIdx.x; i < len; i += RAS_THREADS) {
-            const uint32_t id = (uint32_t)pairs[start + i];
-            const float4* src = ras + 3 * (size_t)id;
-            cp_async16(&S.rec[3 * i], src);
-            cp_async16(&S.rec[3 * i + 1], src + 1);
-            cp_async16(&S.rec[3 * i + 2], src + 2);
-        }
-        cp_async_wait_all();
-        __syncthreads();
-        // per-gaussian tile masks, transposed by ballot: masks[t][k] bit jj = gaussian k*32+jj touches tile t
+        // ---- Phase 1b: per-gaussian tile masks (Alg. 1 lines 5-6), transposed by ballot; records re-laid for f32x2 ----
         for (int k = w; k < HIGS_BATCH_CAP / 32; k += RAS_WARPS) {
-            const int i = k * 32 + lane;
+            const int i = k * 32 + lane;                              // == threadIdx.x + 256*(k/8): the slot this thread gathered
+            if (k * 32 >= len) { S.masks[lane * MASK_PITCH + k] = 0; continue; }
             uint32_t gm = 0;
-            if (i < len) gm = tile_mask(S.rec[3 * i], S.rec[3 * i + 1], mtx, mty, P) & ~cut;
+            if (i < len) {
+                const float4 a = S.rec[4 * i], b = S.rec[4 * i + 1], c = S.rec[4 * i + 2];
+                gm = tile_mask_fast(a.x, a.y, a.z, a.w, b.x, b.y, X0, Y0, fW, fH) & ~cut;
+                S.rec[4 * i + 1] = make_float4(b.x, b.x, b.z, b.z);
+                S.rec[4 * i + 2] = make_float4(b.w, b.w, c.x, c.x);
+                S.rec[4 * i + 3] = make_float4(c.y, c.y, b.y, 0.0f);
+            }
             uint32_t mine = 0;
 #pragma unroll
             for (int t = 0; t < 32; ++t) {
-                const uint32_t b = __ballot_sync(0xffffffffu, (gm >> t) & 1u);
-                if (lane == t) mine = b;
+                const uint32_t bt = __ballot_sync(0xffffffffu, (gm >> t) & 1u);
+                if (lane == t) mine = bt;
             }
             S.masks[lane * MASK_PITCH + k] = mine;
         }
         __syncthreads();
 
-        // ---- Phase 2: warps claim render tiles ----
+        // ---- Phase 2: warps claim render tiles (Alg. 1 lines 9-17), RasterizeTile (Alg. 2) ----
         for (;;) {
             int t = 0;
             if (lane == 0) t = (int)atomicAdd(&S.next_tile, 1u);
             t = __shfl_sync(0xffffffffu, t, 0);
             if (t >= HIGS_MT_TILES) break;
             const uint32_t mine = S.masks[t * MASK_PITCH + lane];      // lane k holds mini-batch k's word
-            const uint32_t nonempty = __ballot_sync(0xffffffffu, mine != 0u);
-            if (!nonempty) continue;
-            const int tx = t & 7, ty = t >> 3;
-            const float pxf = (float)(mtx * HIGS_MT_W + tx * HIGS_TILE + (lane & 7)) + 0.5f;
-            const float py0 = (float)(mty * HIGS_MT_H + ty * HIGS_TILE + (lane >> 3)) + 0.5f;
+            uint32_t rest = __ballot_sync(0xffffffffu, mine != 0u);
+            if (!rest) continue;
+            const float pxf = X0 + (float)((t & 7) * HIGS_TILE + (lane & 7)) + 0.5f;
+            const float py0 = Y0 + (float)((t >> 3) * HIGS_TILE + (lane >> 3)) + 0.5f;
             const float py1 = py0 + 4.0f;
-            float T0 = 1.0f, T1 = 1.0f, r0 = 0, g0c = 0, b0c = 0, r1 = 0, g1c = 0, b1c = 0;
-            uint32_t rest = nonempty;
-            while (rest) {
-                const int k = __ffs(rest) - 1;
-                rest &= rest - 1;
-                uint32_t bits = __shfl_sync(0xffffffffu, mine, k);
-                if (COUNT) n_tp += __popc(bits);
-                do {
-                    const int i = k * 32 + __ffs(bits) - 1;
-                    bits &= bits - 1;
-                    const float4 a = S.rec[3 * i], bq = S.rec[3 * i + 1], cq = S.rec[3 * i + 2];
-                    // N-Q, pinned: dx, u = A dx, a0 = u dx, b0 = B2 dx, t = fma(C, dy, b0), q = fma(t, dy, a0)
+            float2 T2 = make_float2(1.0f, 1.0f), r2 = make_float2(0.f, 0.f), g2 = r2, b2 = r2;
+            const float2 kexp = make_float2(-0.72134752f, -0.72134752f), neg1 = make_float2(-1.0f, -1.0f);
+            uint32_t wr = 0, rd = 0;
+            bool sat = false;
+            // one drain: 8 ring entries starting at rd (a multiple of 8), composited in order
+            auto drain8 = [&]() {
+                const uint4 pk = *reinterpret_cast<const uint4*>(ring + (rd & (RING - 1)));
+                const uint32_t pkw[4] = { pk.x, pk.y, pk.z, pk.w };
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                    const uint32_t idx = (e & 1) ? (pkw[e >> 1] >> 16) : (pkw[e >> 1] & 0xffffu);
+                    const float4* gp = S.rec + 4 * idx;
+                    const float4 a = gp[0], bq = gp[1], cq = gp[2], dq = gp[3];
+                    // N-Q, pinned (DESIGN.md section 3): dx, u = A dx, a0 = u dx, b0 = B2 dx, t = fma(C, dy, b0), q = fma(t, dy, a0)
                     const float dx = __fsub_rn(pxf, a.x);
                     const float uu = __fmul_rn(a.z, dx);
                     const float a0 = __fmul_rn(uu, dx);
                     const float bb = __fmul_rn(a.w, dx);
-                    const float dy0 = __fsub_rn(py0, a.y), dy1 = __fsub_rn(py1, a.y);
-                    const float q0 = __fmaf_rn(__fmaf_rn(bq.x, dy0, bb), dy0, a0);
-                    const float q1 = __fmaf_rn(__fmaf_rn(bq.x, dy1, bb), dy1, a0);
-                    float al0 = fminf(HIGS_ALPHA_MAX, ex2_approx(fmaf(q0, -0.72134752f, bq.z)));
-                    float al1 = fminf(HIGS_ALPHA_MAX, ex2_approx(fmaf(q1, -0.72134752f, bq.z)));
-                    al0 = (q0 <= bq.y) ? al0 : 0.0f;                  // alpha < 1/255: skipped
-                    al1 = (q1 <= bq.y) ? al1 : 0.0f;
-                    const float w0 = T0 * al0, w1 = T1 * al1;
-                    r0 = fmaf(w0, bq.w, r0); g0c = fmaf(w0, cq.x, g0c); b0c = fmaf(w0, cq.y, b0c);
-                    r1 = fmaf(w1, bq.w, r1); g1c = fmaf(w1, cq.x, g1c); b1c = fmaf(w1, cq.y, b1c);
-                    T0 -= w0; T1 -= w1;
-                    if (COUNT) ++n_eval_g;
-                } while (bits);
-                if (__all_sync(0xffffffffu, T0 < HIGS_EPS_T && T1 < HIGS_EPS_T)) break;   // Alg. 2 line 8
+                    const float2 dy = make_float2(__fsub_rn(py0, a.y), __fsub_rn(py1, a.y));
+                    const float2 tq = __ffma2_rn(make_float2(bq.x, bq.y), dy, make_float2(bb, bb));
+                    const float2 q = __ffma2_rn(tq, dy, make_float2(a0, a0));
+                    const float2 ex = __ffma2_rn(q, kexp, make_float2(bq.z, bq.w));
+                    float al0 = fminf(HIGS_ALPHA_MAX, ex2_approx(ex.x));
+                    float al1 = fminf(HIGS_ALPHA_MAX, ex2_approx(ex.y));
+                    al0 = (q.x <= dq.z) ? al0 : 0.0f;                 // alpha < 1/255: skipped
+                    al1 = (q.y <= dq.z) ? al1 : 0.0f;
+                    const float2 wgt = __fmul2_rn(T2, make_float2(al0, al1));
+                    r2 = __ffma2_rn(wgt, make_float2(cq.x, cq.y), r2);
+                    g2 = __ffma2_rn(wgt, make_float2(cq.z, cq.w), g2);
+                    b2 = __ffma2_rn(wgt, make_float2(dq.x, dq.y), b2);
+                    T2 = __ffma2_rn(wgt, neg1, T2);
+                }
+                rd += 8;
+            };
+            while (rest) {
+                const int k = __ffs(rest) - 1;
+                rest &= rest - 1;
+                const uint32_t bits = __shfl_sync(0xffffffffu, mine, k);
+                if ((bits >> lane) & 1u) ring[(wr + __popc(bits & lt_mask)) & (RING - 1)] = (uint16_t)(k * 32 + lane);
+                wr += __popc(bits);
+                __syncwarp();
+                while (wr - rd >= 8u) {
+                    drain8();
+                    if (__all_sync(0xffffffffu, fmaxf(T2.x, T2.y) < HIGS_EPS_T)) { sat = true; break; }   // Alg. 2 line 8
+                }
+                if (sat) break;
             }
+            if (!sat && wr > rd) {                                    // flush: pad the last drain with the null gaussian
+                if (lane < 8) ring[(wr + lane) & (RING - 1)] = (uint16_t)NULL_IDX;
+                __syncwarp();
+                drain8();
+            }
+            __syncwarp();                                             // ring reads done before the next tile's writes
+            if (COUNT) { n_tp += wr; n_eval_g += min(rd, wr); }
             float4* out = partial + ((size_t)u * HIGS_MT_TILES + t) * 64;
-            __stcs(out + lane, make_float4(r0, g0c, b0c, T0));
-            __stcs(out + 32 + lane, make_float4(r1, g1c, b1c, T1));
-            float tm = fmaxf(T0, T1);
+            __stcs(out + lane, make_float4(r2.x, g2.x, b2.x, T2.x));
+            __stcs(out + 32 + lane, make_float4(r2.y, g2.y, b2.y, T2.y));
+            float tm = fmaxf(T2.x, T2.y);
 #pragma unroll
             for (int d = 16; d > 0; d >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, d));
             if (lane == 0) {
@@ -263,11 +324,11 @@ int launch_raster(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
     const int smem = (int)sizeof(RasSmem);
     const int grid = ctx->n_sm * g_raster_ctas_per_sm;
     if (P.flags & HIGS_FLAG_COUNT_EVALS)
-        k_raster<true><<<grid, RAS_THREADS, smem, st>>>(ctx->pairs, ctx->ras, ctx->mt_offset, ctx->mt_count, ctx->batch_offset,
-                                                        ctx->unit_mt, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_maxT);
+        k_raster<true><<<grid, RAS_THREADS, smem, st>>>(ctx->pairs, ctx->rec, ctx->mt_offset, ctx->mt_count, ctx->batch_offset,
+                                                        ctx->unit_mt, ctx->unit_order, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_maxT);
     else
-        k_raster<false><<<grid, RAS_THREADS, smem, st>>>(ctx->pairs, ctx->ras, ctx->mt_offset, ctx->mt_count, ctx->batch_offset,
-                                                         ctx->unit_mt, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_maxT);
+        k_raster<false><<<grid, RAS_THREADS, smem, st>>>(ctx->pairs, ctx->rec, ctx->mt_offset, ctx->mt_count, ctx->batch_offset,
+                                                         ctx->unit_mt, ctx->unit_order, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_maxT);
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }

@@ -35,19 +35,18 @@ def _check_records(rec, pr):
     valid = rec["valid"]
     assert np.array_equal(valid, pr.valid.astype(bool))
     v = np.nonzero(valid)[0]
-    geo, ras = rec["geo"][v], rec["ras"][v]
+    r = rec["rec"][v]        # mux, muy, A, B2, C, tau, log2 o, r, g, b, key, -, -, a, b, c
+    bits = lambda x: np.ascontiguousarray(x).view(np.uint32)
     # decision-feeding values: bit-exact
-    for col, ocol in [(0, 0), (1, 1), (2, 2), (3, 3), (4, 4), (5, 5)]:
-        assert np.array_equal(geo[:, col].view(np.uint32), pr.geo[v, ocol].view(np.uint32)), f"geo column {col}"
-    assert np.array_equal(geo[:, 6].view(np.uint32), pr.key[v])
-    assert np.array_equal(ras[:, 0].view(np.uint32), pr.geo[v, 0].view(np.uint32))
-    assert np.array_equal(ras[:, 1].view(np.uint32), pr.geo[v, 1].view(np.uint32))
+    assert np.array_equal(bits(r[:, 0]), bits(pr.geo[v, 0])) and np.array_equal(bits(r[:, 1]), bits(pr.geo[v, 1])), "mu"
     for col in range(3):
-        assert np.array_equal(ras[:, 2 + col].view(np.uint32), pr.conic[v, col].view(np.uint32)), f"conic {col}"
-    assert np.array_equal(ras[:, 5].view(np.uint32), pr.geo[v, 5].view(np.uint32))
+        assert np.array_equal(bits(r[:, 2 + col]), bits(pr.conic[v, col])), f"conic {col}"
+        assert np.array_equal(bits(r[:, 13 + col]), bits(pr.geo[v, 2 + col])), f"covariance {col}"
+    assert np.array_equal(bits(r[:, 5]), bits(pr.geo[v, 5])), "tau"
+    assert np.array_equal(bits(r[:, 10]), pr.key[v]), "depth key"
     # smooth values
-    np.testing.assert_allclose(ras[:, 6], np.log2(pr.opac[v].astype(np.float64)), atol=2e-6, rtol=2e-6)
-    np.testing.assert_allclose(ras[:, 7:10], pr.rgb[v], atol=RGB_TOL, rtol=RGB_TOL)
+    np.testing.assert_allclose(r[:, 6], np.log2(pr.opac[v].astype(np.float64)), atol=2e-6, rtol=2e-6)
+    np.testing.assert_allclose(r[:, 7:10], pr.rgb[v], atol=RGB_TOL, rtol=RGB_TOL)
 
 
 def _check_lists(ls, ols):
