@@ -194,6 +194,11 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     memset(ctx->hdr_host, 0, sizeof(FrameHeader));
     if (cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(HIGS_E_CUDA);
     for (int i = 0; i < 9; ++i) if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) return fail(HIGS_E_CUDA);
+    for (int i = 0; i < 3; ++i) {
+        if (cudaStreamCreateWithFlags(&ctx->aux_stream[i], cudaStreamNonBlocking) != cudaSuccess) return fail(HIGS_E_CUDA);
+        if (cudaEventCreateWithFlags(&ctx->ev_join[i], cudaEventDisableTiming) != cudaSuccess) return fail(HIGS_E_CUDA);
+    }
+    if (cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess) return fail(HIGS_E_CUDA);
     if ((rc = higs_project_smem_setup(ctx))) return fail(rc);
     if ((rc = higs_binning_smem_setup(ctx))) return fail(rc);
     if ((rc = higs_sort_smem_setup(ctx))) return fail(rc);
@@ -218,6 +223,11 @@ void higs_destroy(higs_ctx* ctx)
     if (ctx->hdr_host) cudaFreeHost(ctx->hdr_host);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     for (int i = 0; i < 9; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    for (int i = 0; i < 3; ++i) {
+        if (ctx->aux_stream[i]) cudaStreamDestroy(ctx->aux_stream[i]);
+        if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     cudaGetLastError();
     delete ctx;
 }

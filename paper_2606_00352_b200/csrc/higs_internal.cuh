@@ -87,6 +87,8 @@ struct higs_ctx {
     int64_t last_n; int last_W, last_H, last_nm; int last_mx, last_my;
     cudaStream_t last_stream;
     cudaStream_t own_stream;
+    cudaStream_t aux_stream[3];   // forked from the render stream for the small sort tiers
+    cudaEvent_t ev_fork, ev_join[3];
     cudaEvent_t ev[9];
     bool timers_valid;
     int n_launches;            // kernels enqueued by the current / last frame

@@ -1,13 +1,17 @@
 // sort.cu -- step a5: segmented depth sort (section 3.3, section 4.4).
 //
 // One segment per macro-tile, items are 64-bit (depth key << 32 | gaussian id); the required order
-// is ascending (key, id) (reading Q7), i.e. ascending as unsigned 64-bit integers.
-//   * tier cascade: segments of <= 1024 / 2048 / 4096 / 8192 items are sorted by ONE CTA in shared
-//     memory (CTA 128 / 256 / 512 / 1024 threads), four stable 8-bit LSD radix passes on the depth
-//     key, passes whose digit is constant over the segment are skipped, then
-//     equal-key runs (rare) are put in id order by an odd-even transposition confined to the run;
-//   * overflow path: longer segments are cut into 8192-item blocks sorted by the top tier, then
-//     merged level by level (run size doubling) with merge-path partitioning.
+// is ascending (key, id) (reading Q7), i.e. ascending as unsigned 64-bit integers.  Ids are
+// unique inside a segment, so all items are distinct and no stability question arises.
+//   * tier cascade: segments of <= 1024 / 2048 / 4096 / 8192 items are sorted by ONE
+//     CTA of 64 / 128 / 256 / 512 threads, 16 items per thread.  Where the paper runs four 8-bit radix
+//     passes, this build runs a block merge sort on the whole 64-bit item: a 63-exchange Batcher network
+//     in registers, then log2(threads) merge-path levels through shared memory.  It needs no tie pass for
+//     equal depth keys and its cost does not depend on the key distribution.
+//     The four tier kernels run concurrently on forked streams (the paper overlaps them with PDL).
+//   * overflow path: longer segments are cut into 8192-item blocks sorted by the top
+//     tier, then merged level by level (run length doubling) with merge-path partitioning, the
+//     partition points found by a warp-cooperative 32-ary search.
 // All sizes are read from device memory; the kernels are persistent over device work counters, so
 // nothing here needs a host synchronisation.
 #include <stdio.h>
@@ -19,6 +23,7 @@ typedef unsigned long long u64;
 
 namespace {
 
+constexpr int IPT = 16;                                   // items per thread of the block sort
 __device__ __forceinline__ int tier_of(uint32_t n) { return n <= 1024u ? 0 : (n <= 2048u ? 1 : (n <= 4096u ? 2 : 3)); }
 
 // ---- sort plan: job lists per tier + merge plan for oversize segments -------------------------
@@ -82,7 +87,7 @@ k_sort_plan(const uint32_t* __restrict__ seg_offset, int n_seg, int honour_overf
                 atomicMax(&s_maxlev, levels);
             }
         }
-        const uint32_t cnt3 = v[3], tiles = v[5];
+        const uint32_t cnt3 = v[3];
         const int t = n > 1 ? (n <= HIGS_SORT_BLOCK ? tier_of(n) : 3) : -1;
         plan_scan<6>(v, carry, s_warp);
         if (t >= 0) {
@@ -94,7 +99,6 @@ k_sort_plan(const uint32_t* __restrict__ seg_offset, int n_seg, int honour_overf
                     jobs[(size_t)3 * max_jobs + v[3] + c] = SortJob{start + cs, min((uint32_t)HIGS_SORT_BLOCK, n - cs), levels & 1u, 0u};
                 }
                 over[v[4]] = OverSeg{start, n, levels, v[5]};
-                (void)tiles;
             }
         }
     }
@@ -107,98 +111,101 @@ k_sort_plan(const uint32_t* __restrict__ seg_offset, int n_seg, int honour_overf
     }
 }
 
-// ---- tier kernel: one CTA sorts one segment (or one 8192-item block) in shared memory ---------
-template <int CAP, int THREADS>
+// ---- tier kernel: one CTA sorts one segment (or one 8192-item block) -----------------------------
+__device__ __forceinline__ void cex(u64& a, u64& b)
+{
+    const bool sw = b < a;
+    const u64 lo = sw ? b : a, hi = sw ? a : b;
+    a = lo; b = hi;
+}
+
+// Batcher's odd-even merge sort network for 16 items: 63 compare-exchanges, written out so that every
+// index is static and the items stay in registers
+__device__ __forceinline__ void reg_sort16(u64 (&v)[IPT])
+{
+#define X(a, b) cex(v[a], v[b]);
+    X(0,1) X(2,3) X(4,5) X(6,7) X(8,9) X(10,11) X(12,13) X(14,15)
+    X(0,2) X(1,3) X(4,6) X(5,7) X(8,10) X(9,11) X(12,14) X(13,15)
+    X(1,2) X(5,6) X(9,10) X(13,14) X(0,4) X(1,5) X(2,6) X(3,7)
+    X(8,12) X(9,13) X(10,14) X(11,15) X(2,4) X(3,5) X(10,12) X(11,13)
+    X(1,2) X(3,4) X(5,6) X(9,10) X(11,12) X(13,14) X(0,8) X(1,9)
+    X(2,10) X(3,11) X(4,12) X(5,13) X(6,14) X(7,15) X(4,8) X(5,9)
+    X(6,10) X(7,11) X(2,4) X(3,5) X(6,8) X(7,9) X(10,12) X(11,13)
+    X(1,2) X(3,4) X(5,6) X(7,8) X(9,10) X(11,12) X(13,14)
+#undef X
+}
+
+// shared-memory index with one padding slot per 16 items: thread t's blocked items t*16.. start at
+// t*17, so a half-warp's 64-bit accesses to "item k of each thread" fall in 16 distinct bank pairs
+__device__ __forceinline__ int sidx(int i) { return i + (i >> 4); }
+
+template <int THREADS>
 __global__ void __launch_bounds__(THREADS)
 k_block_sort(const SortJob* __restrict__ jobs, FrameHeader* __restrict__ hdr, int tier,
              u64* __restrict__ pairs, u64* __restrict__ pairs_alt)
 {
-    constexpr int NW = THREADS / 32;
+    constexpr int CAP = THREADS * IPT;
     extern __shared__ __align__(16) unsigned char s_raw[];
-    u64* buf0 = reinterpret_cast<u64*>(s_raw);
-    u64* buf1 = buf0 + CAP;
-    uint32_t* cnt = reinterpret_cast<uint32_t*>(buf1 + CAP);      // [NW][256]
-    uint32_t* dbase = cnt + NW * 256;                             // [256] exclusive digit bases
+    u64* buf = reinterpret_cast<u64*>(s_raw);                     // sidx(CAP) items
     __shared__ uint32_t s_job;
-    __shared__ int s_skip;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const uint32_t lt_mask = (1u << lane) - 1u;
+    const int t = threadIdx.x;
 
     for (;;) {
-        if (threadIdx.x == 0) s_job = atomicAdd(&hdr->sort_cursor[tier], 1u);
+        __syncthreads();                                         // previous job's shared state is free
+        if (t == 0) s_job = atomicAdd(&hdr->sort_cursor[tier], 1u);
         __syncthreads();
         const uint32_t jb = s_job;
         if (jb >= hdr->n_sort_jobs[tier]) return;
         const SortJob job = jobs[jb];
         const int n = (int)job.len;
-        u64* gsrc = pairs + job.start;
-        for (int i = threadIdx.x; i < n; i += THREADS) buf0[i] = gsrc[i];
-        u64* src = buf0; u64* dst = buf1;
-        const int per = (((n + NW - 1) / NW) + 31) & ~31;         // contiguous chunk per warp, multiple of 32
-        const int beg = min(n, w * per), end = min(n, beg + per);
-
-        for (int pass = 0; pass < 4; ++pass) {
-            const int shift = 32 + 8 * pass;
-            for (int i = threadIdx.x; i < NW * 256; i += THREADS) cnt[i] = 0;
-            __syncthreads();                                     // also covers the load of buf0
-            for (int v = beg + lane; v < end; v += 32)
-                atomicAdd(&cnt[w * 256 + (int)((src[v] >> shift) & 255u)], 1u);
-            __syncthreads();
-            for (int d = threadIdx.x; d < 256; d += THREADS) {    // per digit: exclusive scan over warps
-                uint32_t run = 0;
-#pragma unroll
-                for (int ww = 0; ww < NW; ++ww) { const uint32_t t = cnt[ww * 256 + d]; cnt[ww * 256 + d] = run; run += t; }
-                dbase[d] = run;
-            }
-            __syncthreads();
-            if (w == 0) {                                        // exclusive scan over the 256 digit totals
-                uint32_t t[8], sum = 0; bool full = false;
-#pragma unroll
-                for (int k = 0; k < 8; ++k) { t[k] = dbase[lane * 8 + k]; full |= (t[k] == (uint32_t)n); sum += t[k]; }
-                uint32_t x = sum;
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
-                uint32_t run = x - sum;
-#pragma unroll
-                for (int k = 0; k < 8; ++k) { dbase[lane * 8 + k] = run; run += t[k]; }
-                const bool any_full = __any_sync(0xffffffffu, full);
-                if (lane == 0) s_skip = any_full ? 1 : 0;
-            }
-            __syncthreads();
-            if (s_skip) continue;                                // digit constant over the segment: nothing moves
-            for (int vb = beg; vb < end; vb += 32) {             // stable scatter, warp walks its chunk in order
-                const int v = vb + lane;
-                const bool act = v < end;
-                const u64 item = act ? src[v] : 0ull;
-                const uint32_t d = act ? (uint32_t)((item >> shift) & 255u) : (256u + (uint32_t)lane);
-                const uint32_t peers = __match_any_sync(0xffffffffu, d);
-                const uint32_t rank = __popc(peers & lt_mask);
-                uint32_t pos = 0;
-                if (act) pos = cnt[w * 256 + d] + dbase[d] + rank;
-                __syncwarp();
-                if (act && rank == 0) cnt[w * 256 + d] += __popc(peers);
-                __syncwarp();
-                if (act) dst[pos] = item;
-            }
-            __syncthreads();
-            u64* tmp = src; src = dst; dst = tmp;
-        }
-        // equal depth keys: order by id (odd-even transposition confined to equal-key neighbours)
-        for (;;) {
-            int swapped = 0;
-#pragma unroll
-            for (int phase = 0; phase < 2; ++phase) {
-                for (int i = 2 * threadIdx.x + phase; i + 1 < n; i += 2 * THREADS) {
-                    const u64 a = src[i], b = src[i + 1];
-                    if ((a >> 32) == (b >> 32) && a > b) { src[i] = b; src[i + 1] = a; swapped = 1; }
-                }
-                __syncthreads();
-            }
-            if (!__syncthreads_or(swapped)) break;
-        }
-        u64* gdst = (job.dst_alt ? pairs_alt : pairs) + job.start;
-        for (int i = threadIdx.x; i < n; i += THREADS) gdst[i] = src[i];
+        const u64* gsrc = pairs + job.start;
+        const int n_pad = min(CAP, ((n + IPT - 1) / IPT) * IPT);  // whole threads
+        for (int i = t; i < n_pad; i += THREADS) buf[sidx(i)] = i < n ? gsrc[i] : ~0ull;
         __syncthreads();
+        u64 v[IPT];
+        const bool live = t * IPT < n;                           // threads past the data hold nothing
+        if (live) {
+#pragma unroll
+            for (int k = 0; k < IPT; ++k) v[k] = buf[t * (IPT + 1) + k];
+            reg_sort16(v);
+        }
+        // merge levels: sorted runs of `run` items -> 2*run, each live thread produces its own 16 outputs
+        for (int run = IPT; run < n; run <<= 1) {
+            __syncthreads();
+            if (live) {
+#pragma unroll
+                for (int k = 0; k < IPT; ++k) buf[t * (IPT + 1) + k] = v[k];
+            }
+            __syncthreads();
+            if (live) {
+                const int o0 = t * IPT;
+                const int pb = o0 & ~(2 * run - 1);              // start of this pair of runs
+                const int na = min(run, n_pad - pb), nb = max(0, min(run, n_pad - pb - run));
+                const int A = pb, B = pb + run, diag = o0 - pb;
+                int lo = max(0, diag - nb), hi = min(diag, na);
+                while (lo < hi) {                                // merge path: first `diag` outputs take `lo` items of A
+                    const int mid = (lo + hi) >> 1;
+                    if (buf[sidx(A + mid)] < buf[sidx(B + diag - 1 - mid)]) lo = mid + 1; else hi = mid;
+                }
+                int ia = lo, ib = diag - lo;
+                u64 ka = ia < na ? buf[sidx(A + ia)] : ~0ull, kb = ib < nb ? buf[sidx(B + ib)] : ~0ull;
+#pragma unroll
+                for (int k = 0; k < IPT; ++k) {
+                    const bool take_a = ib >= nb || (ia < na && ka < kb);
+                    v[k] = take_a ? ka : kb;
+                    if (take_a) { ++ia; ka = ia < na ? buf[sidx(A + ia)] : ~0ull; }
+                    else        { ++ib; kb = ib < nb ? buf[sidx(B + ib)] : ~0ull; }
+                }
+            }
+        }
+        __syncthreads();
+        if (live) {
+#pragma unroll
+            for (int k = 0; k < IPT; ++k) buf[t * (IPT + 1) + k] = v[k];
+        }
+        __syncthreads();
+        u64* gdst = (job.dst_alt ? pairs_alt : pairs) + job.start;
+        for (int i = t; i < n; i += THREADS) gdst[i] = buf[sidx(i)];
     }
 }
 
@@ -214,6 +221,23 @@ __device__ __forceinline__ int merge_path(const u64* A, int na, const u64* B, in
     return lo;
 }
 
+// The same search done by one warp on global memory, 32 probes per step instead of one.  The predicate
+// A[mid] < B[diag-1-mid] is monotone in mid (true ... true false ... false); the answer is the first false.
+__device__ __forceinline__ int merge_path_warp(const u64* A, int na, const u64* B, int nb, int diag, int lane)
+{
+    int lo = max(0, diag - nb), hi = min(diag, na);              // answer in [lo, hi]
+    while (lo < hi) {
+        const int step = (hi - lo + 31) >> 5;
+        const int mid = min(hi - 1, lo + step * (lane + 1) - 1); // lane 31 always probes hi-1
+        const uint32_t bal = __ballot_sync(0xffffffffu, A[mid] < B[diag - 1 - mid]);
+        const int ff = bal == 0xffffffffu ? 32 : __ffs(~bal) - 1;   // first probe that answered false
+        const int new_lo = ff == 0 ? lo : min(hi - 1, lo + step * ff - 1) + 1;
+        const int new_hi = ff == 32 ? hi : min(hi - 1, lo + step * (ff + 1) - 1);
+        lo = new_lo; hi = new_hi;
+    }
+    return lo;
+}
+
 constexpr int MERGE_THREADS = 512;
 constexpr int MERGE_ITEMS = HIGS_MERGE_TILE / MERGE_THREADS;
 
@@ -224,6 +248,7 @@ k_merge_levels(const OverSeg* __restrict__ over, const FrameHeader* __restrict__
     __shared__ u64 s_in[HIGS_MERGE_TILE];
     __shared__ int s_part[4];
     const uint32_t n_tiles = hdr->n_merge_tiles, n_over = hdr->n_oversize, max_levels = hdr->max_levels;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     for (uint32_t lev = 0; lev < max_levels; ++lev) {
         for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
             int lo = 0, hi = (int)n_over - 1;                     // last segment with tile_base <= tile
@@ -239,9 +264,10 @@ k_merge_levels(const OverSeg* __restrict__ over, const FrameHeader* __restrict__
             const uint32_t a_beg = ps, a_end = min(sg.len, ps + run), b_end = min(sg.len, ps + 2u * run);
             const u64* A = src + a_beg; const int na = (int)(a_end - a_beg);
             const u64* B = src + a_end; const int nb = (int)(b_end - a_end);
-            if (threadIdx.x < 2) {
-                const int diag = (int)((threadIdx.x == 0 ? o0 : o1) - ps);
-                s_part[threadIdx.x] = merge_path(A, na, B, nb, diag);
+            if (wid < 2) {                                        // warp 0: tile start, warp 1: tile end
+                const int diag = (int)((wid == 0 ? o0 : o1) - ps);
+                const int a = merge_path_warp(A, na, B, nb, diag, lane);
+                if (lane == 0) s_part[wid] = a;
             }
             __syncthreads();
             const int a0 = s_part[0], a1 = s_part[1];
@@ -273,16 +299,28 @@ k_merge_levels(const OverSeg* __restrict__ over, const FrameHeader* __restrict__
 }
 
 int g_merge_ctas_per_sm = 1;
+int g_tier_ctas_per_sm[HIGS_N_TIERS] = {1, 1, 1, 1};
 
-template <int CAP, int THREADS>
-constexpr size_t sort_smem() { return (size_t)CAP * 16 + (size_t)(THREADS / 32) * 256 * 4 + 256 * 4; }
+template <int THREADS>
+constexpr size_t sort_smem() { return (size_t)(THREADS * IPT + THREADS) * sizeof(u64); }
 
-template <int CAP, int THREADS>
-int launch_tier(higs_ctx* ctx, int tier, int ctas, u64* pairs, cudaStream_t st)
+template <int THREADS>
+int launch_tier(higs_ctx* ctx, int tier, u64* pairs, cudaStream_t st)
 {
-    k_block_sort<CAP, THREADS><<<ctas, THREADS, sort_smem<CAP, THREADS>(), st>>>(
+    const int ctas = ctx->n_sm * g_tier_ctas_per_sm[tier];
+    k_block_sort<THREADS><<<ctas, THREADS, sort_smem<THREADS>(), st>>>(
         ctx->sort_jobs + (size_t)tier * ctx->max_jobs, ctx->hdr, tier, pairs, ctx->pairs_alt);
     HIGS_LAUNCHED(ctx);
+    return HIGS_OK;
+}
+
+template <int THREADS>
+int setup_tier(higs_ctx* ctx, int tier)
+{
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_block_sort<THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_smem<THREADS>()));
+    int occ = 0;
+    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_block_sort<THREADS>, THREADS, sort_smem<THREADS>()));
+    g_tier_ctas_per_sm[tier] = occ < 1 ? 1 : occ;
     return HIGS_OK;
 }
 
@@ -290,15 +328,22 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, i
 {
     k_sort_plan<<<1, 1024, 0, st>>>(seg_offset, n_seg, honour_overflow, ctx->sort_jobs, (size_t)ctx->max_jobs, ctx->over_segs, ctx->hdr);
     HIGS_LAUNCHED(ctx);
+    // fork: the three small tiers run beside the top tier + overflow merge (the paper overlaps tiers with PDL)
     int rc;
-    if ((rc = launch_tier<1024, 128>(ctx, 0, ctx->n_sm * 8, pairs, st))) return rc;
-    if ((rc = launch_tier<2048, 256>(ctx, 1, ctx->n_sm * 4, pairs, st))) return rc;
-    if ((rc = launch_tier<4096, 512>(ctx, 2, ctx->n_sm * 2, pairs, st))) return rc;
-    if ((rc = launch_tier<8192, 1024>(ctx, 3, ctx->n_sm, pairs, st))) return rc;
+    HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_fork, st));
+    for (int k = 0; k < 3; ++k) HIGS_CUDA(ctx, cudaStreamWaitEvent(ctx->aux_stream[k], ctx->ev_fork, 0));
+    if ((rc = launch_tier<512>(ctx, 3, pairs, st))) return rc;
+    if ((rc = launch_tier<256>(ctx, 2, pairs, ctx->aux_stream[0]))) return rc;
+    if ((rc = launch_tier<128>(ctx, 1, pairs, ctx->aux_stream[1]))) return rc;
+    if ((rc = launch_tier<64>(ctx, 0, pairs, ctx->aux_stream[2]))) return rc;
     const OverSeg* over = ctx->over_segs; const FrameHeader* hdr = ctx->hdr; u64* alt = ctx->pairs_alt;
     void* args[] = { (void*)&over, (void*)&hdr, (void*)&pairs, (void*)&alt };
     HIGS_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)k_merge_levels, dim3(ctx->n_sm * g_merge_ctas_per_sm), dim3(MERGE_THREADS), args, 0, st));
     ++ctx->n_launches;
+    for (int k = 0; k < 3; ++k) {
+        HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_join[k], ctx->aux_stream[k]));
+        HIGS_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_join[k], 0));
+    }
     return HIGS_OK;
 }
 
@@ -306,10 +351,11 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, i
 
 int higs_sort_smem_setup(higs_ctx* ctx)
 {
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_block_sort<1024, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_smem<1024, 128>()));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_block_sort<2048, 256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_smem<2048, 256>()));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_block_sort<4096, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_smem<4096, 512>()));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_block_sort<8192, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_smem<8192, 1024>()));
+    int rc;
+    if ((rc = setup_tier<64>(ctx, 0))) return rc;
+    if ((rc = setup_tier<128>(ctx, 1))) return rc;
+    if ((rc = setup_tier<256>(ctx, 2))) return rc;
+    if ((rc = setup_tier<512>(ctx, 3))) return rc;
     int occ = 0;
     HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_merge_levels, MERGE_THREADS, 0));
     g_merge_ctas_per_sm = occ < 1 ? 1 : (occ > 2 ? 2 : occ);
