@@ -10,6 +10,8 @@ int higs_binning_smem_setup(higs_ctx*);
 int higs_project_smem_setup(higs_ctx*);
 int higs_sort_smem_setup(higs_ctx*);
 int higs_raster_setup(higs_ctx*);
+int launch_export_lists(higs_ctx*, uint32_t n_pairs, cudaStream_t);      // binning.cu: pairs (key, slot) -> pairs_alt (key, id)
+int launch_export_records(higs_ctx*, int64_t N, cudaStream_t);           // binning.cu: rec[slot] -> rec_export[id]
 
 namespace {
 
@@ -175,7 +177,10 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     const int n_groups_max = (ctx->n_part_batches_max + 31) / 32;
     const size_t pitch = ((size_t)nm + 1) & ~(size_t)1;
     if ((rc = dev_alloc(ctx, &ctx->valid_bits, (size_t)(n + 31) / 32 + 1))) return fail(rc);
-    if ((rc = dev_alloc(ctx, &ctx->rec, (size_t)n * 4))) return fail(rc);
+    const size_t n_slots = (size_t)ctx->n_part_batches_max * HIGS_PART_BATCH;
+    if ((rc = dev_alloc(ctx, &ctx->rec, n_slots * 4))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->bin, n_slots))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->chunk_count, (size_t)ctx->n_part_batches_max * (HIGS_PART_BATCH / HIGS_CHUNK)))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->hist, (size_t)ctx->n_part_batches_max * pitch))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->base, (size_t)(ctx->n_part_batches_max + n_groups_max) * nm))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->mt_count, (size_t)nm + 1))) return fail(rc);
@@ -213,7 +218,7 @@ void higs_destroy(higs_ctx* ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
-    dev_free(ctx->valid_bits); dev_free(ctx->rec); dev_free(ctx->hist); dev_free(ctx->base);
+    dev_free(ctx->valid_bits); dev_free(ctx->rec); dev_free(ctx->bin); dev_free(ctx->chunk_count); dev_free(ctx->rec_export); dev_free(ctx->hist); dev_free(ctx->base);
     dev_free(ctx->mt_count); dev_free(ctx->mt_offset); dev_free(ctx->batch_offset); dev_free(ctx->unit_mt);
     dev_free(ctx->unit_active); dev_free(ctx->pairs); dev_free(ctx->pairs_alt); dev_free(ctx->sort_jobs);
     dev_free(ctx->over_segs); dev_free(ctx->partial); dev_free(ctx->tile_maxT); dev_free(ctx->hdr);
@@ -341,9 +346,14 @@ int higs_get_lists(higs_ctx* ctx, higs_lists* out)
     int rc = fetch_header(ctx);
     if (rc) return rc;
     const FrameHeader& h = *ctx->hdr_host;
+    // the frame's own list carries dense slots; the caller gets gaussian ids (same order: slots are monotone in the id)
+    if (!h.overflow && h.n_pairs) {
+        if ((rc = launch_export_lists(ctx, h.n_pairs, ctx->last_stream))) return rc;
+        HIGS_CUDA(ctx, cudaStreamSynchronize(ctx->last_stream));
+    }
     out->n_pairs = h.n_pairs; out->n_units = h.n_units; out->n_mt = ctx->last_nm;
     out->mt_count = ctx->mt_count; out->mt_offset = ctx->mt_offset; out->batch_offset = ctx->batch_offset;
-    out->pairs = reinterpret_cast<const uint64_t*>(ctx->pairs); out->unit_active = ctx->unit_active;
+    out->pairs = reinterpret_cast<const uint64_t*>(ctx->pairs_alt); out->unit_active = ctx->unit_active;
     return h.overflow ? HIGS_E_CAPACITY : HIGS_OK;
 }
 
@@ -352,8 +362,13 @@ int higs_get_records(higs_ctx* ctx, higs_records* out)
     if (!ctx || !out) return HIGS_E_ARG;
     int rc = fetch_header(ctx);
     if (rc) return rc;
+    if (!ctx->rec_export && (rc = dev_alloc(ctx, &ctx->rec_export, (size_t)(ctx->max_gaussians > 0 ? ctx->max_gaussians : 1) * 16))) return rc;
+    if (ctx->last_n > 0) {
+        if ((rc = launch_export_records(ctx, ctx->last_n, ctx->last_stream))) return rc;
+        HIGS_CUDA(ctx, cudaStreamSynchronize(ctx->last_stream));
+    }
     out->n = ctx->last_n; out->valid_bits = ctx->valid_bits;
-    out->rec = reinterpret_cast<const float*>(ctx->rec);
+    out->rec = ctx->rec_export;
     return HIGS_OK;
 }
 

@@ -160,8 +160,10 @@ k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, con
 
 #define HIGS_DESC_FALLBACK 0x8000000000000000ull   // see project.cu
 
+// a4: one CTA per partition batch, one warp per 512-id chunk; the chunk's survivors sit densely in `bin`, so the
+// loads are coalesced and every lane has work.  Items are (depth key << 32 | slot).
 __global__ void __launch_bounds__(BIN_THREADS)
-k_fill(const uint32_t* __restrict__ valid_bits, const float4* __restrict__ rec, int64_t N, const FrameParams P,
+k_fill(const uint32_t* __restrict__ chunk_count, const uint4* __restrict__ bin, const float4* __restrict__ rec, const FrameParams P,
        const uint32_t* __restrict__ base, const uint32_t* __restrict__ gbase, const uint32_t* __restrict__ mt_offset,
        unsigned long long* __restrict__ pairs, const FrameHeader* __restrict__ hdr)
 {
@@ -171,27 +173,28 @@ k_fill(const uint32_t* __restrict__ valid_bits, const float4* __restrict__ rec, 
     for (int m = threadIdx.x; m < P.n_m; m += BIN_THREADS)
         s_cursor[m] = mt_offset[m] + gbase[(size_t)g * P.n_m + m] + base[(size_t)b * P.n_m + m];
     __syncthreads();
-    const int64_t i0 = (int64_t)b * HIGS_PART_BATCH;
-    for (int k = 0; k < HIGS_PART_BATCH / BIN_THREADS; ++k) {
-        const int64_t i = i0 + k * BIN_THREADS + threadIdx.x;
-        if (i >= N) break;
-        if (!((valid_bits[i >> 5] >> (i & 31)) & 1u)) continue;
-        const float4 s2 = __ldcs(rec + 4 * i + 2), s3 = __ldcs(rec + 4 * i + 3);   // g, b, key, desc_lo | desc_hi, a, b, c
-        const unsigned long long item = ((unsigned long long)__float_as_uint(s2.z) << 32) | (unsigned long long)(uint32_t)i;
-        const unsigned long long desc = ((unsigned long long)__float_as_uint(s3.x) << 32) | __float_as_uint(s2.w);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const uint32_t cnt = chunk_count[b * (HIGS_PART_BATCH / HIGS_CHUNK) + w];
+    const size_t slot0 = (size_t)b * HIGS_PART_BATCH + (size_t)w * HIGS_CHUNK;
+    for (uint32_t k = lane; k < cnt; k += 32) {
+        const size_t slot = slot0 + k;
+        const uint4 bn = __ldcs(bin + slot);         // key, desc lo, desc hi, id
+        const unsigned long long item = ((unsigned long long)bn.x << 32) | (unsigned long long)(uint32_t)slot;
+        const unsigned long long desc = ((unsigned long long)bn.z << 32) | bn.y;
         if (!(desc & HIGS_DESC_FALLBACK)) {
             const int r0 = (int)(desc & 511u), nr = (int)((desc >> 9) & 3u);
             for (int rr = 0; rr <= nr; ++rr) {
                 const uint32_t f = (uint32_t)(desc >> (11 + 13 * rr)) & 0x1fffu;
                 const int m0 = (int)(f & 511u);
                 if (m0 == 511) continue;
-                const int cell0 = (r0 + rr) * P.n_mx + m0, w = (int)(f >> 9);
-                for (int m = 0; m <= w; ++m) pairs[atomicAdd(&s_cursor[cell0 + m], 1u)] = item;
+                const int cell0 = (r0 + rr) * P.n_mx + m0, wd = (int)(f >> 9);
+                for (int m = 0; m <= wd; ++m) pairs[atomicAdd(&s_cursor[cell0 + m], 1u)] = item;
             }
         } else {                                    // span too large for the descriptor: redo the row scan
-            const float4 s0 = __ldcs(rec + 4 * i), s1 = __ldcs(rec + 4 * i + 1);
+            const float4 s0 = __ldcs(rec + 4 * slot), s1 = __ldcs(rec + 4 * slot + 1), s2 = __ldcs(rec + 4 * slot + 2),
+                         s3 = __ldcs(rec + 4 * slot + 3);
             RowScan rs;
-            rs.init(s0.x, s0.y, s3.y, s3.z, s3.w, s1.y, (float)HIGS_MT_H, P.n_my);
+            rs.init(s0.x, s0.y, s2.z, s2.w, s3.x, s1.y, (float)HIGS_MT_H, P.n_my);
             const float fW = (float)P.W, fH = (float)P.H;
             for (int r = rs.r0; r <= rs.r1; ++r) {
                 int m0, m1;
@@ -200,6 +203,30 @@ k_fill(const uint32_t* __restrict__ valid_bits, const float4* __restrict__ rec, 
             }
         }
     }
+}
+
+// test-facing exports (higs_get_lists / higs_get_records; never part of a frame)
+__global__ void k_export_lists(const unsigned long long* __restrict__ pairs, const uint4* __restrict__ bin, uint32_t n,
+                               unsigned long long* __restrict__ out)
+{
+    const uint32_t p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const unsigned long long it = pairs[p];
+    out[p] = (it & 0xffffffff00000000ull) | (unsigned long long)bin[(uint32_t)it].w;
+}
+
+__global__ void k_export_records(const uint32_t* __restrict__ chunk_count, const float4* __restrict__ rec, const uint4* __restrict__ bin,
+                                 int64_t n_slots, float* __restrict__ out)
+{
+    const int64_t slot = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (slot >= n_slots) return;
+    if ((uint32_t)(slot % HIGS_CHUNK) >= chunk_count[slot / HIGS_CHUNK]) return;
+    const float4 q0 = rec[4 * slot], q1 = rec[4 * slot + 1], q2 = rec[4 * slot + 2], q3 = rec[4 * slot + 3];
+    const uint4 bn = bin[slot];
+    float* o = out + (size_t)bn.w * 16;               // mux, muy, A, B2, C, tau, log2 o, r, g, b, bits(key), desc lo, desc hi, a, b, c
+    o[0] = q0.x; o[1] = q0.y; o[2] = q0.z; o[3] = q0.w; o[4] = q1.x; o[5] = q1.y; o[6] = q1.z; o[7] = q1.w;
+    o[8] = q2.x; o[9] = q2.y; o[10] = __uint_as_float(bn.x); o[11] = __uint_as_float(bn.y); o[12] = __uint_as_float(bn.z);
+    o[13] = q2.z; o[14] = q2.w; o[15] = q3.x;
 }
 
 __global__ void k_zero_lists(uint32_t* mt_count, uint32_t* mt_offset, uint32_t* batch_offset, int n_m)
@@ -231,8 +258,23 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
                                ctx->level_hist, ctx->level_cur, ctx->hdr);
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
-    k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->valid_bits, ctx->rec, N, P, ctx->base, gsum, ctx->mt_offset, ctx->pairs, ctx->hdr);
+    k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->chunk_count, ctx->bin, ctx->rec, P, ctx->base, gsum, ctx->mt_offset, ctx->pairs, ctx->hdr);
     HIGS_LAUNCHED(ctx);
+    return HIGS_OK;
+}
+
+int launch_export_lists(higs_ctx* ctx, uint32_t n_pairs, cudaStream_t st)
+{
+    k_export_lists<<<(n_pairs + 255) / 256, 256, 0, st>>>(ctx->pairs, ctx->bin, n_pairs, ctx->pairs_alt);
+    HIGS_CUDA(ctx, cudaGetLastError());
+    return HIGS_OK;
+}
+
+int launch_export_records(higs_ctx* ctx, int64_t N, cudaStream_t st)
+{
+    const int64_t n_slots = ((N + HIGS_PART_BATCH - 1) / HIGS_PART_BATCH) * HIGS_PART_BATCH;
+    k_export_records<<<(unsigned)((n_slots + 255) / 256), 256, 0, st>>>(ctx->chunk_count, ctx->rec, ctx->bin, n_slots, ctx->rec_export);
+    HIGS_CUDA(ctx, cudaGetLastError());
     return HIGS_OK;
 }
 

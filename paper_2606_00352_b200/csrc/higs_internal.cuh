@@ -9,6 +9,7 @@
 #define HIGS_ALPHA_MAX  0.99f
 #define HIGS_MAX_NM     32768        // macro-tiles per frame the shared-memory histograms are sized for
 #define HIGS_N_TIERS    4            // block-sort tiers, capacities 1024 / 2048 / 4096 / 8192
+#define HIGS_CHUNK      512          // consecutive ids projected by one warp; survivors are stored densely per chunk
 #define HIGS_MERGE_TILE 4096         // output items per merge-path tile (overflow path)
 
 // ---- per-frame device header: every data-dependent size lives here, never on the host ----------
@@ -57,8 +58,12 @@ struct higs_ctx {
     int batch_cap;
     // scratch (device)
     uint32_t* valid_bits;      // [ceil(maxN/32)]
-    float4*   rec;             // [maxN][4]  mux,muy,A,B2 | C,tau,log2o,r | g,b,bits(key),desc_lo | desc_hi,a,b,c  (64 B = two sectors:
-                               //            the rasterizer gathers the first 40 B, fill reads the second sector)
+    float4*   rec;             // [slots][4]  mux,muy,A,B2 | C,tau,log2o,r | g,b,a,b | c,bits(key),id,-   (64 B; the rasterizer gathers the
+                               //             first 40 B).  A slot is the dense position of a surviving gaussian: survivor k of the
+                               //             512-id chunk (batch b, warp w) sits at b*8192 + w*512 + k (monotone in the id)
+    uint4*    bin;             // [slots]     bits(key), span descriptor lo, hi, id   (16 B, read by fill)
+    uint32_t* chunk_count;     // [N_B*16]    survivors per chunk
+    float*    rec_export;      // [maxN][16]  test-facing copy indexed by gaussian id, allocated by the first higs_get_records
     uint16_t* hist;            // [N_B][N_M]
     uint32_t* base;            // [N_B][N_M] write base of (batch, macro-tile) relative to mt_offset[m]
     uint32_t* mt_count;        // [max_nm]

@@ -96,127 +96,112 @@ __device__ __forceinline__ void sh_accumulate(const float* __restrict__ shp, flo
 }
 
 constexpr int PROJ_THREADS = 512;
+constexpr int PROJ_WARPS = PROJ_THREADS / 32;
+constexpr int PROJ_CHUNK = HIGS_PART_BATCH / PROJ_WARPS;   // consecutive ids owned by one warp (512)
+constexpr int PROJ_QCAP = 64;                              // per-warp survivor queue (entries), >= 31 + 32
+constexpr int PROJ_QF = 15;                                // words per queued survivor
 
 // 64-bit macro-tile span descriptor (internal): bit 63 = "not representable, rerun the row scan";
 // bits 0-8 first macro-tile row r0, bits 9-10 rows-1 (<= 4 rows), then 13 bits per row:
 // first column m0 (9 bits, 511 = row not touched) and columns-1 (4 bits, <= 16 columns).
 #define HIGS_DESC_FALLBACK 0x8000000000000000ull
 
-template <int DEG>
-__global__ void __launch_bounds__(PROJ_THREADS, 2)
-k_project(const float* __restrict__ means, const float* __restrict__ scales, const float* __restrict__ quats,
-          const float* __restrict__ opac, const float* __restrict__ sh, int64_t N, const FrameParams P,
-          uint32_t* __restrict__ valid_bits, float4* __restrict__ rec, uint16_t* __restrict__ hist, int pitch,
-          FrameHeader* __restrict__ hdr)
+// what phase A hands to phase B for a surviving gaussian
+struct Survivor { float mux, muy, a, b, c, A, B2, C, tau, zc, o, mx, my, mz; uint32_t local; };
+
+// Phase A: N-PROJ steps 1-10 for gaussian i; false = culled.
+__device__ __forceinline__ bool project_cull(const float* __restrict__ means, const float* __restrict__ scales,
+                                             const float* __restrict__ quats, const float* __restrict__ opac,
+                                             int64_t i, const FrameParams& P, Survivor& s)
 {
-    extern __shared__ uint32_t s_hist[];
-    __shared__ uint32_t s_nvis;
-    for (int m = threadIdx.x; m < P.n_m; m += PROJ_THREADS) s_hist[m] = 0;
-    if (threadIdx.x == 0) s_nvis = 0;
-    __syncthreads();
-    const int64_t i0 = (int64_t)blockIdx.x * HIGS_PART_BATCH;
-    uint32_t nvis = 0;
-    for (int it = 0; it < HIGS_PART_BATCH / PROJ_THREADS; ++it) {
-    if (i0 + (int64_t)it * PROJ_THREADS >= N) break;                 // block-uniform
-    const int64_t i = i0 + (int64_t)it * PROJ_THREADS + threadIdx.x;
-    bool ok = i < N;
-    float mx = 0, my = 0, mz = 0;
-    float mux = 0, muy = 0, a = 0, b = 0, c = 0, A = 0, B2 = 0, C = 0, tau = 0, zc = 0, o = 0;
-    if (ok) {
-        mx = __ldcs(means + 3 * i); my = __ldcs(means + 3 * i + 1); mz = __ldcs(means + 3 * i + 2);
-        const float* V = P.V;
-        // 1. camera transform
-        float xc = __fmaf_rn(V[2], mz, __fmaf_rn(V[1], my, __fmaf_rn(V[0], mx, V[3])));
-        float yc = __fmaf_rn(V[6], mz, __fmaf_rn(V[5], my, __fmaf_rn(V[4], mx, V[7])));
-        zc = __fmaf_rn(V[10], mz, __fmaf_rn(V[9], my, __fmaf_rn(V[8], mx, V[11])));
-        ok = (zc > P.near_z) && (zc <= 3.402823466e+38f);
-        if (ok) {
-            // 2. perspective
-            float rz = __frcp_rn(zc);
-            float xz = __fmul_rn(xc, rz), yz = __fmul_rn(yc, rz);
-            mux = __fmaf_rn(P.fx, xz, P.cx); muy = __fmaf_rn(P.fy, yz, P.cy);
-            // 3. clamp inside the Jacobian only
-            float limx = __fdiv_rn(__fmul_rn(0.65f, (float)P.W), P.fx);
-            float limy = __fdiv_rn(__fmul_rn(0.65f, (float)P.H), P.fy);
-            float txz = fminf(limx, fmaxf(-limx, xz));
-            float tyz = fminf(limy, fmaxf(-limy, yz));
-            // 4. rotation from the normalised quaternion
-            float4 q4 = __ldcs(reinterpret_cast<const float4*>(quats) + i);
-            float qw = q4.x, qx = q4.y, qy = q4.z, qz = q4.w;
-            float n2 = __fmaf_rn(qz, qz, __fmaf_rn(qy, qy, __fmaf_rn(qx, qx, __fmul_rn(qw, qw))));
-            ok = finite_pos(n2);
-            if (ok) {
-                float inv = __frcp_rn(__fsqrt_rn(n2));
-                qw = __fmul_rn(qw, inv); qx = __fmul_rn(qx, inv); qy = __fmul_rn(qy, inv); qz = __fmul_rn(qz, inv);
-                float Q00 = __fmaf_rn(-2.0f, __fmaf_rn(qy, qy, __fmul_rn(qz, qz)), 1.0f);
-                float Q01 = __fmul_rn(2.0f, __fmaf_rn(qx, qy, -__fmul_rn(qw, qz)));
-                float Q02 = __fmul_rn(2.0f, __fmaf_rn(qx, qz, __fmul_rn(qw, qy)));
-                float Q10 = __fmul_rn(2.0f, __fmaf_rn(qx, qy, __fmul_rn(qw, qz)));
-                float Q11 = __fmaf_rn(-2.0f, __fmaf_rn(qx, qx, __fmul_rn(qz, qz)), 1.0f);
-                float Q12 = __fmul_rn(2.0f, __fmaf_rn(qy, qz, -__fmul_rn(qw, qx)));
-                float Q20 = __fmul_rn(2.0f, __fmaf_rn(qx, qz, -__fmul_rn(qw, qy)));
-                float Q21 = __fmul_rn(2.0f, __fmaf_rn(qy, qz, __fmul_rn(qw, qx)));
-                float Q22 = __fmaf_rn(-2.0f, __fmaf_rn(qx, qx, __fmul_rn(qy, qy)), 1.0f);
-                // 5. M = Q diag(s)
-                float s0 = __ldcs(scales + 3 * i), s1 = __ldcs(scales + 3 * i + 1), s2 = __ldcs(scales + 3 * i + 2);
-                float M00 = __fmul_rn(Q00, s0), M01 = __fmul_rn(Q01, s1), M02 = __fmul_rn(Q02, s2);
-                float M10 = __fmul_rn(Q10, s0), M11 = __fmul_rn(Q11, s1), M12 = __fmul_rn(Q12, s2);
-                float M20 = __fmul_rn(Q20, s0), M21 = __fmul_rn(Q21, s1), M22 = __fmul_rn(Q22, s2);
-                // 6. J, G = J R_view, Tm = G M
-                float J00 = __fmul_rn(P.fx, rz), J02 = __fmul_rn(-__fmul_rn(P.fx, txz), rz);
-                float J11 = __fmul_rn(P.fy, rz), J12 = __fmul_rn(-__fmul_rn(P.fy, tyz), rz);
-                float G00 = __fmaf_rn(J02, V[8], __fmul_rn(J00, V[0]));
-                float G01 = __fmaf_rn(J02, V[9], __fmul_rn(J00, V[1]));
-                float G02 = __fmaf_rn(J02, V[10], __fmul_rn(J00, V[2]));
-                float G10 = __fmaf_rn(J12, V[8], __fmul_rn(J11, V[4]));
-                float G11 = __fmaf_rn(J12, V[9], __fmul_rn(J11, V[5]));
-                float G12 = __fmaf_rn(J12, V[10], __fmul_rn(J11, V[6]));
-                float T00 = __fmaf_rn(G02, M20, __fmaf_rn(G01, M10, __fmul_rn(G00, M00)));
-                float T01 = __fmaf_rn(G02, M21, __fmaf_rn(G01, M11, __fmul_rn(G00, M01)));
-                float T02 = __fmaf_rn(G02, M22, __fmaf_rn(G01, M12, __fmul_rn(G00, M02)));
-                float T10 = __fmaf_rn(G12, M20, __fmaf_rn(G11, M10, __fmul_rn(G10, M00)));
-                float T11 = __fmaf_rn(G12, M21, __fmaf_rn(G11, M11, __fmul_rn(G10, M01)));
-                float T12 = __fmaf_rn(G12, M22, __fmaf_rn(G11, M12, __fmul_rn(G10, M02)));
-                // 7. 2D covariance + 0.3 I
-                a = __fadd_rn(__fmaf_rn(T02, T02, __fmaf_rn(T01, T01, __fmul_rn(T00, T00))), 0.3f);
-                b = __fmaf_rn(T02, T12, __fmaf_rn(T01, T11, __fmul_rn(T00, T10)));
-                c = __fadd_rn(__fmaf_rn(T12, T12, __fmaf_rn(T11, T11, __fmul_rn(T10, T10))), 0.3f);
-                // 8. conic
-                float det = __fmaf_rn(a, c, -__fmul_rn(b, b));
-                ok = finite_pos(det);
-                if (ok) {
-                    float rd = __frcp_rn(det);
-                    A = __fmul_rn(c, rd); B2 = -__fmul_rn(__fadd_rn(b, b), rd); C = __fmul_rn(a, rd);
-                    ok = (A <= 3.402823466e+38f) && (C <= 3.402823466e+38f) && (fabsf(B2) <= 3.402823466e+38f);
-                }
-                if (ok) {
-                    // 9. opacity threshold: alpha >= 1/255 <=> q <= tau = 2 ln(255 o)
-                    o = __ldcs(opac + i);
-                    float x255 = __fmul_rn(255.0f, o);
-                    ok = (x255 > 1.0f) && (x255 <= 3.402823466e+38f);
-                    if (ok) {
-                        tau = __fmul_rn(2.0f, ln_spec(x255));
-                        ok = tau > 0.0f;
-                    }
-                }
-                if (ok) {
-                    // 10. off-screen cull on the threshold ellipse's bounding box
-                    float hx = __fsqrt_rn(__fmul_rn(tau, a)), hy = __fsqrt_rn(__fmul_rn(tau, c));
-                    ok = (__fadd_rn(mux, hx) > 0.0f) && (__fsub_rn(mux, hx) < (float)P.W) &&
-                         (__fadd_rn(muy, hy) > 0.0f) && (__fsub_rn(muy, hy) < (float)P.H);
-                }
-            }
-        }
-    }
-    const uint32_t vmask = __ballot_sync(0xffffffffu, ok);
-    if ((threadIdx.x & 31) == 0 && (i < N)) valid_bits[i >> 5] = vmask;   // warp bases are multiples of 32
-    if (!ok) continue;
-    ++nvis;
-    // a2: macro-tile row scan (N-SCAN, pinned) -> private histogram + span descriptor
+    const float mx = __ldcs(means + 3 * i), my = __ldcs(means + 3 * i + 1), mz = __ldcs(means + 3 * i + 2);
+    const float* V = P.V;
+    // 1. camera transform
+    const float xc = __fmaf_rn(V[2], mz, __fmaf_rn(V[1], my, __fmaf_rn(V[0], mx, V[3])));
+    const float yc = __fmaf_rn(V[6], mz, __fmaf_rn(V[5], my, __fmaf_rn(V[4], mx, V[7])));
+    const float zc = __fmaf_rn(V[10], mz, __fmaf_rn(V[9], my, __fmaf_rn(V[8], mx, V[11])));
+    if (!((zc > P.near_z) && (zc <= 3.402823466e+38f))) return false;
+    // 2. perspective
+    const float rz = __frcp_rn(zc);
+    const float xz = __fmul_rn(xc, rz), yz = __fmul_rn(yc, rz);
+    const float mux = __fmaf_rn(P.fx, xz, P.cx), muy = __fmaf_rn(P.fy, yz, P.cy);
+    // 3. clamp inside the Jacobian only
+    const float limx = __fdiv_rn(__fmul_rn(0.65f, (float)P.W), P.fx);
+    const float limy = __fdiv_rn(__fmul_rn(0.65f, (float)P.H), P.fy);
+    const float txz = fminf(limx, fmaxf(-limx, xz));
+    const float tyz = fminf(limy, fmaxf(-limy, yz));
+    // 4. rotation from the normalised quaternion
+    const float4 q4 = __ldcs(reinterpret_cast<const float4*>(quats) + i);
+    float qw = q4.x, qx = q4.y, qy = q4.z, qz = q4.w;
+    const float n2 = __fmaf_rn(qz, qz, __fmaf_rn(qy, qy, __fmaf_rn(qx, qx, __fmul_rn(qw, qw))));
+    if (!finite_pos(n2)) return false;
+    const float inv = __frcp_rn(__fsqrt_rn(n2));
+    qw = __fmul_rn(qw, inv); qx = __fmul_rn(qx, inv); qy = __fmul_rn(qy, inv); qz = __fmul_rn(qz, inv);
+    const float Q00 = __fmaf_rn(-2.0f, __fmaf_rn(qy, qy, __fmul_rn(qz, qz)), 1.0f);
+    const float Q01 = __fmul_rn(2.0f, __fmaf_rn(qx, qy, -__fmul_rn(qw, qz)));
+    const float Q02 = __fmul_rn(2.0f, __fmaf_rn(qx, qz, __fmul_rn(qw, qy)));
+    const float Q10 = __fmul_rn(2.0f, __fmaf_rn(qx, qy, __fmul_rn(qw, qz)));
+    const float Q11 = __fmaf_rn(-2.0f, __fmaf_rn(qx, qx, __fmul_rn(qz, qz)), 1.0f);
+    const float Q12 = __fmul_rn(2.0f, __fmaf_rn(qy, qz, -__fmul_rn(qw, qx)));
+    const float Q20 = __fmul_rn(2.0f, __fmaf_rn(qx, qz, -__fmul_rn(qw, qy)));
+    const float Q21 = __fmul_rn(2.0f, __fmaf_rn(qy, qz, __fmul_rn(qw, qx)));
+    const float Q22 = __fmaf_rn(-2.0f, __fmaf_rn(qx, qx, __fmul_rn(qy, qy)), 1.0f);
+    // 5. M = Q diag(s)
+    const float s0 = __ldcs(scales + 3 * i), s1 = __ldcs(scales + 3 * i + 1), s2 = __ldcs(scales + 3 * i + 2);
+    const float M00 = __fmul_rn(Q00, s0), M01 = __fmul_rn(Q01, s1), M02 = __fmul_rn(Q02, s2);
+    const float M10 = __fmul_rn(Q10, s0), M11 = __fmul_rn(Q11, s1), M12 = __fmul_rn(Q12, s2);
+    const float M20 = __fmul_rn(Q20, s0), M21 = __fmul_rn(Q21, s1), M22 = __fmul_rn(Q22, s2);
+    // 6. J, G = J R_view, Tm = G M
+    const float J00 = __fmul_rn(P.fx, rz), J02 = __fmul_rn(-__fmul_rn(P.fx, txz), rz);
+    const float J11 = __fmul_rn(P.fy, rz), J12 = __fmul_rn(-__fmul_rn(P.fy, tyz), rz);
+    const float G00 = __fmaf_rn(J02, V[8], __fmul_rn(J00, V[0]));
+    const float G01 = __fmaf_rn(J02, V[9], __fmul_rn(J00, V[1]));
+    const float G02 = __fmaf_rn(J02, V[10], __fmul_rn(J00, V[2]));
+    const float G10 = __fmaf_rn(J12, V[8], __fmul_rn(J11, V[4]));
+    const float G11 = __fmaf_rn(J12, V[9], __fmul_rn(J11, V[5]));
+    const float G12 = __fmaf_rn(J12, V[10], __fmul_rn(J11, V[6]));
+    const float T00 = __fmaf_rn(G02, M20, __fmaf_rn(G01, M10, __fmul_rn(G00, M00)));
+    const float T01 = __fmaf_rn(G02, M21, __fmaf_rn(G01, M11, __fmul_rn(G00, M01)));
+    const float T02 = __fmaf_rn(G02, M22, __fmaf_rn(G01, M12, __fmul_rn(G00, M02)));
+    const float T10 = __fmaf_rn(G12, M20, __fmaf_rn(G11, M10, __fmul_rn(G10, M00)));
+    const float T11 = __fmaf_rn(G12, M21, __fmaf_rn(G11, M11, __fmul_rn(G10, M01)));
+    const float T12 = __fmaf_rn(G12, M22, __fmaf_rn(G11, M12, __fmul_rn(G10, M02)));
+    // 7. 2D covariance + 0.3 I
+    const float a = __fadd_rn(__fmaf_rn(T02, T02, __fmaf_rn(T01, T01, __fmul_rn(T00, T00))), 0.3f);
+    const float b = __fmaf_rn(T02, T12, __fmaf_rn(T01, T11, __fmul_rn(T00, T10)));
+    const float c = __fadd_rn(__fmaf_rn(T12, T12, __fmaf_rn(T11, T11, __fmul_rn(T10, T10))), 0.3f);
+    // 8. conic
+    const float det = __fmaf_rn(a, c, -__fmul_rn(b, b));
+    if (!finite_pos(det)) return false;
+    const float rd = __frcp_rn(det);
+    const float A = __fmul_rn(c, rd), B2 = -__fmul_rn(__fadd_rn(b, b), rd), C = __fmul_rn(a, rd);
+    if (!((A <= 3.402823466e+38f) && (C <= 3.402823466e+38f) && (fabsf(B2) <= 3.402823466e+38f))) return false;
+    // 9. opacity threshold: alpha >= 1/255 <=> q <= tau = 2 ln(255 o)
+    const float o = __ldcs(opac + i);
+    const float x255 = __fmul_rn(255.0f, o);
+    if (!((x255 > 1.0f) && (x255 <= 3.402823466e+38f))) return false;
+    const float tau = __fmul_rn(2.0f, ln_spec(x255));
+    if (!(tau > 0.0f)) return false;
+    // 10. off-screen cull on the threshold ellipse's bounding box
+    const float hx = __fsqrt_rn(__fmul_rn(tau, a)), hy = __fsqrt_rn(__fmul_rn(tau, c));
+    if (!((__fadd_rn(mux, hx) > 0.0f) && (__fsub_rn(mux, hx) < (float)P.W) &&
+          (__fadd_rn(muy, hy) > 0.0f) && (__fsub_rn(muy, hy) < (float)P.H))) return false;
+    s.mux = mux; s.muy = muy; s.a = a; s.b = b; s.c = c; s.A = A; s.B2 = B2; s.C = C; s.tau = tau; s.zc = zc; s.o = o;
+    s.mx = mx; s.my = my; s.mz = mz;
+    return true;
+}
+
+// Phase B for one survivor: a2 macro-tile row scan (N-SCAN, pinned) -> private histogram + span descriptor,
+// SH colour, and the two records at dense slot `slot`.
+template <int DEG>
+__device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size_t slot, const float* __restrict__ sh,
+                                              const FrameParams& P, uint32_t* s_hist, float4* __restrict__ rec,
+                                              uint4* __restrict__ bin)
+{
     unsigned long long desc = 0;
     {
         RowScan rs;
-        rs.init(mux, muy, a, b, c, tau, (float)HIGS_MT_H, P.n_my);
+        rs.init(s.mux, s.muy, s.a, s.b, s.c, s.tau, (float)HIGS_MT_H, P.n_my);
         const float fW = (float)P.W, fH = (float)P.H;
         bool fits = (rs.r1 - rs.r0) <= 3 && P.n_mx <= 511 && rs.r0 <= 511;
         desc = (unsigned long long)(uint32_t)rs.r0 | ((unsigned long long)(uint32_t)((rs.r1 - rs.r0) & 3) << 9);
@@ -233,19 +218,83 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
         if (!fits) desc = HIGS_DESC_FALLBACK;
     }
     // 11./12. depth key, colour
-    float dx = mx - P.cam[0], dy = my - P.cam[1], dz = mz - P.cam[2];
-    float len2 = dx * dx + dy * dy + dz * dz;
-    float rl = len2 > 0.0f ? rsqrtf(len2) : 0.0f;
+    const float dx = s.mx - P.cam[0], dy = s.my - P.cam[1], dz = s.mz - P.cam[2];
+    const float len2 = dx * dx + dy * dy + dz * dz;
+    const float rl = len2 > 0.0f ? rsqrtf(len2) : 0.0f;
     float r, g, bl;
     sh_accumulate<DEG>(sh + i * (int64_t)((DEG + 1) * (DEG + 1) * 3), dx * rl, dy * rl, dz * rl, r, g, bl);
-    float4* rp = rec + 4 * i;
-    rp[0] = make_float4(mux, muy, A, B2);
-    rp[1] = make_float4(C, tau, log2f(o), r);
-    rp[2] = make_float4(g, bl, __uint_as_float(__float_as_uint(zc)), __uint_as_float((uint32_t)desc));
-    rp[3] = make_float4(__uint_as_float((uint32_t)(desc >> 32)), a, b, c);
-    }   // partition-batch loop
-    nvis = __reduce_add_sync(0xffffffffu, nvis);
-    if ((threadIdx.x & 31) == 0 && nvis) atomicAdd(&s_nvis, nvis);
+    const uint32_t key = __float_as_uint(s.zc);
+    float4* rp = rec + 4 * slot;
+    rp[0] = make_float4(s.mux, s.muy, s.A, s.B2);
+    rp[1] = make_float4(s.C, s.tau, log2f(s.o), r);
+    rp[2] = make_float4(g, bl, s.a, s.b);
+    rp[3] = make_float4(s.c, __uint_as_float(key), __uint_as_float((uint32_t)i), 0.0f);
+    bin[slot] = make_uint4(key, (uint32_t)desc, (uint32_t)(desc >> 32), (uint32_t)i);
+}
+
+// One CTA per partition batch (8192 ids), one warp per chunk of 512 consecutive ids.  A warp runs phase A on 32
+// gaussians at a time and queues the survivors (about 4 in 10 at paper scale) in shared memory; whenever 32 are
+// queued it runs phase B on them with every lane busy.  Survivor k of chunk (b, w) gets dense slot
+// b*8192 + w*512 + k: slots are monotone in the gaussian id, so (key, slot) order = (key, id) order (Q7).
+template <int DEG>
+__global__ void __launch_bounds__(PROJ_THREADS, 2)
+k_project(const float* __restrict__ means, const float* __restrict__ scales, const float* __restrict__ quats,
+          const float* __restrict__ opac, const float* __restrict__ sh, int64_t N, const FrameParams P,
+          uint32_t* __restrict__ valid_bits, float4* __restrict__ rec, uint4* __restrict__ bin,
+          uint32_t* __restrict__ chunk_count, uint16_t* __restrict__ hist, int pitch, FrameHeader* __restrict__ hdr)
+{
+    extern __shared__ uint32_t s_dyn[];
+    __shared__ uint32_t s_nvis;
+    uint32_t* s_hist = s_dyn;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    float* q = reinterpret_cast<float*>(s_dyn + ((P.n_m + 3) & ~3)) + w * (PROJ_QF * PROJ_QCAP);
+    for (int m = threadIdx.x; m < P.n_m; m += PROJ_THREADS) s_hist[m] = 0;
+    if (threadIdx.x == 0) s_nvis = 0;
+    __syncthreads();
+    const int64_t c0 = (int64_t)blockIdx.x * HIGS_PART_BATCH + (int64_t)w * PROJ_CHUNK;
+    const size_t slot0 = (size_t)c0;
+    const uint32_t lt = (1u << lane) - 1u;
+    uint32_t head = 0, tail = 0;
+
+    auto drain = [&](uint32_t n_live) {                              // phase B on queue entries head .. head+n_live-1
+        if ((uint32_t)lane < n_live) {
+            const int e = (int)((head + lane) & (PROJ_QCAP - 1));
+            Survivor s;
+            s.mux = q[0 * PROJ_QCAP + e]; s.muy = q[1 * PROJ_QCAP + e]; s.a = q[2 * PROJ_QCAP + e]; s.b = q[3 * PROJ_QCAP + e];
+            s.c = q[4 * PROJ_QCAP + e]; s.A = q[5 * PROJ_QCAP + e]; s.B2 = q[6 * PROJ_QCAP + e]; s.C = q[7 * PROJ_QCAP + e];
+            s.tau = q[8 * PROJ_QCAP + e]; s.zc = q[9 * PROJ_QCAP + e]; s.o = q[10 * PROJ_QCAP + e];
+            s.mx = q[11 * PROJ_QCAP + e]; s.my = q[12 * PROJ_QCAP + e]; s.mz = q[13 * PROJ_QCAP + e];
+            s.local = __float_as_uint(q[14 * PROJ_QCAP + e]);
+            emit_survivor<DEG>(s, c0 + s.local, slot0 + head + lane, sh, P, s_hist, rec, bin);
+        }
+        head += n_live;
+        __syncwarp();
+    };
+
+    for (int it = 0; it < PROJ_CHUNK / 32; ++it) {
+        const int64_t i = c0 + it * 32 + lane;
+        if (c0 + it * 32 >= N) break;                                // warp-uniform
+        Survivor s;
+        const bool ok = (i < N) && project_cull(means, scales, quats, opac, i, P, s);
+        const uint32_t vmask = __ballot_sync(0xffffffffu, ok);
+        if (lane == 0) valid_bits[i >> 5] = vmask;                   // chunk bases are multiples of 32
+        if (ok) {
+            const int e = (int)((tail + __popc(vmask & lt)) & (PROJ_QCAP - 1));
+            q[0 * PROJ_QCAP + e] = s.mux; q[1 * PROJ_QCAP + e] = s.muy; q[2 * PROJ_QCAP + e] = s.a; q[3 * PROJ_QCAP + e] = s.b;
+            q[4 * PROJ_QCAP + e] = s.c; q[5 * PROJ_QCAP + e] = s.A; q[6 * PROJ_QCAP + e] = s.B2; q[7 * PROJ_QCAP + e] = s.C;
+            q[8 * PROJ_QCAP + e] = s.tau; q[9 * PROJ_QCAP + e] = s.zc; q[10 * PROJ_QCAP + e] = s.o;
+            q[11 * PROJ_QCAP + e] = s.mx; q[12 * PROJ_QCAP + e] = s.my; q[13 * PROJ_QCAP + e] = s.mz;
+            q[14 * PROJ_QCAP + e] = __uint_as_float((uint32_t)(it * 32 + lane));
+        }
+        tail += __popc(vmask);
+        __syncwarp();
+        if (tail - head >= 32u) drain(32u);
+    }
+    if (tail > head) drain(tail - head);
+    if (lane == 0) {
+        chunk_count[blockIdx.x * PROJ_WARPS + w] = tail;
+        if (tail) atomicAdd(&s_nvis, tail);
+    }
     __syncthreads();
     uint32_t* row = reinterpret_cast<uint32_t*>(hist + (size_t)blockIdx.x * pitch);   // pitch is even
     for (int m2 = threadIdx.x; m2 < pitch / 2; m2 += PROJ_THREADS) {
@@ -258,15 +307,20 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
 
 } // namespace
 
+static size_t project_smem_bytes(int n_m)
+{
+    return sizeof(uint32_t) * (size_t)((n_m + 3) & ~3) + sizeof(float) * (size_t)PROJ_WARPS * PROJ_QF * PROJ_QCAP;
+}
+
 int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, const float* scales, const float* quats,
                    const float* opac, const float* sh, int64_t N, cudaStream_t st)
 {
     if (N <= 0) return HIGS_OK;
     const unsigned grid = (unsigned)((N + HIGS_PART_BATCH - 1) / HIGS_PART_BATCH);
-    const size_t smem = sizeof(uint32_t) * (size_t)P.n_m;
+    const size_t smem = project_smem_bytes(P.n_m);
     const int pitch = (P.n_m + 1) & ~1;
 #define HIGS_PROJ(D) k_project<D><<<grid, PROJ_THREADS, smem, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
-                                                                   ctx->hist, pitch, ctx->hdr)
+                                                                   ctx->bin, ctx->chunk_count, ctx->hist, pitch, ctx->hdr)
     switch (P.degree) {
         case 0: HIGS_PROJ(0); break;
         case 1: HIGS_PROJ(1); break;
@@ -280,12 +334,10 @@ int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, cons
 
 int higs_project_smem_setup(higs_ctx* ctx)
 {
-    const int bytes = (int)(sizeof(uint32_t) * (size_t)ctx->max_nm);
-    if (bytes > 48 * 1024) {
-        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-        HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    }
+    const int bytes = (int)project_smem_bytes(ctx->max_nm);
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     return HIGS_OK;
 }
