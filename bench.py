@@ -88,6 +88,9 @@ class ClockSampler:
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thr = threading.Thread(target=self._pump, daemon=True)
             self.thr.start()
+            t_end = time.time() + 10.0                  # nvidia-smi needs a second or two before its first row
+            while not self.rows and time.time() < t_end and self.proc.poll() is None:
+                time.sleep(0.05)
         except OSError:
             self.proc = None
 
@@ -108,7 +111,10 @@ class ClockSampler:
 
     def summary(self, t0: float, t1: float) -> dict:
         sm, mx, reasons = [], [], set()
-        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.06] or [r for _, r in self.rows[-3:]]
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.06]
+        if not rows and self.rows:                      # timed region shorter than a sampling period: nearest samples
+            mid = 0.5 * (t0 + t1)
+            rows = [r for _, r in sorted(self.rows, key=lambda tr: abs(tr[0] - mid))[:3]]
         for r in rows:
             f = [x.strip() for x in r.split(",")]
             if len(f) < 7:
@@ -223,7 +229,6 @@ def run_higs(args) -> int:
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-        time.sleep(0.3)
     hg.higs_set_flags(ctx, 0)
     for i in range(args.warmup):
         frame(i)

@@ -109,12 +109,26 @@ constexpr int PROJ_QF = 15;                                // words per queued s
 // what phase A hands to phase B for a surviving gaussian
 struct Survivor { float mux, muy, a, b, c, A, B2, C, tau, zc, o, mx, my, mz; uint32_t local; };
 
-// Phase A: N-PROJ steps 1-10 for gaussian i; false = culled.
-__device__ __forceinline__ bool project_cull(const float* __restrict__ means, const float* __restrict__ scales,
-                                             const float* __restrict__ quats, const float* __restrict__ opac,
-                                             int64_t i, const FrameParams& P, Survivor& s)
+// The 44 input bytes of one gaussian.  All eleven words are requested up front, one iteration ahead of their use
+// (register double buffer in k_project), so a warp pays one exposed DRAM round trip per 32 gaussians at most
+// instead of four dependent ones (means -> quats -> scales -> opacity).
+struct RawIn { float mx, my, mz, s0, s1, s2, o; float4 q; };
+
+__device__ __forceinline__ RawIn load_raw(const float* __restrict__ means, const float* __restrict__ scales,
+                                          const float* __restrict__ quats, const float* __restrict__ opac, int64_t i)
 {
-    const float mx = __ldcs(means + 3 * i), my = __ldcs(means + 3 * i + 1), mz = __ldcs(means + 3 * i + 2);
+    RawIn r;
+    r.mx = __ldcs(means + 3 * i); r.my = __ldcs(means + 3 * i + 1); r.mz = __ldcs(means + 3 * i + 2);
+    r.q = __ldcs(reinterpret_cast<const float4*>(quats) + i);
+    r.s0 = __ldcs(scales + 3 * i); r.s1 = __ldcs(scales + 3 * i + 1); r.s2 = __ldcs(scales + 3 * i + 2);
+    r.o = __ldcs(opac + i);
+    return r;
+}
+
+// Phase A: N-PROJ steps 1-10 for one gaussian; false = culled.
+__device__ __forceinline__ bool project_cull(const RawIn& in, const FrameParams& P, Survivor& s)
+{
+    const float mx = in.mx, my = in.my, mz = in.mz;
     const float* V = P.V;
     // 1. camera transform
     const float xc = __fmaf_rn(V[2], mz, __fmaf_rn(V[1], my, __fmaf_rn(V[0], mx, V[3])));
@@ -131,7 +145,7 @@ __device__ __forceinline__ bool project_cull(const float* __restrict__ means, co
     const float txz = fminf(limx, fmaxf(-limx, xz));
     const float tyz = fminf(limy, fmaxf(-limy, yz));
     // 4. rotation from the normalised quaternion
-    const float4 q4 = __ldcs(reinterpret_cast<const float4*>(quats) + i);
+    const float4 q4 = in.q;
     float qw = q4.x, qx = q4.y, qy = q4.z, qz = q4.w;
     const float n2 = __fmaf_rn(qz, qz, __fmaf_rn(qy, qy, __fmaf_rn(qx, qx, __fmul_rn(qw, qw))));
     if (!finite_pos(n2)) return false;
@@ -147,7 +161,7 @@ __device__ __forceinline__ bool project_cull(const float* __restrict__ means, co
     const float Q21 = __fmul_rn(2.0f, __fmaf_rn(qy, qz, __fmul_rn(qw, qx)));
     const float Q22 = __fmaf_rn(-2.0f, __fmaf_rn(qx, qx, __fmul_rn(qy, qy)), 1.0f);
     // 5. M = Q diag(s)
-    const float s0 = __ldcs(scales + 3 * i), s1 = __ldcs(scales + 3 * i + 1), s2 = __ldcs(scales + 3 * i + 2);
+    const float s0 = in.s0, s1 = in.s1, s2 = in.s2;
     const float M00 = __fmul_rn(Q00, s0), M01 = __fmul_rn(Q01, s1), M02 = __fmul_rn(Q02, s2);
     const float M10 = __fmul_rn(Q10, s0), M11 = __fmul_rn(Q11, s1), M12 = __fmul_rn(Q12, s2);
     const float M20 = __fmul_rn(Q20, s0), M21 = __fmul_rn(Q21, s1), M22 = __fmul_rn(Q22, s2);
@@ -177,7 +191,7 @@ __device__ __forceinline__ bool project_cull(const float* __restrict__ means, co
     const float A = __fmul_rn(c, rd), B2 = -__fmul_rn(__fadd_rn(b, b), rd), C = __fmul_rn(a, rd);
     if (!((A <= 3.402823466e+38f) && (C <= 3.402823466e+38f) && (fabsf(B2) <= 3.402823466e+38f))) return false;
     // 9. opacity threshold: alpha >= 1/255 <=> q <= tau = 2 ln(255 o)
-    const float o = __ldcs(opac + i);
+    const float o = in.o;
     const float x255 = __fmul_rn(255.0f, o);
     if (!((x255 > 1.0f) && (x255 <= 3.402823466e+38f))) return false;
     const float tau = __fmul_rn(2.0f, ln_spec(x255));
@@ -271,11 +285,15 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
         __syncwarp();
     };
 
+    RawIn nxt = {};
+    if (c0 + lane < N) nxt = load_raw(means, scales, quats, opac, c0 + lane);
     for (int it = 0; it < PROJ_CHUNK / 32; ++it) {
         const int64_t i = c0 + it * 32 + lane;
         if (c0 + it * 32 >= N) break;                                // warp-uniform
+        const RawIn cur = nxt;
+        if (it + 1 < PROJ_CHUNK / 32 && i + 32 < N) nxt = load_raw(means, scales, quats, opac, i + 32);
         Survivor s;
-        const bool ok = (i < N) && project_cull(means, scales, quats, opac, i, P, s);
+        const bool ok = (i < N) && project_cull(cur, P, s);
         const uint32_t vmask = __ballot_sync(0xffffffffu, ok);
         if (lane == 0) valid_bits[i >> 5] = vmask;                   // chunk bases are multiples of 32
         if (ok) {
