@@ -173,25 +173,33 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(HIGS_E_CUDA);
     ctx->n_sm = prop.multiProcessorCount;
     const int64_t n = max_gaussians > 0 ? max_gaussians : 1;
-    ctx->n_part_batches_max = (int)((n + HIGS_PART_BATCH - 1) / HIGS_PART_BATCH);
-    const int n_groups_max = (ctx->n_part_batches_max + 31) / 32;
-    const size_t pitch = ((size_t)nm + 1) & ~(size_t)1;
+    ctx->n_chunks_max = (n + HIGS_CHUNK - 1) / HIGS_CHUNK;
+    if ((rc = higs_project_smem_setup(ctx))) return fail(rc);       // also fixes n_part_max = n_sm x resident CTAs
+    const int n_groups_max = (ctx->n_part_max + 31) / 32;
     if ((rc = dev_alloc(ctx, &ctx->valid_bits, (size_t)(n + 31) / 32 + 1))) return fail(rc);
-    const size_t n_slots = (size_t)ctx->n_part_batches_max * HIGS_PART_BATCH;
+    const size_t n_slots = (size_t)ctx->n_chunks_max * HIGS_CHUNK;
     if ((rc = dev_alloc(ctx, &ctx->rec, n_slots * 4))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->bin, n_slots))) return fail(rc);
-    if ((rc = dev_alloc(ctx, &ctx->chunk_count, (size_t)ctx->n_part_batches_max * (HIGS_PART_BATCH / HIGS_CHUNK)))) return fail(rc);
-    if ((rc = dev_alloc(ctx, &ctx->hist, (size_t)ctx->n_part_batches_max * pitch))) return fail(rc);
-    if ((rc = dev_alloc(ctx, &ctx->base, (size_t)(ctx->n_part_batches_max + n_groups_max) * nm))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->chunk_count, (size_t)ctx->n_chunks_max))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->part_list, (size_t)ctx->n_chunks_max))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->part_desc, (size_t)ctx->n_part_max))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->hist, (size_t)ctx->n_part_max * nm))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->base, (size_t)(ctx->n_part_max + n_groups_max) * nm))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->mt_count, (size_t)nm + 1))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->mt_offset, (size_t)nm + 1))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->batch_offset, (size_t)nm + 1))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->pairs, (size_t)max_pairs))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->pairs_alt, (size_t)max_pairs))) return fail(rc);
-    ctx->max_jobs = nm + max_pairs / HIGS_SORT_BLOCK + 2;
     ctx->max_over = max_pairs / HIGS_SORT_BLOCK + 1;
-    if ((rc = dev_alloc(ctx, &ctx->sort_jobs, (size_t)ctx->max_jobs * HIGS_N_TIERS))) return fail(rc);
+    ctx->max_buckets = max_pairs / HIGS_BUCKET_TARGET + ctx->max_over + 1;
+    ctx->max_jobs = nm + ctx->max_buckets + max_pairs / HIGS_SORT_BLOCK + 2;
+    if ((rc = dev_alloc(ctx, &ctx->sort_jobs, (size_t)ctx->max_jobs * HIGS_N_TIERS * 2))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->over_segs, (size_t)ctx->max_over))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->split_segs, (size_t)ctx->max_over))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->splitters, (size_t)ctx->max_buckets))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->bucket_count, (size_t)ctx->max_buckets))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->bucket_cursor, (size_t)ctx->max_buckets))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->bucket_seg, (size_t)ctx->max_buckets))) return fail(rc);
     if ((rc = alloc_unit_buffers(ctx))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->hdr, 1))) return fail(rc);
     if (cudaMallocHost((void**)&ctx->hdr_host, sizeof(FrameHeader)) != cudaSuccess) return fail(HIGS_E_NOMEM);
@@ -199,12 +207,12 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     memset(ctx->hdr_host, 0, sizeof(FrameHeader));
     if (cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(HIGS_E_CUDA);
     for (int i = 0; i < 9; ++i) if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) return fail(HIGS_E_CUDA);
-    for (int i = 0; i < 3; ++i) {
+    for (int i = 0; i < 4; ++i) {
         if (cudaStreamCreateWithFlags(&ctx->aux_stream[i], cudaStreamNonBlocking) != cudaSuccess) return fail(HIGS_E_CUDA);
         if (cudaEventCreateWithFlags(&ctx->ev_join[i], cudaEventDisableTiming) != cudaSuccess) return fail(HIGS_E_CUDA);
     }
     if (cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess) return fail(HIGS_E_CUDA);
-    if ((rc = higs_project_smem_setup(ctx))) return fail(rc);
+    if (cudaEventCreateWithFlags(&ctx->ev_fork2, cudaEventDisableTiming) != cudaSuccess) return fail(HIGS_E_CUDA);
     if ((rc = higs_binning_smem_setup(ctx))) return fail(rc);
     if ((rc = higs_sort_smem_setup(ctx))) return fail(rc);
     if ((rc = higs_raster_setup(ctx))) return fail(rc);
@@ -218,21 +226,23 @@ void higs_destroy(higs_ctx* ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
-    dev_free(ctx->valid_bits); dev_free(ctx->rec); dev_free(ctx->bin); dev_free(ctx->chunk_count); dev_free(ctx->rec_export); dev_free(ctx->hist); dev_free(ctx->base);
+    dev_free(ctx->valid_bits); dev_free(ctx->rec); dev_free(ctx->bin); dev_free(ctx->chunk_count); dev_free(ctx->part_list); dev_free(ctx->part_desc); dev_free(ctx->rec_export); dev_free(ctx->hist); dev_free(ctx->base);
     dev_free(ctx->mt_count); dev_free(ctx->mt_offset); dev_free(ctx->batch_offset); dev_free(ctx->unit_mt);
     dev_free(ctx->unit_active); dev_free(ctx->pairs); dev_free(ctx->pairs_alt); dev_free(ctx->sort_jobs);
-    dev_free(ctx->over_segs); dev_free(ctx->partial); dev_free(ctx->tile_maxT); dev_free(ctx->hdr);
+    dev_free(ctx->over_segs); dev_free(ctx->split_segs); dev_free(ctx->splitters); dev_free(ctx->bucket_count);
+    dev_free(ctx->bucket_cursor); dev_free(ctx->bucket_seg); dev_free(ctx->partial); dev_free(ctx->tile_maxT); dev_free(ctx->hdr);
     dev_free(ctx->unit_order); dev_free(ctx->level_hist); dev_free(ctx->level_cur);
     dev_free(ctx->s_means); dev_free(ctx->s_scales); dev_free(ctx->s_quats); dev_free(ctx->s_opac); dev_free(ctx->s_sh);
     dev_free(ctx->s_img);
     if (ctx->hdr_host) cudaFreeHost(ctx->hdr_host);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     for (int i = 0; i < 9; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
-    for (int i = 0; i < 3; ++i) {
+    for (int i = 0; i < 4; ++i) {
         if (ctx->aux_stream[i]) cudaStreamDestroy(ctx->aux_stream[i]);
         if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
     }
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_fork2) cudaEventDestroy(ctx->ev_fork2);
     cudaGetLastError();
     delete ctx;
 }

@@ -1,10 +1,11 @@
 // binning.cu -- steps a3 scan, a4 fill, a6 batch schedule (section 3.2,
 // PAPER.md:247-257 section 4.3, section 3.1).  The count pass (a2) lives in project.cu.
 //
-// Count and fill each run one CTA per partitioning batch of B_p = 8192 consecutive gaussian ids
-// (PAPER.md:89, 251); fill consumes the per-warp visibility bitfield of a1, so culled gaussians never
-// reach it.  The count CTA's histogram arrives as uint16 (a cell holds <= 8192) in the
-// N_B x N_M matrix; the scan widens it to 32-bit write bases in two levels (groups of 32 batches);
+// Count and fill each run one CTA per partitioning batch.  Here a batch is the set of
+// 512-id chunks one persistent projection CTA claimed (project.cu), so N_B = a whole number of CTAs per SM;
+// fill only touches the dense survivor slots, so culled gaussians never reach it.  The
+// count CTA's histogram is one row of the N_B x N_M matrix; the scan turns it into write bases in two
+// levels (groups of 32 batches);
 // the fill CTA replays the intersection -- from the 64-bit span descriptor the count left in the
 // record, or by redoing the row scan N-SCAN when the span did not fit -- and drops
 // (depth key << 32 | id) at base + local rank.
@@ -13,13 +14,13 @@
 
 namespace {
 
-constexpr int BIN_THREADS = 512;
+constexpr int BIN_THREADS = 1024;   // two CTAs per SM at 32 registers: the pass is latency-bound, so warps in flight decide
 constexpr int SCAN_GROUP  = 32;      // batches per first-level scan group
 
 // First scan level: CTA (column chunk, group) walks its <= 32 batches; base[b][m] = pairs of
 // macro-tile m in the earlier batches of the same group; gsum[g][m] = total of the group.
 __global__ void __launch_bounds__(256)
-k_scan_groups(const uint16_t* __restrict__ hist, int pitch, int n_batches, int n_m,
+k_scan_groups(const uint32_t* __restrict__ hist, int pitch, int n_batches, int n_m,
               uint32_t* __restrict__ base, uint32_t* __restrict__ gsum)
 {
     const int m = blockIdx.x * 256 + threadIdx.x;
@@ -160,25 +161,48 @@ k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, con
 
 #define HIGS_DESC_FALLBACK 0x8000000000000000ull   // see project.cu
 
-// a4: one CTA per partition batch, one warp per 512-id chunk; the chunk's survivors sit densely in `bin`, so the
-// loads are coalesced and every lane has work.  Items are (depth key << 32 | slot).
-__global__ void __launch_bounds__(BIN_THREADS)
-k_fill(const uint32_t* __restrict__ chunk_count, const uint4* __restrict__ bin, const float4* __restrict__ rec, const FrameParams P,
-       const uint32_t* __restrict__ base, const uint32_t* __restrict__ gbase, const uint32_t* __restrict__ mt_offset,
+// a4: one CTA per partition batch = per CTA of the projection kernel, which left the list of chunks it claimed.
+// The survivors of those chunks sit densely in `bin`; the CTA flattens them (prefix sum over the chunk counts) and
+// strides over them with all its threads, so the loads are coalesced, independent, and every lane has work.
+// Items are (depth key << 32 | slot).
+__global__ void __launch_bounds__(BIN_THREADS, 2)
+k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ part_list, const uint2* __restrict__ part_desc, int lcap,
+       const uint4* __restrict__ bin, const float4* __restrict__ rec,
+       const FrameParams P, const uint32_t* __restrict__ base, const uint32_t* __restrict__ gbase, const uint32_t* __restrict__ mt_offset,
        unsigned long long* __restrict__ pairs, const FrameHeader* __restrict__ hdr)
 {
     extern __shared__ uint32_t s_cursor[];
+    uint32_t* s_chunk = s_cursor + P.n_m;           // [lcap]
+    uint32_t* s_pref = s_chunk + lcap;              // [lcap + 1] exclusive prefix of the chunk counts
     if (hdr->overflow) return;                      // capacity exceeded: write nothing (HIGS_E_CAPACITY)
-    const int b = blockIdx.x, g = b / SCAN_GROUP;
+    const uint32_t b = blockIdx.x, g = b / SCAN_GROUP;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const uint2 pd = part_desc[b];
+    const uint32_t n_list = min(pd.y, (uint32_t)lcap);
+    if (w == 0) {                                   // chunk list + prefix of the counts (a few dozen entries)
+        uint32_t run = 0;
+        for (uint32_t e0 = 0; e0 < n_list; e0 += 32) {
+            const uint32_t e = e0 + lane;
+            const uint32_t c = e < n_list ? part_list[pd.x + e] : 0u;
+            const uint32_t n = e < n_list ? chunk_count[c] : 0u;
+            uint32_t x = n;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
+            if (e < n_list) { s_chunk[e] = c; s_pref[e] = run + x - n; }
+            run += __shfl_sync(0xffffffffu, x, 31);
+        }
+        if (lane == 0) s_pref[n_list] = run;
+    }
     for (int m = threadIdx.x; m < P.n_m; m += BIN_THREADS)
         s_cursor[m] = mt_offset[m] + gbase[(size_t)g * P.n_m + m] + base[(size_t)b * P.n_m + m];
     __syncthreads();
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const uint32_t cnt = chunk_count[b * (HIGS_PART_BATCH / HIGS_CHUNK) + w];
-    const size_t slot0 = (size_t)b * HIGS_PART_BATCH + (size_t)w * HIGS_CHUNK;
-    for (uint32_t k = lane; k < cnt; k += 32) {
-        const size_t slot = slot0 + k;
-        const uint4 bn = __ldcs(bin + slot);         // key, desc lo, desc hi, id
+    const uint32_t total = s_pref[n_list];
+    auto slot_of = [&](uint32_t k) -> size_t {
+        uint32_t lo = 0, hi = n_list - 1;           // last entry with pref <= k
+        while (lo < hi) { const uint32_t mid = (lo + hi + 1) >> 1; if (s_pref[mid] <= k) lo = mid; else hi = mid - 1; }
+        return (size_t)s_chunk[lo] * HIGS_CHUNK + (k - s_pref[lo]);
+    };
+    auto emit = [&](size_t slot, const uint4 bn) {  // bn = key, desc lo, desc hi, id
         const unsigned long long item = ((unsigned long long)bn.x << 32) | (unsigned long long)(uint32_t)slot;
         const unsigned long long desc = ((unsigned long long)bn.z << 32) | bn.y;
         if (!(desc & HIGS_DESC_FALLBACK)) {
@@ -202,6 +226,10 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint4* __restrict__ bin, 
                 for (int m = m0; m <= m1; ++m) pairs[atomicAdd(&s_cursor[r * P.n_mx + m], 1u)] = item;
             }
         }
+    };
+    for (uint32_t k = threadIdx.x; k < total; k += BIN_THREADS) {
+        const size_t slot = slot_of(k);
+        emit(slot, __ldcs(bin + slot));
     }
 }
 
@@ -240,25 +268,26 @@ __global__ void k_zero_lists(uint32_t* mt_count, uint32_t* mt_offset, uint32_t* 
 
 int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t st, cudaEvent_t ev_count, cudaEvent_t ev_scan)
 {
-    const int n_b = (int)((N + HIGS_PART_BATCH - 1) / HIGS_PART_BATCH);
-    const int pitch = (P.n_m + 1) & ~1;
+    const int n_b = N > 0 ? higs_part_grid(ctx, N) : 0;
+    const int pitch = P.n_m;
     if (n_b == 0) {
         k_zero_lists<<<(P.n_m + 256) / 256, 256, 0, st>>>(ctx->mt_count, ctx->mt_offset, ctx->batch_offset, P.n_m);
         HIGS_LAUNCHED(ctx);
         if (ev_count) { cudaEventRecord(ev_count, st); cudaEventRecord(ev_scan, st); }
         return HIGS_OK;
     }
-    const size_t smem = sizeof(uint32_t) * (size_t)P.n_m;
+    const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, n_b);
+    const size_t smem = sizeof(uint32_t) * ((size_t)P.n_m + 2 * (size_t)lcap + 1);
     if (ev_count) cudaEventRecord(ev_count, st);    // the count pass ran inside k_project: this stage is empty
     const int n_groups = (n_b + SCAN_GROUP - 1) / SCAN_GROUP;
-    uint32_t* gsum = ctx->base + (size_t)ctx->n_part_batches_max * ctx->max_nm;   // tail of the base allocation
+    uint32_t* gsum = ctx->base + (size_t)ctx->n_part_max * ctx->max_nm;   // tail of the base allocation
     k_scan_groups<<<dim3((P.n_m + 255) / 256, n_groups), 256, 0, st>>>(ctx->hist, pitch, n_b, P.n_m, ctx->base, gsum);
     HIGS_LAUNCHED(ctx);
     k_plan<<<1, 1024, 0, st>>>(gsum, n_groups, P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->unit_mt, ctx->unit_order,
                                ctx->level_hist, ctx->level_cur, ctx->hdr);
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
-    k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->chunk_count, ctx->bin, ctx->rec, P, ctx->base, gsum, ctx->mt_offset, ctx->pairs, ctx->hdr);
+    k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->chunk_count, ctx->part_list, ctx->part_desc, lcap, ctx->bin, ctx->rec, P, ctx->base, gsum, ctx->mt_offset, ctx->pairs, ctx->hdr);
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }
@@ -272,7 +301,7 @@ int launch_export_lists(higs_ctx* ctx, uint32_t n_pairs, cudaStream_t st)
 
 int launch_export_records(higs_ctx* ctx, int64_t N, cudaStream_t st)
 {
-    const int64_t n_slots = ((N + HIGS_PART_BATCH - 1) / HIGS_PART_BATCH) * HIGS_PART_BATCH;
+    const int64_t n_slots = ((N + HIGS_CHUNK - 1) / HIGS_CHUNK) * HIGS_CHUNK;
     k_export_records<<<(unsigned)((n_slots + 255) / 256), 256, 0, st>>>(ctx->chunk_count, ctx->rec, ctx->bin, n_slots, ctx->rec_export);
     HIGS_CUDA(ctx, cudaGetLastError());
     return HIGS_OK;
@@ -280,7 +309,9 @@ int launch_export_records(higs_ctx* ctx, int64_t N, cudaStream_t st)
 
 int higs_binning_smem_setup(higs_ctx* ctx)
 {
-    const int bytes = (int)(sizeof(uint32_t) * (size_t)ctx->max_nm);
+    int lcap_max = higs_part_lcap(ctx->n_chunks_max, ctx->n_sm);
+    if (lcap_max < 96) lcap_max = 96;
+    const int bytes = (int)(sizeof(uint32_t) * ((size_t)ctx->max_nm + 2 * (size_t)lcap_max + 1));
     if (bytes > 48 * 1024) {
         HIGS_CUDA(ctx, cudaFuncSetAttribute(k_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     }

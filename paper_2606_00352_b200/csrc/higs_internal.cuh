@@ -11,6 +11,9 @@
 #define HIGS_N_TIERS    4            // block-sort tiers, capacities 1024 / 2048 / 4096 / 8192
 #define HIGS_CHUNK      512          // consecutive ids projected by one warp; survivors are stored densely per chunk
 #define HIGS_MERGE_TILE 4096         // output items per merge-path tile (overflow path)
+#define HIGS_SPLIT_TILE 4096         // items per CTA pass of the bucket count / scatter kernels
+#define HIGS_BUCKET_TARGET 1536      // mean items per depth bucket of an oversize segment
+#define HIGS_MAX_SPLIT  512          // most buckets per oversize segment (splitters live in shared memory)
 
 // ---- per-frame device header: every data-dependent size lives here, never on the host ----------
 struct FrameHeader {
@@ -18,21 +21,28 @@ struct FrameHeader {
     uint32_t n_units;          // N_R (0 when overflow)
     uint32_t overflow;         // pairs or units exceeded the preallocated capacity
     uint32_t max_segment;
-    uint32_t n_oversize;       // segments > HIGS_SORT_BLOCK
-    uint32_t n_merge_tiles;    // sum over oversize segments of ceil(n / HIGS_MERGE_TILE)
-    uint32_t max_levels;       // merge levels needed by the longest oversize segment
-    uint32_t n_sort_jobs[HIGS_N_TIERS];
-    uint32_t sort_cursor[HIGS_N_TIERS];   // work counters (persistent kernels)
+    uint32_t n_oversize;       // segments > HIGS_SORT_BLOCK: split into depth buckets first (sort.cu)
+    uint32_t n_split_tiles;    // sum over oversize segments of ceil(n / HIGS_SPLIT_TILE)
+    uint32_t n_buckets;        // buckets of all oversize segments
+    uint32_t n_fallback;       // buckets that still exceed HIGS_SORT_BLOCK: block sort + merge levels
+    uint32_t n_merge_tiles;    // sum over fallback buckets of ceil(n / HIGS_MERGE_TILE)
+    uint32_t max_levels;       // merge levels needed by the longest fallback bucket
+    uint32_t n_sort_jobs[2][HIGS_N_TIERS];   // [0] whole segments, [1] buckets of oversize segments
+    uint32_t sort_cursor[2][HIGS_N_TIERS];   // work counters (persistent kernels)
+    uint32_t split_cursor[3];  // work counters of the split / count / scatter kernels
     uint32_t raster_cursor;
     uint32_t merge_barrier;    // software grid barrier of the merge kernel
     uint32_t n_visible;
-    uint32_t pad0;
+    uint32_t proj_cursor;      // chunk counter of the projection kernel
+    uint32_t part_list_cursor; // entries of part_list handed out
+    uint32_t pad1;
     unsigned long long n_evals;
     unsigned long long n_tile_pairs;
 };
 
-struct SortJob   { uint32_t start, len, dst_alt, pad; };           // dst_alt: write sorted chunk to the alternate buffer
-struct OverSeg   { uint32_t start, len, levels, tile_base; };     // an oversize segment and its merge plan
+struct SortJob   { uint32_t start, len, flags, pad; };             // flags bit 0: write the sorted run to the alternate buffer, bit 1: read it there
+struct OverSeg   { uint32_t start, len, levels, tile_base; };     // a fallback bucket and its merge plan
+struct SplitSeg  { uint32_t start, len, nb, bucket_base, tile_base, items_before, oversample, pad; };   // an oversize segment and its bucket plan
 
 // camera + frame constants handed to the kernels by value
 struct FrameParams {
@@ -52,7 +62,8 @@ struct higs_ctx {
     int64_t max_gaussians;
     int max_W, max_H, max_nm;
     int64_t max_pairs, max_units;
-    int n_part_batches_max;
+    int n_part_max;            // partition CTAs (= histogram rows): n_sm x resident k_project CTAs
+    int64_t n_chunks_max;
     int n_sm;
     uint32_t flags;
     int batch_cap;
@@ -60,11 +71,13 @@ struct higs_ctx {
     uint32_t* valid_bits;      // [ceil(maxN/32)]
     float4*   rec;             // [slots][4]  mux,muy,A,B2 | C,tau,log2o,r | g,b,a,b | c,bits(key),id,-   (64 B; the rasterizer gathers the
                                //             first 40 B).  A slot is the dense position of a surviving gaussian: survivor k of the
-                               //             512-id chunk (batch b, warp w) sits at b*8192 + w*512 + k (monotone in the id)
+                               //             512-id chunk c sits at c*512 + k (monotone in the id)
     uint4*    bin;             // [slots]     bits(key), span descriptor lo, hi, id   (16 B, read by fill)
-    uint32_t* chunk_count;     // [N_B*16]    survivors per chunk
+    uint32_t* chunk_count;     // [chunks]    survivors of the chunk
+    uint32_t* part_list;       // [chunks]    chunk ids grouped by the partition CTA that claimed them
+    uint2*    part_desc;       // [N_B]       (first entry, entries) of each partition CTA in part_list
     float*    rec_export;      // [maxN][16]  test-facing copy indexed by gaussian id, allocated by the first higs_get_records
-    uint16_t* hist;            // [N_B][N_M]
+    uint32_t* hist;            // [N_B][N_M]
     uint32_t* base;            // [N_B][N_M] write base of (batch, macro-tile) relative to mt_offset[m]
     uint32_t* mt_count;        // [max_nm]
     uint32_t* mt_offset;       // [max_nm+1]
@@ -76,10 +89,16 @@ struct higs_ctx {
     uint32_t* level_cur;       // [max_units+2]
     unsigned long long* pairs; // [max_pairs]
     unsigned long long* pairs_alt; // [max_pairs] ping-pong buffer of the overflow merge
-    SortJob*  sort_jobs;       // [HIGS_N_TIERS][max_jobs]
+    SortJob*  sort_jobs;       // [2][HIGS_N_TIERS][max_jobs]  list 0: whole segments, list 1: buckets
     int64_t   max_jobs;
-    OverSeg*  over_segs;       // [max_over]
+    OverSeg*  over_segs;       // [max_over]   fallback buckets (merge path)
+    SplitSeg* split_segs;      // [max_over]   oversize segments
     int64_t   max_over;
+    unsigned long long* splitters;   // [max_buckets]  bucket b of a segment holds items in [splitter[b-1], splitter[b])
+    uint32_t* bucket_count;    // [max_buckets]
+    uint32_t* bucket_cursor;   // [max_buckets]  write position of the scatter pass
+    uint32_t* bucket_seg;      // [max_buckets]  index into split_segs
+    int64_t   max_buckets;
     float4*   partial;         // [max_units][32 tiles][64 px] (r,g,b,T)
     float*    tile_maxT;       // [max_units][32] largest transmittance left in (unit, tile); 1 = unknown
     FrameHeader* hdr;          // device
@@ -92,8 +111,8 @@ struct higs_ctx {
     int64_t last_n; int last_W, last_H, last_nm; int last_mx, last_my;
     cudaStream_t last_stream;
     cudaStream_t own_stream;
-    cudaStream_t aux_stream[3];   // forked from the render stream for the small sort tiers
-    cudaEvent_t ev_fork, ev_join[3];
+    cudaStream_t aux_stream[4];   // forked from the render stream for the sort tiers
+    cudaEvent_t ev_fork, ev_fork2, ev_join[4];
     cudaEvent_t ev[9];
     bool timers_valid;
     int n_launches;            // kernels enqueued by the current / last frame
@@ -110,6 +129,8 @@ struct higs_ctx {
 // ---- launch entry points, one per pipeline step (defined in the .cu files) ----------------------
 int launch_project(higs_ctx*, const FrameParams&, const float* means, const float* scales, const float* quats,
                    const float* opac, const float* sh, int64_t N, cudaStream_t);
+int higs_part_grid(const higs_ctx*, int64_t N);
+int higs_part_lcap(int64_t n_chunks, int grid);
 int launch_binning(higs_ctx*, const FrameParams&, int64_t N, cudaStream_t, cudaEvent_t ev_count, cudaEvent_t ev_scan);
 int launch_sort(higs_ctx*, const FrameParams&, cudaStream_t);
 int launch_sort_only(higs_ctx*, unsigned long long* pairs, const uint32_t* seg_offset, int n_seg, cudaStream_t);

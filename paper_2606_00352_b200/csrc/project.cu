@@ -1,7 +1,7 @@
 // project.cu -- steps a1 + a2: fused EWA projection + cull + SH colour (section 4.2), with the
-// count pass of the partitioning folded in: one CTA per partition batch of B_p = 8192
-// consecutive ids keeps the private shared-memory histogram with one counter per macro-tile and flushes it as
-// packed uint16 into the N_B x N_M matrix.  The kernel is HBM-latency-bound, so the row scan runs in issue
+// count pass of the partitioning folded in: every persistent CTA is one partition batch
+// (the chunks of 512 consecutive ids its warps claim), keeps the private shared-memory histogram with one counter
+// per macro-tile and flushes it as one row of the N_B x N_M matrix (N_B = CTAs = a whole number per SM).  The kernel is HBM-latency-bound, so the row scan runs in issue
 // slots that were idle; the macro-tile span it finds is also packed into a 64-bit descriptor in the record, so
 // the fill pass replays it without redoing the arithmetic.  (Section 4.2:
 // "Each thread processes one gaussian end-to-end: camera-space transformation, 2D covariance via
@@ -97,7 +97,6 @@ __device__ __forceinline__ void sh_accumulate(const float* __restrict__ shp, flo
 
 constexpr int PROJ_THREADS = 512;
 constexpr int PROJ_WARPS = PROJ_THREADS / 32;
-constexpr int PROJ_CHUNK = HIGS_PART_BATCH / PROJ_WARPS;   // consecutive ids owned by one warp (512)
 constexpr int PROJ_QCAP = 64;                              // per-warp survivor queue (entries), >= 31 + 32
 constexpr int PROJ_QF = 15;                                // words per queued survivor
 
@@ -246,99 +245,148 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
     bin[slot] = make_uint4(key, (uint32_t)desc, (uint32_t)(desc >> 32), (uint32_t)i);
 }
 
-// One CTA per partition batch (8192 ids), one warp per chunk of 512 consecutive ids.  A warp runs phase A on 32
-// gaussians at a time and queues the survivors (about 4 in 10 at paper scale) in shared memory; whenever 32 are
-// queued it runs phase B on them with every lane busy.  Survivor k of chunk (b, w) gets dense slot
-// b*8192 + w*512 + k: slots are monotone in the gaussian id, so (key, slot) order = (key, id) order (Q7).
+// Persistent CTAs (a whole number per SM), one histogram row per CTA.  A warp claims chunks of HIGS_CHUNK = 512
+// consecutive ids from a device counter, so the load balances itself and the grid never has a partial wave; the
+// paper's fixed partition batch of B_p consecutive ids becomes "the chunks one CTA happened to
+// claim", recorded in chunk_count's high half for the fill pass.  A warp runs phase A on 32 gaussians at a time
+// and queues the survivors (about 4 in 10 at paper scale) in shared memory; whenever 32 are queued it runs phase B
+// on them with every lane busy.  Survivor k of chunk c gets dense slot c*512 + k: slots are monotone in the
+// gaussian id, so (key, slot) order = (key, id) order (Q7).
 template <int DEG>
 __global__ void __launch_bounds__(PROJ_THREADS, 2)
 k_project(const float* __restrict__ means, const float* __restrict__ scales, const float* __restrict__ quats,
           const float* __restrict__ opac, const float* __restrict__ sh, int64_t N, const FrameParams P,
           uint32_t* __restrict__ valid_bits, float4* __restrict__ rec, uint4* __restrict__ bin,
-          uint32_t* __restrict__ chunk_count, uint16_t* __restrict__ hist, int pitch, FrameHeader* __restrict__ hdr)
+          uint32_t* __restrict__ chunk_count, uint32_t* __restrict__ hist, uint32_t* __restrict__ part_list,
+          uint2* __restrict__ part_desc, int lcap, FrameHeader* __restrict__ hdr)
 {
     extern __shared__ uint32_t s_dyn[];
-    __shared__ uint32_t s_nvis;
+    __shared__ uint32_t s_nvis, s_nlist, s_lbase;
     uint32_t* s_hist = s_dyn;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     float* q = reinterpret_cast<float*>(s_dyn + ((P.n_m + 3) & ~3)) + w * (PROJ_QF * PROJ_QCAP);
+    uint32_t* s_list = s_dyn + ((P.n_m + 3) & ~3) + PROJ_WARPS * PROJ_QF * PROJ_QCAP;   // [lcap] chunks this CTA claimed
     for (int m = threadIdx.x; m < P.n_m; m += PROJ_THREADS) s_hist[m] = 0;
-    if (threadIdx.x == 0) s_nvis = 0;
+    if (threadIdx.x == 0) { s_nvis = 0; s_nlist = 0; }
     __syncthreads();
-    const int64_t c0 = (int64_t)blockIdx.x * HIGS_PART_BATCH + (int64_t)w * PROJ_CHUNK;
-    const size_t slot0 = (size_t)c0;
+    const uint32_t n_chunks = (uint32_t)((N + HIGS_CHUNK - 1) / HIGS_CHUNK);
     const uint32_t lt = (1u << lane) - 1u;
-    uint32_t head = 0, tail = 0;
+    uint32_t n_mine = 0;
 
-    auto drain = [&](uint32_t n_live) {                              // phase B on queue entries head .. head+n_live-1
-        if ((uint32_t)lane < n_live) {
-            const int e = (int)((head + lane) & (PROJ_QCAP - 1));
+    for (;;) {
+        uint32_t chunk = 0xffffffffu;
+        if (lane == 0) {                                             // a list entry first, then the chunk that goes in it
+            const uint32_t e = atomicAdd(&s_nlist, 1u);
+            if (e < (uint32_t)lcap) {
+                chunk = atomicAdd(&hdr->proj_cursor, 1u);
+                s_list[e] = chunk < n_chunks ? chunk : 0xffffffffu;
+            }
+        }
+        chunk = __shfl_sync(0xffffffffu, chunk, 0);
+        if (chunk >= n_chunks) break;
+        const int64_t c0 = (int64_t)chunk * HIGS_CHUNK;
+        const size_t slot0 = (size_t)c0;
+        uint32_t head = 0, tail = 0;
+
+        auto drain = [&](uint32_t n_live) {                          // phase B on queue entries head .. head+n_live-1
+            if ((uint32_t)lane < n_live) {
+                const int e = (int)((head + lane) & (PROJ_QCAP - 1));
+                Survivor s;
+                s.mux = q[0 * PROJ_QCAP + e]; s.muy = q[1 * PROJ_QCAP + e]; s.a = q[2 * PROJ_QCAP + e]; s.b = q[3 * PROJ_QCAP + e];
+                s.c = q[4 * PROJ_QCAP + e]; s.A = q[5 * PROJ_QCAP + e]; s.B2 = q[6 * PROJ_QCAP + e]; s.C = q[7 * PROJ_QCAP + e];
+                s.tau = q[8 * PROJ_QCAP + e]; s.zc = q[9 * PROJ_QCAP + e]; s.o = q[10 * PROJ_QCAP + e];
+                s.mx = q[11 * PROJ_QCAP + e]; s.my = q[12 * PROJ_QCAP + e]; s.mz = q[13 * PROJ_QCAP + e];
+                s.local = __float_as_uint(q[14 * PROJ_QCAP + e]);
+                emit_survivor<DEG>(s, c0 + s.local, slot0 + head + lane, sh, P, s_hist, rec, bin);
+            }
+            head += n_live;
+            __syncwarp();
+        };
+
+        RawIn nxt = {};
+        if (c0 + lane < N) nxt = load_raw(means, scales, quats, opac, c0 + lane);
+        for (int it = 0; it < HIGS_CHUNK / 32; ++it) {
+            const int64_t i = c0 + it * 32 + lane;
+            if (c0 + it * 32 >= N) break;                            // warp-uniform
+            const RawIn cur = nxt;
+            if (it + 1 < HIGS_CHUNK / 32 && i + 32 < N) nxt = load_raw(means, scales, quats, opac, i + 32);
             Survivor s;
-            s.mux = q[0 * PROJ_QCAP + e]; s.muy = q[1 * PROJ_QCAP + e]; s.a = q[2 * PROJ_QCAP + e]; s.b = q[3 * PROJ_QCAP + e];
-            s.c = q[4 * PROJ_QCAP + e]; s.A = q[5 * PROJ_QCAP + e]; s.B2 = q[6 * PROJ_QCAP + e]; s.C = q[7 * PROJ_QCAP + e];
-            s.tau = q[8 * PROJ_QCAP + e]; s.zc = q[9 * PROJ_QCAP + e]; s.o = q[10 * PROJ_QCAP + e];
-            s.mx = q[11 * PROJ_QCAP + e]; s.my = q[12 * PROJ_QCAP + e]; s.mz = q[13 * PROJ_QCAP + e];
-            s.local = __float_as_uint(q[14 * PROJ_QCAP + e]);
-            emit_survivor<DEG>(s, c0 + s.local, slot0 + head + lane, sh, P, s_hist, rec, bin);
+            const bool ok = (i < N) && project_cull(cur, P, s);
+            const uint32_t vmask = __ballot_sync(0xffffffffu, ok);
+            if (lane == 0) valid_bits[i >> 5] = vmask;               // chunk bases are multiples of 32
+            if (ok) {
+                const int e = (int)((tail + __popc(vmask & lt)) & (PROJ_QCAP - 1));
+                q[0 * PROJ_QCAP + e] = s.mux; q[1 * PROJ_QCAP + e] = s.muy; q[2 * PROJ_QCAP + e] = s.a; q[3 * PROJ_QCAP + e] = s.b;
+                q[4 * PROJ_QCAP + e] = s.c; q[5 * PROJ_QCAP + e] = s.A; q[6 * PROJ_QCAP + e] = s.B2; q[7 * PROJ_QCAP + e] = s.C;
+                q[8 * PROJ_QCAP + e] = s.tau; q[9 * PROJ_QCAP + e] = s.zc; q[10 * PROJ_QCAP + e] = s.o;
+                q[11 * PROJ_QCAP + e] = s.mx; q[12 * PROJ_QCAP + e] = s.my; q[13 * PROJ_QCAP + e] = s.mz;
+                q[14 * PROJ_QCAP + e] = __uint_as_float((uint32_t)(it * 32 + lane));
+            }
+            tail += __popc(vmask);
+            __syncwarp();
+            if (tail - head >= 32u) drain(32u);
         }
-        head += n_live;
-        __syncwarp();
-    };
-
-    RawIn nxt = {};
-    if (c0 + lane < N) nxt = load_raw(means, scales, quats, opac, c0 + lane);
-    for (int it = 0; it < PROJ_CHUNK / 32; ++it) {
-        const int64_t i = c0 + it * 32 + lane;
-        if (c0 + it * 32 >= N) break;                                // warp-uniform
-        const RawIn cur = nxt;
-        if (it + 1 < PROJ_CHUNK / 32 && i + 32 < N) nxt = load_raw(means, scales, quats, opac, i + 32);
-        Survivor s;
-        const bool ok = (i < N) && project_cull(cur, P, s);
-        const uint32_t vmask = __ballot_sync(0xffffffffu, ok);
-        if (lane == 0) valid_bits[i >> 5] = vmask;                   // chunk bases are multiples of 32
-        if (ok) {
-            const int e = (int)((tail + __popc(vmask & lt)) & (PROJ_QCAP - 1));
-            q[0 * PROJ_QCAP + e] = s.mux; q[1 * PROJ_QCAP + e] = s.muy; q[2 * PROJ_QCAP + e] = s.a; q[3 * PROJ_QCAP + e] = s.b;
-            q[4 * PROJ_QCAP + e] = s.c; q[5 * PROJ_QCAP + e] = s.A; q[6 * PROJ_QCAP + e] = s.B2; q[7 * PROJ_QCAP + e] = s.C;
-            q[8 * PROJ_QCAP + e] = s.tau; q[9 * PROJ_QCAP + e] = s.zc; q[10 * PROJ_QCAP + e] = s.o;
-            q[11 * PROJ_QCAP + e] = s.mx; q[12 * PROJ_QCAP + e] = s.my; q[13 * PROJ_QCAP + e] = s.mz;
-            q[14 * PROJ_QCAP + e] = __uint_as_float((uint32_t)(it * 32 + lane));
-        }
-        tail += __popc(vmask);
-        __syncwarp();
-        if (tail - head >= 32u) drain(32u);
+        if (tail > head) drain(tail - head);
+        if (lane == 0) chunk_count[chunk] = tail;
+        n_mine += tail;
     }
-    if (tail > head) drain(tail - head);
-    if (lane == 0) {
-        chunk_count[blockIdx.x * PROJ_WARPS + w] = tail;
-        if (tail) atomicAdd(&s_nvis, tail);
-    }
+    if (lane == 0 && n_mine) atomicAdd(&s_nvis, n_mine);
     __syncthreads();
-    uint32_t* row = reinterpret_cast<uint32_t*>(hist + (size_t)blockIdx.x * pitch);   // pitch is even
-    for (int m2 = threadIdx.x; m2 < pitch / 2; m2 += PROJ_THREADS) {
-        const int m = 2 * m2;
-        const uint32_t lo = s_hist[m], hi = (m + 1 < P.n_m) ? s_hist[m + 1] : 0u;
-        row[m2] = lo | (hi << 16);                                   // a cell holds <= 8192: uint16 is enough
+    // this CTA's partition batch = the chunks it claimed: compacted into the global list for the fill pass
+    if (w == 0) {
+        const uint32_t n_e = min(s_nlist, (uint32_t)lcap);
+        uint32_t n_valid = 0;
+        for (uint32_t e0 = 0; e0 < n_e; e0 += 32) n_valid += __popc(__ballot_sync(0xffffffffu, e0 + lane < n_e && s_list[e0 + lane] != 0xffffffffu));
+        if (lane == 0) {
+            s_lbase = atomicAdd(&hdr->part_list_cursor, n_valid);
+            part_desc[blockIdx.x] = make_uint2(s_lbase, n_valid);
+        }
+        __syncwarp();
+        uint32_t at = s_lbase;
+        for (uint32_t e0 = 0; e0 < n_e; e0 += 32) {
+            const uint32_t c = e0 + lane < n_e ? s_list[e0 + lane] : 0xffffffffu;
+            const uint32_t ok = __ballot_sync(0xffffffffu, c != 0xffffffffu);
+            if (c != 0xffffffffu) part_list[at + __popc(ok & lt)] = c;
+            at += __popc(ok);
+        }
     }
+    uint32_t* row = hist + (size_t)blockIdx.x * P.n_m;
+    for (int m = threadIdx.x; m < P.n_m; m += PROJ_THREADS) row[m] = s_hist[m];
     if (threadIdx.x == 0 && s_nvis) atomicAdd(&hdr->n_visible, s_nvis);
 }
 
 } // namespace
 
-static size_t project_smem_bytes(int n_m)
+static size_t project_smem_bytes(int n_m, int lcap)
 {
-    return sizeof(uint32_t) * (size_t)((n_m + 3) & ~3) + sizeof(float) * (size_t)PROJ_WARPS * PROJ_QF * PROJ_QCAP;
+    return sizeof(uint32_t) * (size_t)((n_m + 3) & ~3) + sizeof(float) * (size_t)PROJ_WARPS * PROJ_QF * PROJ_QCAP + sizeof(uint32_t) * (size_t)lcap;
+}
+
+// list capacity of one partition CTA: four times its fair share of the chunks, so a CTA that fills its list and
+// retires early always leaves others with room (sum of capacities > chunks: every chunk finds a taker)
+int higs_part_lcap(int64_t n_chunks, int grid) { return (int)(4 * ((n_chunks + grid - 1) / grid) + 2 * PROJ_WARPS); }
+
+static int g_proj_ctas_per_sm = 2;
+
+// CTAs of the partition passes (project+count, fill) for N gaussians: a whole number per SM, fewer only when
+// there are not enough chunks to give every warp one
+int higs_part_grid(const higs_ctx* ctx, int64_t N)
+{
+    const int64_t n_chunks = (N + HIGS_CHUNK - 1) / HIGS_CHUNK;
+    const int64_t want = (n_chunks + PROJ_WARPS - 1) / PROJ_WARPS;
+    const int64_t cap = (int64_t)ctx->n_part_max;
+    return (int)(want < 1 ? 1 : (want > cap ? cap : want));
 }
 
 int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, const float* scales, const float* quats,
                    const float* opac, const float* sh, int64_t N, cudaStream_t st)
 {
     if (N <= 0) return HIGS_OK;
-    const unsigned grid = (unsigned)((N + HIGS_PART_BATCH - 1) / HIGS_PART_BATCH);
-    const size_t smem = project_smem_bytes(P.n_m);
-    const int pitch = (P.n_m + 1) & ~1;
+    const unsigned grid = (unsigned)higs_part_grid(ctx, N);
+    const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, (int)grid);
+    const size_t smem = project_smem_bytes(P.n_m, lcap);
 #define HIGS_PROJ(D) k_project<D><<<grid, PROJ_THREADS, smem, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
-                                                                   ctx->bin, ctx->chunk_count, ctx->hist, pitch, ctx->hdr)
+                                                                   ctx->bin, ctx->chunk_count, ctx->hist, ctx->part_list, ctx->part_desc, lcap, ctx->hdr)
     switch (P.degree) {
         case 0: HIGS_PROJ(0); break;
         case 1: HIGS_PROJ(1); break;
@@ -352,10 +400,16 @@ int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, cons
 
 int higs_project_smem_setup(higs_ctx* ctx)
 {
-    const int bytes = (int)project_smem_bytes(ctx->max_nm);
+    // worst case for the list: the full grid on max_gaussians (a smaller grid has at most 16 chunks per CTA)
+    const int lcap_max = higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) > 6 * PROJ_WARPS ? higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) : 6 * PROJ_WARPS;
+    const int bytes = (int)project_smem_bytes(ctx->max_nm, lcap_max);
     HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    int occ = 0;
+    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3>, PROJ_THREADS, (size_t)bytes));
+    g_proj_ctas_per_sm = occ < 1 ? 1 : occ;
+    ctx->n_part_max = ctx->n_sm * g_proj_ctas_per_sm;
     return HIGS_OK;
 }

@@ -232,6 +232,27 @@ def test_sort_segments_alone_against_numpy(hg):
     hg.higs_destroy(ctx)
 
 
+def test_sort_huge_segment_takes_bucket_fallback(hg):
+    """A 5 M-item segment: more than 512 buckets x 8192, so buckets exceed one block and take the merge-level path."""
+    import torch
+    rng = np.random.default_rng(10)
+    sizes = [5_000_000, 9000, 3]
+    off = np.concatenate([[0], np.cumsum(sizes)]).astype(np.uint32)
+    n = int(off[-1])
+    keys = rng.integers(0x3f000000, 0x41000000, n, dtype=np.uint64)
+    pairs = (keys << np.uint64(32)) | rng.permutation(n).astype(np.uint64)
+    ctx = hg.higs_create(0, 1000, 640, 480, max_pairs=n + 10)
+    d_pairs = torch.from_numpy(pairs.view(np.int64)).cuda()
+    d_off = torch.from_numpy(off.view(np.int32)).cuda()
+    hg.higs_sort_segments(ctx, d_pairs, d_off)
+    torch.cuda.synchronize()
+    got = d_pairs.cpu().numpy().view(np.uint64)
+    for s in range(len(sizes)):
+        a, b = int(off[s]), int(off[s + 1])
+        assert np.array_equal(got[a:b], np.sort(pairs[a:b])), f"segment {s} of size {sizes[s]}"
+    hg.higs_destroy(ctx)
+
+
 def test_cfg3_shaped_reduced_scene_lists_and_sampled_pixels(hg):
     """The large generator at 300k gaussians, 1080p: lists bit-exact, pixels checked on sampled windows."""
     s = hs.scene_large(N=300_000, W=1920, H=1080)
