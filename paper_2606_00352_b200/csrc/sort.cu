@@ -94,7 +94,7 @@ k_sort_plan(const uint32_t* __restrict__ seg_offset, int n_seg, int honour_overf
         if (t >= 0) jobs[(size_t)t * max_jobs + v[t]] = SortJob{start, n, 0u, 0u};
         if (over) {
             uint32_t a = 8192u / nb;                    // sample = a * nb <= 8192 items, sorted by one CTA
-            a = a > 32u ? 32u : a;
+            a = a > 16u ? 16u : a;                      // 16 sample items per bucket: bucket sizes within about +-25 % (1 sigma)
             split[v[4]] = SplitSeg{start, n, nb, v[6], v[5], v[7], a, 0u};
         }
     }
@@ -499,7 +499,6 @@ int setup_tier(higs_ctx* ctx, int tier)
 
 int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, int honour_overflow, cudaStream_t st)
 {
-    static const int sched = getenv("HIGS_SORT_SCHED") ? atoi(getenv("HIGS_SORT_SCHED")) : 0;
     SortJob* jobs0 = ctx->sort_jobs;
     SortJob* jobs1 = ctx->sort_jobs + (size_t)HIGS_N_TIERS * ctx->max_jobs;
     u64* alt = ctx->pairs_alt;
@@ -510,7 +509,7 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, i
     // while the main stream splits the oversize segments into buckets
     HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_fork, st));
     for (int k = 0; k < 4; ++k) HIGS_CUDA(ctx, cudaStreamWaitEvent(ctx->aux_stream[k], ctx->ev_fork, 0));
-    if (sched == 0) { if ((rc = launch_tier<512>(ctx, 0, 3, pairs, ctx->aux_stream[0]))) return rc; }
+    if ((rc = launch_tier<512>(ctx, 0, 3, pairs, ctx->aux_stream[0]))) return rc;
     if ((rc = launch_tier<256>(ctx, 0, 2, pairs, ctx->aux_stream[1]))) return rc;
     if ((rc = launch_tier<128>(ctx, 0, 1, pairs, ctx->aux_stream[2]))) return rc;
     if ((rc = launch_tier<64>(ctx, 0, 0, pairs, ctx->aux_stream[3]))) return rc;
@@ -528,7 +527,6 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, i
     HIGS_LAUNCHED(ctx);
     HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_fork2, st));
     for (int k = 1; k < 4; ++k) HIGS_CUDA(ctx, cudaStreamWaitEvent(ctx->aux_stream[k], ctx->ev_fork2, 0));
-    if (sched != 0) { if ((rc = launch_tier<512>(ctx, 0, 3, pairs, st))) return rc; }
     if ((rc = launch_tier<512>(ctx, 1, 3, pairs, st))) return rc;
     if ((rc = launch_tier<256>(ctx, 1, 2, pairs, ctx->aux_stream[1]))) return rc;
     if ((rc = launch_tier<128>(ctx, 1, 1, pairs, ctx->aux_stream[2]))) return rc;
