@@ -38,12 +38,12 @@ int alloc_unit_buffers(higs_ctx* ctx)
     ctx->max_units = ctx->max_nm + (ctx->max_pairs + ctx->batch_cap - 1) / ctx->batch_cap + 1;
     int rc;
     if ((rc = dev_alloc(ctx, &ctx->unit_mt, (size_t)ctx->max_units))) return rc;
-    if ((rc = dev_alloc(ctx, &ctx->unit_active, (size_t)ctx->max_units))) return rc;
-    if ((rc = dev_alloc(ctx, &ctx->unit_order, (size_t)ctx->max_units))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->unit_active, (size_t)ctx->max_units * HIGS_RASTER_SPLIT))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->unit_order, (size_t)ctx->max_units * HIGS_RASTER_SPLIT))) return rc;
     if ((rc = dev_alloc(ctx, &ctx->level_hist, (size_t)ctx->max_units + 2))) return rc;
-    if ((rc = dev_alloc(ctx, &ctx->level_cur, (size_t)ctx->max_units + 2))) return rc;
-    if ((rc = dev_alloc(ctx, &ctx->partial, (size_t)ctx->max_units * HIGS_MT_TILES * 64))) return rc;
-    if ((rc = dev_alloc(ctx, &ctx->tile_maxT, (size_t)ctx->max_units * HIGS_MT_TILES))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->level_cur, 3 * ((size_t)ctx->max_units + 2)))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->partial, (size_t)ctx->max_units * HIGS_RASTER_SPLIT * HIGS_MT_TILES * 64))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->tile_maxT, (size_t)ctx->max_units * HIGS_RASTER_SPLIT * HIGS_MT_TILES))) return rc;
     return HIGS_OK;
 }
 
@@ -78,7 +78,7 @@ int render_impl(higs_ctx* ctx, const float* means, const float* scales, const fl
     ctx->n_launches = 0;
     HIGS_CUDA(ctx, cudaMemsetAsync(ctx->hdr, 0, sizeof(FrameHeader), st));
     if (!(ctx->flags & HIGS_FLAG_NO_XBATCH_CUT))
-        HIGS_CUDA(ctx, cudaMemsetAsync(ctx->tile_maxT, 0, sizeof(float) * (size_t)ctx->max_units * HIGS_MT_TILES, st));
+        HIGS_CUDA(ctx, cudaMemsetAsync(ctx->tile_maxT, 0, sizeof(float) * (size_t)ctx->max_units * HIGS_RASTER_SPLIT * HIGS_MT_TILES, st));
     if (timers) cudaEventRecord(ev[0], st);
     if ((rc = launch_project(ctx, P, means, scales, quats, opac, sh, N, st))) return rc;
     if (timers) cudaEventRecord(ev[1], st);

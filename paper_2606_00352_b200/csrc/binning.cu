@@ -115,7 +115,9 @@ k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, con
         hdr->max_segment = s_max;
     }
     if (overflow) return;
-    // pass 2: unit table, and the order the rasterizer claims units in: batch index j major ("level" j =
+    uint32_t* level_base = level_cur + (P.max_units + 2);
+    uint32_t* level_cnt = level_base + (P.max_units + 2);
+    // pass 2: unit table, and the order the rasterizer claims (sub-)units in: batch index j major ("level" j =
     // the j-th batch of every macro-tile that has one), so that by the time a deep batch starts the batches
     // in front of it have published their transmittance bounds (cross-batch cut).
     const uint32_t max_nb = (s_max + br - 1) / br;
@@ -147,7 +149,7 @@ k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, con
             const uint32_t cnt = (j < max_nb) ? n_nonempty - v[0] : 0u;     // macro-tiles with nb > j
             uint32_t b[1] = { cnt };
             block_scan_excl<1>(b, c_base, s_warp);
-            if (j < max_nb) level_cur[j] = b[0];
+            if (j < max_nb) { level_cur[j] = b[0]; level_base[j] = b[0]; level_cnt[j] = cnt; }
         }
     }
     __syncthreads();
@@ -155,7 +157,12 @@ k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, con
         int lo = 0, hi = P.n_m - 1;                                       // last m with batch_offset[m] <= u and a batch there
         while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (batch_offset[mid] <= u) lo = mid; else hi = mid - 1; }
         unit_mt[u] = (uint32_t)lo;
-        unit_order[atomicAdd(&level_cur[u - batch_offset[lo]], 1u)] = u;
+        // sub-unit (u, h) = part h of unit u (HIGS_RASTER_SPLIT parts): level j's first parts, then its second parts, ...
+        const uint32_t lvl = u - batch_offset[lo];
+        const uint32_t p = atomicAdd(&level_cur[lvl], 1u) - level_base[lvl];
+#pragma unroll
+        for (uint32_t h = 0; h < HIGS_RASTER_SPLIT; ++h)
+            unit_order[HIGS_RASTER_SPLIT * level_base[lvl] + h * level_cnt[lvl] + p] = u * HIGS_RASTER_SPLIT + h;
     }
 }
 

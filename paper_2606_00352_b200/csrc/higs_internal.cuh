@@ -83,10 +83,11 @@ struct higs_ctx {
     uint32_t* mt_offset;       // [max_nm+1]
     uint32_t* batch_offset;    // [max_nm+1]
     uint32_t* unit_mt;         // [max_units] macro-tile of unit u
-    uint32_t* unit_active;     // [max_units]
-    uint32_t* unit_order;      // [max_units] units in the order the rasterizer claims them: batch index j major
+    uint32_t* unit_active;     // [max_units * HIGS_RASTER_SPLIT] per sub-unit
+    uint32_t* unit_order;      // [max_units * HIGS_RASTER_SPLIT] sub-units in the order the rasterizer claims them: batch index j major,
+                               //             within a level all first parts, then all second parts
     uint32_t* level_hist;      // [max_units+2] scratch of k_plan: macro-tiles per batch count, then level cursors
-    uint32_t* level_cur;       // [max_units+2]
+    uint32_t* level_cur;       // [3][max_units+2] level cursors, level bases, level sizes
     unsigned long long* pairs; // [max_pairs]
     unsigned long long* pairs_alt; // [max_pairs] ping-pong buffer of the overflow merge
     SortJob*  sort_jobs;       // [2][HIGS_N_TIERS][max_jobs]  list 0: whole segments, list 1: buckets
@@ -99,8 +100,8 @@ struct higs_ctx {
     uint32_t* bucket_cursor;   // [max_buckets]  write position of the scatter pass
     uint32_t* bucket_seg;      // [max_buckets]  index into split_segs
     int64_t   max_buckets;
-    float4*   partial;         // [max_units][32 tiles][64 px] (r,g,b,T)
-    float*    tile_maxT;       // [max_units][32] largest transmittance left in (unit, tile); 1 = unknown
+    float4*   partial;         // [max_units * HIGS_RASTER_SPLIT][32 tiles][64 px] (r,g,b,T)
+    float*    tile_maxT;       // [max_units * HIGS_RASTER_SPLIT][32] largest transmittance left in (sub-unit, tile); 0 = unknown
     FrameHeader* hdr;          // device
     FrameHeader* hdr_host;     // pinned
     // resident scene / host staging

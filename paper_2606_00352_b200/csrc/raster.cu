@@ -23,20 +23,23 @@
 
 namespace {
 
-constexpr int RAS_THREADS = 256;
+constexpr int RAS_THREADS = 256;                  // 3 CTAs per SM (80 registers, 71 KB shared memory each)
 constexpr int RAS_WARPS = RAS_THREADS / 32;
-constexpr int MASK_PITCH = 33;
+constexpr int RAS_SUB = HIGS_BATCH_CAP / HIGS_RASTER_SPLIT;   // gaussians per sub-unit: a unit is rasterized in parts
+constexpr int RAS_MB = RAS_SUB / 32;              // mini-batches of 32 gaussians per sub-unit
+constexpr int MASK_PITCH = RAS_MB + 1;
 constexpr int RING = 64;                          // per-warp index ring (u16), drained 8 at a time (B_d, 8x unroll)
-constexpr int NULL_IDX = HIGS_BATCH_CAP;          // index of the "null" gaussian that pads the last drain
+constexpr int NULL_IDX = RAS_SUB;                 // index of the "null" gaussian that pads the last drain
 
 // Shared-memory record of one staged gaussian, 64 B, laid out for packed f32x2 math: operands that multiply both
 // pixels of a lane sit duplicated in an aligned pair, so an LDS.128 lands them straight in an FFMA2 operand.
 //   f4[0] = mux, muy, A, B2      f4[1] = (C, C), (log2 o, log2 o)      f4[2] = (r, r), (g, g)      f4[3] = (b, b), tau, -
 struct __align__(16) RasSmem {
-    float4 rec[(HIGS_BATCH_CAP + 1) * 4];
+    float4 rec[(RAS_SUB + 1) * 4];
     uint32_t masks[HIGS_MT_TILES * MASK_PITCH];   // [tile][mini-batch]: bit j = gaussian k*32+j touches the tile
     uint16_t ring[RAS_WARPS][RING];
-    uint32_t unit, next_tile, active, cut;
+    uint32_t unit, next_tile, n_tiles, active, cut;
+    uint8_t order[HIGS_MT_TILES];                 // tile of the i-th tile claim: most gaussians first
 };
 
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
@@ -88,7 +91,7 @@ __device__ __forceinline__ uint32_t tile_mask_fast(float mux, float muy, float A
 }
 
 template <bool COUNT>
-__global__ void __launch_bounds__(RAS_THREADS, 3)
+__global__ void __launch_bounds__(RAS_THREADS, 768 / RAS_THREADS)
 k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict__ rec,
          const uint32_t* __restrict__ mt_offset, const uint32_t* __restrict__ mt_count,
          const uint32_t* __restrict__ batch_offset, const uint32_t* __restrict__ unit_mt,
@@ -100,7 +103,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
     RasSmem& S = *reinterpret_cast<RasSmem*>(s_raw);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const uint32_t lt_mask = (1u << lane) - 1u;
-    const uint32_t n_units = hdr->n_units;
+    const uint32_t n_sub = hdr->n_units * HIGS_RASTER_SPLIT;
     const bool use_cut = !(P.flags & HIGS_FLAG_NO_XBATCH_CUT);
     const float fW = (float)P.W, fH = (float)P.H;
     unsigned long long n_eval_g = 0, n_tp = 0;
@@ -114,18 +117,23 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
         __syncthreads();                                              // everyone is done with the previous unit's shared state
         if (threadIdx.x == 0) {
             const uint32_t c = atomicAdd(&hdr->raster_cursor, 1u);
-            S.unit = c < n_units ? unit_order[c] : 0xffffffffu;
+            S.unit = c < n_sub ? unit_order[c] : 0xffffffffu;
             S.next_tile = 0; S.active = 0; S.cut = 0;
         }
         __syncthreads();
-        const uint32_t u = S.unit;
-        if (u == 0xffffffffu) break;
+        const uint32_t v = S.unit;                                    // sub-unit: part h of unit u; outputs are indexed by v
+        if (v == 0xffffffffu) break;
+        const uint32_t u = v / HIGS_RASTER_SPLIT, h = v % HIGS_RASTER_SPLIT;
         const uint32_t m = unit_mt[u];
         const uint32_t u0 = batch_offset[m];
         const uint32_t j = u - u0;
         const uint32_t seg_n = mt_count[m];
-        const uint32_t start = mt_offset[m] + j * (uint32_t)P.batch_cap;
-        const int len = (int)min((uint32_t)P.batch_cap, seg_n - j * (uint32_t)P.batch_cap);
+        const uint32_t start = mt_offset[m] + j * (uint32_t)P.batch_cap + h * RAS_SUB;
+        const int len = min(RAS_SUB, (int)min((uint32_t)P.batch_cap, seg_n - j * (uint32_t)P.batch_cap) - (int)(h * RAS_SUB));
+        if (len <= 0) {                                               // the unit ends in an earlier part
+            if (threadIdx.x == 0) unit_active[v] = 0;
+            continue;
+        }
         const int mtx = (int)(m % (uint32_t)P.n_mx), mty = (int)(m / (uint32_t)P.n_mx);
         const float X0 = (float)(mtx * HIGS_MT_W), Y0 = (float)(mty * HIGS_MT_H);
 
@@ -146,9 +154,9 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             const int tiles_y = min(4, (P.H - mty * HIGS_MT_H + HIGS_TILE - 1) / HIGS_TILE);
             float bound = 1.0f;
             if (use_cut) {
-                for (uint32_t jj = 0; jj < j; ++jj) {
-                    const float v = __ldcg(tile_maxT + (size_t)(u0 + jj) * HIGS_MT_TILES + lane);
-                    bound *= (v > 0.0f ? v : 1.0f);                   // 0 = not published yet
+                for (uint32_t vv = u0 * HIGS_RASTER_SPLIT; vv < v; ++vv) {   // every earlier sub-unit of this macro-tile
+                    const float mt = __ldcg(tile_maxT + (size_t)vv * HIGS_MT_TILES + lane);
+                    bound *= (mt > 0.0f ? mt : 1.0f);                 // 0 = not published (yet, or an empty part)
                     if (__all_sync(0xffffffffu, bound < HIGS_EPS_T)) break;
                 }
             }
@@ -160,13 +168,13 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
         __syncthreads();
         const uint32_t cut = S.cut;
         if (cut == 0xffffffffu) {                                     // nothing left to see behind the earlier batches
-            if (threadIdx.x == 0) unit_active[u] = 0;
+            if (threadIdx.x == 0) unit_active[v] = 0;
             continue;
         }
 
         // ---- Phase 1b: per-gaussian tile masks (Alg. 1 lines 5-6), transposed by ballot; records re-laid for f32x2 ----
-        for (int k = w; k < HIGS_BATCH_CAP / 32; k += RAS_WARPS) {
-            const int i = k * 32 + lane;                              // == threadIdx.x + 256*(k/8): the slot this thread gathered
+        for (int k = w; k < RAS_MB; k += RAS_WARPS) {
+            const int i = k * 32 + lane;                              // == threadIdx.x + RAS_THREADS*(k/RAS_WARPS): the slot this thread gathered
             if (k * 32 >= len) { S.masks[lane * MASK_PITCH + k] = 0; continue; }
             uint32_t gm = 0;
             if (i < len) {
@@ -185,16 +193,32 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             S.masks[lane * MASK_PITCH + k] = mine;
         }
         __syncthreads();
+        // tiles are handed out most-gaussians-first (the longest tile bounds the unit's tail); tiles nobody touches get
+        // no claim at all.  lane = tile.
+        if (w == 0) {
+            uint32_t cnt = 0;
+#pragma unroll
+            for (int kk = 0; kk < RAS_MB; ++kk) cnt += __popc(S.masks[lane * MASK_PITCH + kk]);
+            const uint32_t key = (cnt << 5) | (uint32_t)(31 - lane);
+            uint32_t rank = 0;
+#pragma unroll
+            for (int o = 0; o < 32; ++o) rank += __shfl_sync(0xffffffffu, key, o) > key ? 1u : 0u;
+            if (cnt) S.order[rank] = (uint8_t)lane;
+            const uint32_t nt = __popc(__ballot_sync(0xffffffffu, cnt != 0u));
+            if (lane == 0) S.n_tiles = nt;
+        }
+        __syncthreads();
+        const int n_tiles = (int)S.n_tiles;
 
         // ---- Phase 2: warps claim render tiles (Alg. 1 lines 9-17), RasterizeTile (Alg. 2) ----
         for (;;) {
             int t = 0;
             if (lane == 0) t = (int)atomicAdd(&S.next_tile, 1u);
             t = __shfl_sync(0xffffffffu, t, 0);
-            if (t >= HIGS_MT_TILES) break;
-            const uint32_t mine = S.masks[t * MASK_PITCH + lane];      // lane k holds mini-batch k's word
+            if (t >= n_tiles) break;
+            t = (int)S.order[t];
+            const uint32_t mine = lane < RAS_MB ? S.masks[t * MASK_PITCH + lane] : 0u;   // lane k holds mini-batch k's word
             uint32_t rest = __ballot_sync(0xffffffffu, mine != 0u);
-            if (!rest) continue;
             const float pxf = X0 + (float)((t & 7) * HIGS_TILE + (lane & 7)) + 0.5f;
             const float py0 = Y0 + (float)((t >> 3) * HIGS_TILE + (lane >> 3)) + 0.5f;
             const float py1 = py0 + 4.0f;
@@ -252,19 +276,19 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             }
             __syncwarp();                                             // ring reads done before the next tile's writes
             if (COUNT) { n_tp += wr; n_eval_g += min(rd, wr); }
-            float4* out = partial + ((size_t)u * HIGS_MT_TILES + t) * 64;
+            float4* out = partial + ((size_t)v * HIGS_MT_TILES + t) * 64;
             __stcs(out + lane, make_float4(r2.x, g2.x, b2.x, T2.x));
             __stcs(out + 32 + lane, make_float4(r2.y, g2.y, b2.y, T2.y));
             float tm = fmaxf(T2.x, T2.y);
 #pragma unroll
             for (int d = 16; d > 0; d >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, d));
             if (lane == 0) {
-                __stcg(tile_maxT + (size_t)u * HIGS_MT_TILES + t, fmaxf(tm, 1e-30f));
+                __stcg(tile_maxT + (size_t)v * HIGS_MT_TILES + t, fmaxf(tm, 1e-30f));
                 atomicOr(&S.active, 1u << t);
             }
         }
         __syncthreads();
-        if (threadIdx.x == 0) unit_active[u] = S.active;
+        if (threadIdx.x == 0) unit_active[v] = S.active;
     }
     if (COUNT && lane == 0) {                                         // both counters are warp-uniform
         atomicAdd(&hdr->n_evals, n_eval_g * 64ull);
@@ -287,7 +311,7 @@ k_merge_image(const float4* __restrict__ partial, const uint32_t* __restrict__ u
     const int y0 = mty * HIGS_MT_H + (t >> 3) * HIGS_TILE + (lane >> 3);
     if (mtx * HIGS_MT_W + (t & 7) * HIGS_TILE >= P.W || mty * HIGS_MT_H + (t >> 3) * HIGS_TILE >= P.H) return;
     uint32_t u0 = 0, nb = 0;
-    if (!hdr->overflow) { u0 = batch_offset[m]; nb = batch_offset[m + 1] - u0; }
+    if (!hdr->overflow) { u0 = batch_offset[m] * HIGS_RASTER_SPLIT; nb = batch_offset[m + 1] * HIGS_RASTER_SPLIT - u0; }   // sub-units, in depth order
     float T0 = 1.0f, T1 = 1.0f, r0 = 0, g0 = 0, b0 = 0, r1 = 0, g1 = 0, b1 = 0;
     for (uint32_t j = 0; j < nb; ++j) {
         const uint32_t act = __ldg(unit_active + u0 + j);
