@@ -186,7 +186,7 @@ def workload_config(scene, args, world) -> dict:
     return {"workload": "configs[3]: large scene, paper scale (heavy-tailed planes/shells + 20% background + 10% hot region)",
             "n_gaussians": scene.N, "sh_degree": scene.degree, "image": "1920x1080", "fov_x_deg": 60,
             "views": f"orbit of {len(scene.cameras)} poses, step i -> view (i*{world}+rank) % {len(scene.cameras)}; view 0 = configs[3]'s pose",
-            "tiles": "8x8 px render tiles, 8x4 macro-tiles (64x32 px), B_r=1024, B_p=8192",
+            "tiles": "8x8 px render tiles, 8x4 macro-tiles (64x32 px), B_r=1024, partition batches = 2 persistent CTAs per SM over 512-id chunks",
             "l2": "inputs (1.37 GB) and per-frame records (0.46 GB) exceed the 126 MB L2; no flush between frames",
             "parallelism": f"replicas x{world} (views sharded, no collective)"}
 
@@ -276,19 +276,22 @@ def run_higs(args) -> int:
 
     # -- rooflines (algorithmic work per launch / mean CUDA-event duration of that stage) --
     K = (scene.degree + 1) ** 2
+    n_sm_early = torch.cuda.get_device_properties(local).multi_processor_count
     N, n_vis, n_pairs, n_units = scene.N, mean_of("n_visible"), mean_of("n_pairs"), mean_of("n_units")
-    n_b, n_m = (N + 8191) // 8192, 30 * 34
+    n_b, n_m = 2 * n_sm_early, 30 * 34                                   # partition CTAs = histogram rows (2 per SM), macro-tiles at 1080p
     hbm = peaks["hbm_gbs"]
     alg_bytes = {
-        "project": 44.0 * N + (12.0 * K + 80.0) * n_vis,
-        "count": N / 8.0 + 32.0 * n_vis + 2.0 * n_b * n_m,
-        "fill": N / 8.0 + 32.0 * n_vis + 4.0 * n_b * n_m + 8.0 * n_pairs,
+        "project": 44.0 * N + (12.0 * K + 80.0) * n_vis + 4.0 * n_b * n_m,           # inputs, SH rows, 64-B + 16-B records, histogram rows (count is folded in)
+        "fill": 16.0 * n_vis + 12.0 * n_b * n_m + 8.0 * n_pairs,                    # 16-B bin record per survivor, bases, pairs written
         "sort": 16.0 * n_pairs,
     }
+    # DRAM bytes per launch (read + write) from the committed ncu --set full capture of this workload
+    # (profiles/r01_final.md); measured once per round under the profiler, not in this run
+    NCU_TRAFFIC = {"project": 1.458e9, "fill": 1.16e8, "sort": 1.30e8, "raster": 5.76e8}
     def hbm_roof(stage, nbytes):
         ms = stage_ms[stage]
         ach = nbytes / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
-        return {"bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm, "traffic": None,
+        return {"bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm, "traffic": NCU_TRAFFIC.get(stage),
                 "peak_source": peaks["which"], "algorithmic_bytes": nbytes, "ms": ms}
     sm_hz = peaks["sm_max_mhz"] * 1e6
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
@@ -297,11 +300,11 @@ def run_higs(args) -> int:
     ras_ach = n_evals * RASTER_FP32_INST_PER_EVAL / (ras_ms * 1e-3) / 1e9 if ras_ms > 0 else 0.0
     roof = {k: hbm_roof(k, v) for k, v in alg_bytes.items()}
     roof["raster"] = {"bound": "alu", "achieved": ras_ach, "peak": alu_peak, "unit": "G FP32 thread-inst/s",
-                      "frac": ras_ach / alu_peak, "traffic": None, "peak_source": f"{n_sm} SMs x {FP32_LANES_PER_SM} lanes x {peaks['sm_max_mhz']:.0f} MHz",
+                      "frac": ras_ach / alu_peak, "traffic": NCU_TRAFFIC["raster"], "peak_source": f"{n_sm} SMs x {FP32_LANES_PER_SM} lanes x {peaks['sm_max_mhz']:.0f} MHz",
                       "evals_per_frame": n_evals, "tile_pairs_per_frame": n_tile_pairs,
                       "gevals_per_s": n_evals / (ras_ms * 1e-3) / 1e9 if ras_ms > 0 else 0.0,
                       "fp32_inst_per_eval": RASTER_FP32_INST_PER_EVAL, "ms": ras_ms}
-    dominant = max(("project", "count", "fill", "sort", "raster"), key=lambda k: stage_ms[k])
+    dominant = max(("project", "fill", "sort", "raster"), key=lambda k: stage_ms[k])
 
     # -- e2e: the same frames through higs_render_host (pinned host arrays in, host image out) --
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
