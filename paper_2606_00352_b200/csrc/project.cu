@@ -16,6 +16,9 @@
 #include <stdio.h>
 #include "higs_internal.cuh"
 
+#ifndef HIGS_LD
+#define HIGS_LD __ldg
+#endif
 namespace {
 
 // ln_spec (DESIGN.md N-LN): frexp + atanh series, separate mul and add, x in (1, 255].
@@ -52,12 +55,12 @@ __device__ __forceinline__ void sh_accumulate(const float* __restrict__ shp, flo
         const float4* p4 = reinterpret_cast<const float4*>(shp);
 #pragma unroll
         for (int k = 0; k < K * 3 / 4; ++k) {
-            float4 v = __ldcs(p4 + k);
+            float4 v = HIGS_LD(p4 + k);
             c[4 * k] = v.x; c[4 * k + 1] = v.y; c[4 * k + 2] = v.z; c[4 * k + 3] = v.w;
         }
     } else {
 #pragma unroll
-        for (int k = 0; k < K * 3; ++k) c[k] = __ldcs(shp + k);
+        for (int k = 0; k < K * 3; ++k) c[k] = HIGS_LD(shp + k);
     }
     float Y[K];
     Y[0] = 0.28209479177387814f;
@@ -117,10 +120,10 @@ __device__ __forceinline__ RawIn load_raw(const float* __restrict__ means, const
                                           const float* __restrict__ quats, const float* __restrict__ opac, int64_t i)
 {
     RawIn r;
-    r.mx = __ldcs(means + 3 * i); r.my = __ldcs(means + 3 * i + 1); r.mz = __ldcs(means + 3 * i + 2);
-    r.q = __ldcs(reinterpret_cast<const float4*>(quats) + i);
-    r.s0 = __ldcs(scales + 3 * i); r.s1 = __ldcs(scales + 3 * i + 1); r.s2 = __ldcs(scales + 3 * i + 2);
-    r.o = __ldcs(opac + i);
+    r.mx = HIGS_LD(means + 3 * i); r.my = HIGS_LD(means + 3 * i + 1); r.mz = HIGS_LD(means + 3 * i + 2);
+    r.q = HIGS_LD(reinterpret_cast<const float4*>(quats) + i);
+    r.s0 = HIGS_LD(scales + 3 * i); r.s1 = HIGS_LD(scales + 3 * i + 1); r.s2 = HIGS_LD(scales + 3 * i + 2);
+    r.o = HIGS_LD(opac + i);
     return r;
 }
 
