@@ -267,3 +267,51 @@ def test_cfg3_shaped_reduced_scene_lists_and_sampled_pixels(hg):
         ref = oracle.render(pr, window=win)
         assert np.abs(img[y0:y0 + 32, x0:x0 + 64] - ref).max() <= PIX_TOL
     r.close()
+
+
+def _full_size_check(hg, scene, cam, n_windows, seed):
+    """Full-size frame in the configuration bench.py times: lists and per-gaussian records bit-exact against the
+    oracle, pixels on sampled macro-tile windows (the oracle composites a window from the same global order)."""
+    r, img = _render(hg, scene, cam)
+    pr = oracle.project(scene, cam)
+    ols = oracle.bin_lists(pr)
+    st = r.stats()
+    assert st["overflow"] == 0 and st["n_visible"] == pr.n_vis
+    _check_records(r.records(), pr)
+    _check_lists(r.lists(), ols)
+    rng = np.random.default_rng(seed)
+    n_mx = (cam.W + 63) // 64
+    # half of the windows on the densest macro-tiles (oversize segments, many batches), half anywhere
+    dense = np.argsort(ols.mt_count)[::-1][:n_windows // 2]
+    anywhere = rng.integers(0, len(ols.mt_count), n_windows - len(dense))
+    worst = 0.0
+    for m in list(dense) + list(anywhere):
+        x0, y0 = int(m % n_mx) * 64, int(m // n_mx) * 32
+        x1, y1 = min(x0 + 64, cam.W), min(y0 + 32, cam.H)
+        ref = oracle.render(pr, window=(x0, y0, x1, y1))
+        worst = max(worst, float(np.abs(img[y0:y1, x0:x1] - ref).max()))
+    assert worst <= PIX_TOL, f"max abs pixel error {worst}"
+    # properties that hold at any size: finite, non-negative, every batch within B_r
+    assert np.isfinite(img).all() and img.min() >= 0.0
+    nb = np.diff(ols.batch_offset)
+    assert np.array_equal(nb, (ols.mt_count + 1023) // 1024)
+    r.close()
+
+
+def test_cfg3_full_size_5p8M_1080p(hg):
+    """BASELINE.json configs[3] as bench.py renders it: 5.8 M gaussians, SH degree 3, 1920x1080, orbit view 0."""
+    s = hs.scene_large(N=5_800_000, W=1920, H=1080)
+    _full_size_check(hg, s, s.cameras[0], n_windows=16, seed=3)
+
+
+def test_cfg4_full_size_5p8M_4k_view(hg):
+    """BASELINE.json configs[4]: the same scene at 3840x2160, one off-axis orbit view (elevation and radius differ from view 0)."""
+    s = hs.retarget(hs.scene_large(N=5_800_000, W=1920, H=1080), 3840, 2160)
+    _full_size_check(hg, s, s.cameras[5], n_windows=12, seed=4)
+
+
+def test_cfg2_full_size_1M_hotspots(hg):
+    """BASELINE.json configs[2]: 1 M gaussians with tight clusters, 1080p, two of the eight orbit poses."""
+    s = hs.scene_cfg2()
+    for v in (0, 3):
+        _full_size_check(hg, s, s.cameras[v], n_windows=8, seed=5 + v)
