@@ -76,7 +76,8 @@ int render_impl(higs_ctx* ctx, const float* means, const float* scales, const fl
     int rc;
 
     ctx->n_launches = 0;
-    HIGS_CUDA(ctx, cudaMemsetAsync(ctx->hdr, 0, sizeof(FrameHeader), st));
+    // one memset: frame header, per-macro-tile pair counts and fill cursors (one allocation)
+    HIGS_CUDA(ctx, cudaMemsetAsync(ctx->hdr, 0, sizeof(uint32_t) * (HIGS_HDR_WORDS + 2 * ((size_t)ctx->max_nm + 1)), st));
     if (!(ctx->flags & HIGS_FLAG_NO_XBATCH_CUT))
         HIGS_CUDA(ctx, cudaMemsetAsync(ctx->tile_maxT, 0, sizeof(float) * (size_t)ctx->max_units * HIGS_RASTER_SPLIT * HIGS_MT_TILES, st));
     if (timers) cudaEventRecord(ev[0], st);
@@ -175,7 +176,6 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     const int64_t n = max_gaussians > 0 ? max_gaussians : 1;
     ctx->n_chunks_max = (n + HIGS_CHUNK - 1) / HIGS_CHUNK;
     if ((rc = higs_project_smem_setup(ctx))) return fail(rc);       // also fixes n_part_max = n_sm x resident CTAs
-    const int n_groups_max = (ctx->n_part_max + 31) / 32;
     if ((rc = dev_alloc(ctx, &ctx->valid_bits, (size_t)(n + 31) / 32 + 1))) return fail(rc);
     const size_t n_slots = (size_t)ctx->n_chunks_max * HIGS_CHUNK;
     if ((rc = dev_alloc(ctx, &ctx->rec, n_slots * 4))) return fail(rc);
@@ -184,8 +184,11 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     if ((rc = dev_alloc(ctx, &ctx->part_list, (size_t)ctx->n_chunks_max))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->part_desc, (size_t)ctx->n_part_max))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->hist, (size_t)ctx->n_part_max * nm))) return fail(rc);
-    if ((rc = dev_alloc(ctx, &ctx->base, (size_t)(ctx->n_part_max + n_groups_max) * nm))) return fail(rc);
-    if ((rc = dev_alloc(ctx, &ctx->mt_count, (size_t)nm + 1))) return fail(rc);
+    static_assert(sizeof(FrameHeader) <= sizeof(uint32_t) * HIGS_HDR_WORDS, "frame header outgrew its block");
+    if ((rc = dev_alloc(ctx, &ctx->hdr_block, HIGS_HDR_WORDS + 2 * ((size_t)nm + 1)))) return fail(rc);
+    ctx->hdr = reinterpret_cast<FrameHeader*>(ctx->hdr_block);
+    ctx->mt_count = ctx->hdr_block + HIGS_HDR_WORDS;
+    ctx->mt_fill = ctx->mt_count + (nm + 1);
     if ((rc = dev_alloc(ctx, &ctx->mt_offset, (size_t)nm + 1))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->batch_offset, (size_t)nm + 1))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->pairs, (size_t)max_pairs))) return fail(rc);
@@ -201,9 +204,8 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     if ((rc = dev_alloc(ctx, &ctx->bucket_cursor, (size_t)ctx->max_buckets))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->bucket_seg, (size_t)ctx->max_buckets))) return fail(rc);
     if ((rc = alloc_unit_buffers(ctx))) return fail(rc);
-    if ((rc = dev_alloc(ctx, &ctx->hdr, 1))) return fail(rc);
     if (cudaMallocHost((void**)&ctx->hdr_host, sizeof(FrameHeader)) != cudaSuccess) return fail(HIGS_E_NOMEM);
-    if (cudaMemset(ctx->hdr, 0, sizeof(FrameHeader)) != cudaSuccess) return fail(HIGS_E_CUDA);
+    if (cudaMemset(ctx->hdr_block, 0, sizeof(uint32_t) * (HIGS_HDR_WORDS + 2 * ((size_t)nm + 1))) != cudaSuccess) return fail(HIGS_E_CUDA);
     memset(ctx->hdr_host, 0, sizeof(FrameHeader));
     if (cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking) != cudaSuccess) return fail(HIGS_E_CUDA);
     for (int i = 0; i < 9; ++i) if (cudaEventCreate(&ctx->ev[i]) != cudaSuccess) return fail(HIGS_E_CUDA);
@@ -226,11 +228,11 @@ void higs_destroy(higs_ctx* ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
-    dev_free(ctx->valid_bits); dev_free(ctx->rec); dev_free(ctx->bin); dev_free(ctx->chunk_count); dev_free(ctx->part_list); dev_free(ctx->part_desc); dev_free(ctx->rec_export); dev_free(ctx->hist); dev_free(ctx->base);
-    dev_free(ctx->mt_count); dev_free(ctx->mt_offset); dev_free(ctx->batch_offset); dev_free(ctx->unit_mt);
+    dev_free(ctx->valid_bits); dev_free(ctx->rec); dev_free(ctx->bin); dev_free(ctx->chunk_count); dev_free(ctx->part_list); dev_free(ctx->part_desc); dev_free(ctx->rec_export); dev_free(ctx->hist); dev_free(ctx->hdr_block);
+    dev_free(ctx->mt_offset); dev_free(ctx->batch_offset); dev_free(ctx->unit_mt);
     dev_free(ctx->unit_active); dev_free(ctx->pairs); dev_free(ctx->pairs_alt); dev_free(ctx->sort_jobs);
     dev_free(ctx->over_segs); dev_free(ctx->split_segs); dev_free(ctx->splitters); dev_free(ctx->bucket_count);
-    dev_free(ctx->bucket_cursor); dev_free(ctx->bucket_seg); dev_free(ctx->partial); dev_free(ctx->tile_maxT); dev_free(ctx->hdr);
+    dev_free(ctx->bucket_cursor); dev_free(ctx->bucket_seg); dev_free(ctx->partial); dev_free(ctx->tile_maxT);
     dev_free(ctx->unit_order); dev_free(ctx->level_hist); dev_free(ctx->level_cur);
     dev_free(ctx->s_means); dev_free(ctx->s_scales); dev_free(ctx->s_quats); dev_free(ctx->s_opac); dev_free(ctx->s_sh);
     dev_free(ctx->s_img);

@@ -11,31 +11,11 @@
 // (depth key << 32 | id) at base + local rank.
 #include <stdio.h>
 #include "higs_internal.cuh"
+#include "sort_plan.cuh"
 
 namespace {
 
 constexpr int BIN_THREADS = 1024;   // two CTAs per SM at 32 registers: the pass is latency-bound, so warps in flight decide
-constexpr int SCAN_GROUP  = 32;      // batches per first-level scan group
-
-// First scan level: CTA (column chunk, group) walks its <= 32 batches; base[b][m] = pairs of
-// macro-tile m in the earlier batches of the same group; gsum[g][m] = total of the group.
-__global__ void __launch_bounds__(256)
-k_scan_groups(const uint32_t* __restrict__ hist, int pitch, int n_batches, int n_m,
-              uint32_t* __restrict__ base, uint32_t* __restrict__ gsum)
-{
-    const int m = blockIdx.x * 256 + threadIdx.x;
-    const int g = blockIdx.y;
-    if (m >= n_m) return;
-    const int b0 = g * SCAN_GROUP, b1 = min(n_batches, b0 + SCAN_GROUP);
-    uint32_t run = 0;
-#pragma unroll 8
-    for (int b = b0; b < b1; ++b) {
-        const uint32_t h = hist[(size_t)b * pitch + m];
-        base[(size_t)b * n_m + m] = run;
-        run += h;
-    }
-    gsum[(size_t)g * n_m + m] = run;
-}
 
 // exclusive block scan of NV values per thread position (1024 threads), with a running carry
 template <int NV>
@@ -73,16 +53,18 @@ __device__ __forceinline__ void block_scan_excl(uint32_t (&v)[NV], uint32_t (&ca
     __syncthreads();
 }
 
-// Second scan level + batch schedule (a6), one CTA of 1024 threads:
-//   gbase[g][m] = exclusive scan of gsum over g; mt_count[m]; mt_offset = exclusive scan over m;
-//   nb[m] = ceil(n_m / B_r); batch_offset = exclusive scan; unit_mt[u] = m.
+// Scan (a3) + batch schedule (a6) + sort plan, one CTA of 1024 threads:
+//   mt_count[m] was accumulated by the projection CTAs (one atomicAdd per touched macro-tile per CTA);
+//   mt_offset = exclusive scan over m; nb[m] = ceil(n_m / B_r); batch_offset = exclusive scan; unit_mt[u] = m
+//   (PAPER.md:81); then the tier job lists of the segmented sort (sort_plan.cuh) and the order of the units.
 __global__ void __launch_bounds__(1024)
-k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, const FrameParams P,
-       uint32_t* __restrict__ mt_count, uint32_t* __restrict__ mt_offset, uint32_t* __restrict__ batch_offset,
+k_plan(const FrameParams P,
+       const uint32_t* __restrict__ mt_count, uint32_t* __restrict__ mt_offset, uint32_t* __restrict__ batch_offset,
        uint32_t* __restrict__ unit_mt, uint32_t* __restrict__ unit_order, uint32_t* __restrict__ level_hist,
-       uint32_t* __restrict__ level_cur, FrameHeader* __restrict__ hdr)
+       uint32_t* __restrict__ level_cur, SortJob* __restrict__ sort_jobs, size_t max_jobs, SplitSeg* __restrict__ split,
+       FrameHeader* __restrict__ hdr)
 {
-    __shared__ uint32_t s_warp[33 * 2];
+    __shared__ uint32_t s_warp[33 * 8];
     __shared__ uint32_t s_max;
     if (threadIdx.x == 0) s_max = 0;
     uint32_t carry[2] = {0, 0};
@@ -92,12 +74,7 @@ k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, con
         const int m = m0 + threadIdx.x;
         uint32_t n = 0;
         if (m < P.n_m) {
-            for (int g = 0; g < n_groups; ++g) {
-                const uint32_t s = gsum[(size_t)g * P.n_m + m];
-                gsum[(size_t)g * P.n_m + m] = n;
-                n += s;
-            }
-            mt_count[m] = n;
+            n = mt_count[m];
             if (n) atomicMax(&s_max, n);
         }
         uint32_t v[2] = { n, (n + br - 1) / br };
@@ -114,7 +91,10 @@ k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, con
         hdr->overflow = overflow ? 1u : 0u;
         hdr->max_segment = s_max;
     }
+    __syncthreads();                                              // mt_offset is complete (and visible to this CTA)
+    sort_plan_body(mt_offset, P.n_m, overflow, sort_jobs, max_jobs, split, hdr, s_warp);
     if (overflow) return;
+    __syncthreads();
     uint32_t* level_base = level_cur + (P.max_units + 2);
     uint32_t* level_cnt = level_base + (P.max_units + 2);
     // pass 2: unit table, and the order the rasterizer claims (sub-)units in: batch index j major ("level" j =
@@ -175,14 +155,14 @@ k_plan(uint32_t* __restrict__ gsum /* in: sums, out: bases */, int n_groups, con
 __global__ void __launch_bounds__(BIN_THREADS, 2)
 k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ part_list, const uint2* __restrict__ part_desc, int lcap,
        const uint4* __restrict__ bin, const float4* __restrict__ rec,
-       const FrameParams P, const uint32_t* __restrict__ base, const uint32_t* __restrict__ gbase, const uint32_t* __restrict__ mt_offset,
+       const FrameParams P, const uint32_t* __restrict__ hist, uint32_t* __restrict__ mt_fill, const uint32_t* __restrict__ mt_offset,
        unsigned long long* __restrict__ pairs, const FrameHeader* __restrict__ hdr)
 {
     extern __shared__ uint32_t s_cursor[];
     uint32_t* s_chunk = s_cursor + P.n_m;           // [lcap]
     uint32_t* s_pref = s_chunk + lcap;              // [lcap + 1] exclusive prefix of the chunk counts
     if (hdr->overflow) return;                      // capacity exceeded: write nothing (HIGS_E_CAPACITY)
-    const uint32_t b = blockIdx.x, g = b / SCAN_GROUP;
+    const uint32_t b = blockIdx.x;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const uint2 pd = part_desc[b];
     const uint32_t n_list = min(pd.y, (uint32_t)lcap);
@@ -200,8 +180,12 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
         }
         if (lane == 0) s_pref[n_list] = run;
     }
-    for (int m = threadIdx.x; m < P.n_m; m += BIN_THREADS)
-        s_cursor[m] = mt_offset[m] + gbase[(size_t)g * P.n_m + m] + base[(size_t)b * P.n_m + m];
+    // this batch's share of every macro-tile it touches: reserved with one atomic on the macro-tile's fill counter
+    // (which batch lands where inside a segment is arbitrary; the depth sort orders the segment anyway)
+    for (int m = threadIdx.x; m < P.n_m; m += BIN_THREADS) {
+        const uint32_t h = hist[(size_t)b * P.n_m + m];
+        s_cursor[m] = h ? mt_offset[m] + atomicAdd(&mt_fill[m], h) : 0u;
+    }
     __syncthreads();
     const uint32_t total = s_pref[n_list];
     auto slot_of = [&](uint32_t k) -> size_t {
@@ -276,7 +260,6 @@ __global__ void k_zero_lists(uint32_t* mt_count, uint32_t* mt_offset, uint32_t* 
 int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t st, cudaEvent_t ev_count, cudaEvent_t ev_scan)
 {
     const int n_b = N > 0 ? higs_part_grid(ctx, N) : 0;
-    const int pitch = P.n_m;
     if (n_b == 0) {
         k_zero_lists<<<(P.n_m + 256) / 256, 256, 0, st>>>(ctx->mt_count, ctx->mt_offset, ctx->batch_offset, P.n_m);
         HIGS_LAUNCHED(ctx);
@@ -286,15 +269,11 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, n_b);
     const size_t smem = sizeof(uint32_t) * ((size_t)P.n_m + 2 * (size_t)lcap + 1);
     if (ev_count) cudaEventRecord(ev_count, st);    // the count pass ran inside k_project: this stage is empty
-    const int n_groups = (n_b + SCAN_GROUP - 1) / SCAN_GROUP;
-    uint32_t* gsum = ctx->base + (size_t)ctx->n_part_max * ctx->max_nm;   // tail of the base allocation
-    k_scan_groups<<<dim3((P.n_m + 255) / 256, n_groups), 256, 0, st>>>(ctx->hist, pitch, n_b, P.n_m, ctx->base, gsum);
-    HIGS_LAUNCHED(ctx);
-    k_plan<<<1, 1024, 0, st>>>(gsum, n_groups, P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->unit_mt, ctx->unit_order,
-                               ctx->level_hist, ctx->level_cur, ctx->hdr);
+    k_plan<<<1, 1024, 0, st>>>(P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->unit_mt, ctx->unit_order,
+                               ctx->level_hist, ctx->level_cur, ctx->sort_jobs, (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr);
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
-    k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->chunk_count, ctx->part_list, ctx->part_desc, lcap, ctx->bin, ctx->rec, P, ctx->base, gsum, ctx->mt_offset, ctx->pairs, ctx->hdr);
+    k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->chunk_count, ctx->part_list, ctx->part_desc, lcap, ctx->bin, ctx->rec, P, ctx->hist, ctx->mt_fill, ctx->mt_offset, ctx->pairs, ctx->hdr);
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }

@@ -7,9 +7,12 @@
 
 #define HIGS_EPS_T      1e-4f        // transmittance threshold, reading Q1
 #define HIGS_ALPHA_MAX  0.99f
+#define HIGS_HDR_WORDS  64           // 32-bit words reserved for the FrameHeader at the head of its block
 #define HIGS_MAX_NM     32768        // macro-tiles per frame the shared-memory histograms are sized for
 #define HIGS_N_TIERS    4            // block-sort tiers, capacities 1024 / 2048 / 4096 / 8192
-#define HIGS_CHUNK      512          // consecutive ids projected by one warp; survivors are stored densely per chunk
+#ifndef HIGS_CHUNK
+#define HIGS_CHUNK      256          // consecutive ids projected by one warp; survivors are stored densely per chunk
+#endif
 #define HIGS_MERGE_TILE 4096         // output items per merge-path tile (overflow path)
 #define HIGS_SPLIT_TILE 4096         // items per CTA pass of the bucket count / scatter kernels
 #define HIGS_BUCKET_TARGET 1536      // mean items per depth bucket of an oversize segment
@@ -78,8 +81,9 @@ struct higs_ctx {
     uint2*    part_desc;       // [N_B]       (first entry, entries) of each partition CTA in part_list
     float*    rec_export;      // [maxN][16]  test-facing copy indexed by gaussian id, allocated by the first higs_get_records
     uint32_t* hist;            // [N_B][N_M]
-    uint32_t* base;            // [N_B][N_M] write base of (batch, macro-tile) relative to mt_offset[m]
-    uint32_t* mt_count;        // [max_nm]
+    uint32_t* hdr_block;       // one allocation, zeroed per frame: FrameHeader (HIGS_HDR_WORDS words) | mt_count | mt_fill
+    uint32_t* mt_count;        // [max_nm+1]  pairs per macro-tile, accumulated by the projection CTAs
+    uint32_t* mt_fill;         // [max_nm+1]  pairs of the macro-tile handed out so far (fill pass)
     uint32_t* mt_offset;       // [max_nm+1]
     uint32_t* batch_offset;    // [max_nm+1]
     uint32_t* unit_mt;         // [max_units] macro-tile of unit u

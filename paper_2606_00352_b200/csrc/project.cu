@@ -260,7 +260,7 @@ __global__ void __launch_bounds__(PROJ_THREADS, 2)
 k_project(const float* __restrict__ means, const float* __restrict__ scales, const float* __restrict__ quats,
           const float* __restrict__ opac, const float* __restrict__ sh, int64_t N, const FrameParams P,
           uint32_t* __restrict__ valid_bits, float4* __restrict__ rec, uint4* __restrict__ bin,
-          uint32_t* __restrict__ chunk_count, uint32_t* __restrict__ hist, uint32_t* __restrict__ part_list,
+          uint32_t* __restrict__ chunk_count, uint32_t* __restrict__ hist, uint32_t* __restrict__ mt_count, uint32_t* __restrict__ part_list,
           uint2* __restrict__ part_desc, int lcap, FrameHeader* __restrict__ hdr)
 {
     extern __shared__ uint32_t s_dyn[];
@@ -354,7 +354,11 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
         }
     }
     uint32_t* row = hist + (size_t)blockIdx.x * P.n_m;
-    for (int m = threadIdx.x; m < P.n_m; m += PROJ_THREADS) row[m] = s_hist[m];
+    for (int m = threadIdx.x; m < P.n_m; m += PROJ_THREADS) {
+        const uint32_t h = s_hist[m];
+        row[m] = h;
+        if (h) atomicAdd(&mt_count[m], h);                           // segment sizes accumulate here: no scan over the batches
+    }
     if (threadIdx.x == 0 && s_nvis) atomicAdd(&hdr->n_visible, s_nvis);
 }
 
@@ -389,7 +393,7 @@ int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, cons
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, (int)grid);
     const size_t smem = project_smem_bytes(P.n_m, lcap);
 #define HIGS_PROJ(D) k_project<D><<<grid, PROJ_THREADS, smem, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
-                                                                   ctx->bin, ctx->chunk_count, ctx->hist, ctx->part_list, ctx->part_desc, lcap, ctx->hdr)
+                                                                   ctx->bin, ctx->chunk_count, ctx->hist, ctx->mt_count, ctx->part_list, ctx->part_desc, lcap, ctx->hdr)
     switch (P.degree) {
         case 0: HIGS_PROJ(0); break;
         case 1: HIGS_PROJ(1); break;

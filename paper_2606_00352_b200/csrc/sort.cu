@@ -21,6 +21,7 @@
 #include <stdio.h>
 #include <cooperative_groups.h>
 #include "higs_internal.cuh"
+#include "sort_plan.cuh"
 
 namespace cg = cooperative_groups;
 typedef unsigned long long u64;
@@ -28,87 +29,13 @@ typedef unsigned long long u64;
 namespace {
 
 constexpr int IPT = 16;                                   // items per thread of the block sort
-__device__ __forceinline__ int tier_of(uint32_t n) { return n <= 1024u ? 0 : (n <= 2048u ? 1 : (n <= 4096u ? 2 : 3)); }
-
-// exclusive block scan (1024 threads) of NV values per thread position, with a running carry
-template <int NV>
-__device__ __forceinline__ void plan_scan(uint32_t (&v)[NV], uint32_t (&carry)[NV], uint32_t* s_warp /* [33*NV] */)
-{
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    uint32_t incl[NV];
-#pragma unroll
-    for (int q = 0; q < NV; ++q) {
-        uint32_t x = v[q];
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
-        incl[q] = x;
-        if (lane == 31) s_warp[wid * NV + q] = x;
-    }
-    __syncthreads();
-    if (wid == 0) {
-#pragma unroll
-        for (int q = 0; q < NV; ++q) {
-            const uint32_t x = s_warp[lane * NV + q];
-            uint32_t t = x;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, t, d); if (lane >= d) t += y; }
-            s_warp[lane * NV + q] = t - x;
-            if (lane == 31) s_warp[32 * NV + q] = t;
-        }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int q = 0; q < NV; ++q) {
-        const uint32_t excl = carry[q] + s_warp[wid * NV + q] + incl[q] - v[q];
-        carry[q] += s_warp[32 * NV + q];
-        v[q] = excl;
-    }
-    __syncthreads();
-}
-
-// ---- plan A: whole segments -> tier job lists (list 0); oversize segments -> split plan --------------
-__device__ __forceinline__ uint32_t buckets_of(uint32_t n)
-{
-    const uint32_t nb = (n + HIGS_BUCKET_TARGET - 1) / HIGS_BUCKET_TARGET;
-    return nb > HIGS_MAX_SPLIT ? HIGS_MAX_SPLIT : nb;
-}
 
 __global__ void __launch_bounds__(1024)
-k_sort_plan(const uint32_t* __restrict__ seg_offset, int n_seg, int honour_overflow, SortJob* __restrict__ jobs,
+k_sort_plan(const uint32_t* __restrict__ seg_offset, int n_seg, SortJob* __restrict__ jobs,
             size_t max_jobs, SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr)
 {
     __shared__ uint32_t s_warp[33 * 8];
-    const bool dead = honour_overflow && hdr->overflow;
-    uint32_t carry[8] = {0, 0, 0, 0, 0, 0, 0, 0};       // tiers 0-3, oversize segments, split tiles, buckets, oversize items
-    for (int s0 = 0; s0 < n_seg; s0 += 1024) {
-        const int s = s0 + threadIdx.x;
-        uint32_t start = 0, n = 0;
-        if (s < n_seg && !dead) { start = seg_offset[s]; n = seg_offset[s + 1] - start; }
-        uint32_t v[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        const bool over = n > HIGS_SORT_BLOCK;
-        const int t = n > 1 && !over ? tier_of(n) : -1;
-        uint32_t nb = 0;
-        if (t >= 0) v[t] = 1;
-        if (over) { nb = buckets_of(n); v[4] = 1; v[5] = (n + HIGS_SPLIT_TILE - 1) / HIGS_SPLIT_TILE; v[6] = nb; v[7] = n; }
-        plan_scan<8>(v, carry, s_warp);
-        if (t >= 0) jobs[(size_t)t * max_jobs + v[t]] = SortJob{start, n, 0u, 0u};
-        if (over) {
-            uint32_t a = 8192u / nb;                    // sample = a * nb <= 8192 items, sorted by one CTA
-            a = a > 16u ? 16u : a;                      // 16 sample items per bucket: bucket sizes within about +-25 % (1 sigma)
-            split[v[4]] = SplitSeg{start, n, nb, v[6], v[5], v[7], a, 0u};
-        }
-    }
-    if (threadIdx.x == 0) {
-        for (int t = 0; t < HIGS_N_TIERS; ++t) {
-            hdr->n_sort_jobs[0][t] = carry[t]; hdr->sort_cursor[0][t] = 0;
-            hdr->n_sort_jobs[1][t] = 0; hdr->sort_cursor[1][t] = 0;
-        }
-        hdr->n_oversize = carry[4];
-        hdr->n_split_tiles = carry[5];
-        hdr->n_buckets = carry[6];
-        hdr->n_fallback = 0; hdr->n_merge_tiles = 0; hdr->max_levels = 0;
-        hdr->split_cursor[0] = 0; hdr->split_cursor[1] = 0; hdr->split_cursor[2] = 0;
-    }
+    sort_plan_body(seg_offset, n_seg, false, jobs, max_jobs, split, hdr, s_warp);
 }
 
 // ---- block merge sort of up to THREADS*16 items held in shared memory ------------------------------
@@ -497,14 +424,16 @@ int setup_tier(higs_ctx* ctx, int tier)
     return HIGS_OK;
 }
 
-int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, int honour_overflow, cudaStream_t st)
+int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, bool plan_done, cudaStream_t st)
 {
     SortJob* jobs0 = ctx->sort_jobs;
     SortJob* jobs1 = ctx->sort_jobs + (size_t)HIGS_N_TIERS * ctx->max_jobs;
     u64* alt = ctx->pairs_alt;
     int rc;
-    k_sort_plan<<<1, 1024, 0, st>>>(seg_offset, n_seg, honour_overflow, jobs0, (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr);
-    HIGS_LAUNCHED(ctx);
+    if (!plan_done) {                                             // inside a frame k_plan has already done this (binning.cu)
+        k_sort_plan<<<1, 1024, 0, st>>>(seg_offset, n_seg, jobs0, (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr);
+        HIGS_LAUNCHED(ctx);
+    }
     // fork: whole segments go through the tier kernels on side streams (the paper overlaps tiers with PDL)
     // while the main stream splits the oversize segments into buckets
     HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_fork, st));
@@ -560,10 +489,10 @@ int higs_sort_smem_setup(higs_ctx* ctx)
 
 int launch_sort(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
 {
-    return run_sort(ctx, ctx->pairs, ctx->mt_offset, P.n_m, 1, st);
+    return run_sort(ctx, ctx->pairs, ctx->mt_offset, P.n_m, true, st);
 }
 
 int launch_sort_only(higs_ctx* ctx, unsigned long long* pairs, const uint32_t* seg_offset, int n_seg, cudaStream_t st)
 {
-    return run_sort(ctx, pairs, seg_offset, n_seg, 0, st);
+    return run_sort(ctx, pairs, seg_offset, n_seg, false, st);
 }
