@@ -64,6 +64,7 @@ k_plan(const FrameParams P,
        uint32_t* __restrict__ level_cur, SortJob* __restrict__ sort_jobs, size_t max_jobs, SplitSeg* __restrict__ split,
        FrameHeader* __restrict__ hdr)
 {
+    extern __shared__ uint32_t s_bo[];                            // [n_m + 1] copy of batch_offset for the unit -> macro-tile search
     __shared__ uint32_t s_warp[33 * 8];
     __shared__ uint32_t s_max;
     if (threadIdx.x == 0) s_max = 0;
@@ -79,13 +80,13 @@ k_plan(const FrameParams P,
         }
         uint32_t v[2] = { n, (n + br - 1) / br };
         block_scan_excl<2>(v, carry, s_warp);
-        if (m < P.n_m) { mt_offset[m] = v[0]; batch_offset[m] = v[1]; }
+        if (m < P.n_m) { mt_offset[m] = v[0]; batch_offset[m] = v[1]; s_bo[m] = v[1]; }
     }
     __syncthreads();
     const uint32_t n_pairs = carry[0], n_units = carry[1];
     const bool overflow = n_pairs > P.max_pairs || n_units > P.max_units;
     if (threadIdx.x == 0) {
-        mt_offset[P.n_m] = n_pairs; batch_offset[P.n_m] = n_units;
+        mt_offset[P.n_m] = n_pairs; batch_offset[P.n_m] = n_units; s_bo[P.n_m] = n_units;
         hdr->n_pairs = overflow ? 0u : n_pairs;
         hdr->n_units = overflow ? 0u : n_units;
         hdr->overflow = overflow ? 1u : 0u;
@@ -135,10 +136,10 @@ k_plan(const FrameParams P,
     __syncthreads();
     for (uint32_t u = threadIdx.x; u < n_units; u += 1024) {
         int lo = 0, hi = P.n_m - 1;                                       // last m with batch_offset[m] <= u and a batch there
-        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (batch_offset[mid] <= u) lo = mid; else hi = mid - 1; }
+        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_bo[mid] <= u) lo = mid; else hi = mid - 1; }
         unit_mt[u] = (uint32_t)lo;
         // sub-unit (u, h) = part h of unit u (HIGS_RASTER_SPLIT parts): level j's first parts, then its second parts, ...
-        const uint32_t lvl = u - batch_offset[lo];
+        const uint32_t lvl = u - s_bo[lo];
         const uint32_t p = atomicAdd(&level_cur[lvl], 1u) - level_base[lvl];
 #pragma unroll
         for (uint32_t h = 0; h < HIGS_RASTER_SPLIT; ++h)
@@ -269,7 +270,7 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, n_b);
     const size_t smem = sizeof(uint32_t) * ((size_t)P.n_m + 2 * (size_t)lcap + 1);
     if (ev_count) cudaEventRecord(ev_count, st);    // the count pass ran inside k_project: this stage is empty
-    k_plan<<<1, 1024, 0, st>>>(P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->unit_mt, ctx->unit_order,
+    k_plan<<<1, 1024, sizeof(uint32_t) * ((size_t)P.n_m + 1), st>>>(P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->unit_mt, ctx->unit_order,
                                ctx->level_hist, ctx->level_cur, ctx->sort_jobs, (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr);
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
@@ -301,5 +302,7 @@ int higs_binning_smem_setup(higs_ctx* ctx)
     if (bytes > 48 * 1024) {
         HIGS_CUDA(ctx, cudaFuncSetAttribute(k_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     }
+    const int plan_bytes = (int)(sizeof(uint32_t) * ((size_t)ctx->max_nm + 1));
+    if (plan_bytes > 40 * 1024) HIGS_CUDA(ctx, cudaFuncSetAttribute(k_plan, cudaFuncAttributeMaxDynamicSharedMemorySize, plan_bytes));
     return HIGS_OK;
 }
