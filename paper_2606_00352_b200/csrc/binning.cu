@@ -67,6 +67,7 @@ k_plan(const FrameParams P,
     extern __shared__ uint32_t s_bo[];                            // [n_m + 1] copy of batch_offset for the unit -> macro-tile search
     __shared__ uint32_t s_warp[33 * 8];
     __shared__ uint32_t s_max;
+    pdl_wait(); pdl_trigger();
     if (threadIdx.x == 0) s_max = 0;
     uint32_t carry[2] = {0, 0};
     const uint32_t br = (uint32_t)P.batch_cap;
@@ -162,6 +163,7 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
     extern __shared__ uint32_t s_cursor[];
     uint32_t* s_chunk = s_cursor + P.n_m;           // [lcap]
     uint32_t* s_pref = s_chunk + lcap;              // [lcap + 1] exclusive prefix of the chunk counts
+    pdl_wait(); pdl_trigger();
     if (hdr->overflow) return;                      // capacity exceeded: write nothing (HIGS_E_CAPACITY)
     const uint32_t b = blockIdx.x;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -270,11 +272,13 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, n_b);
     const size_t smem = sizeof(uint32_t) * ((size_t)P.n_m + 2 * (size_t)lcap + 1);
     if (ev_count) cudaEventRecord(ev_count, st);    // the count pass ran inside k_project: this stage is empty
-    k_plan<<<1, 1024, sizeof(uint32_t) * ((size_t)P.n_m + 1), st>>>(P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->unit_mt, ctx->unit_order,
-                               ctx->level_hist, ctx->level_cur, ctx->sort_jobs, (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr);
+    HIGS_CUDA(ctx, launch_pdl(k_plan, dim3(1), dim3(1024), sizeof(uint32_t) * ((size_t)P.n_m + 1), st, P, ctx->mt_count, ctx->mt_offset,
+                              ctx->batch_offset, ctx->unit_mt, ctx->unit_order, ctx->level_hist, ctx->level_cur, ctx->sort_jobs,
+                              (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr));
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
-    k_fill<<<n_b, BIN_THREADS, smem, st>>>(ctx->chunk_count, ctx->part_list, ctx->part_desc, lcap, ctx->bin, ctx->rec, P, ctx->hist, ctx->mt_fill, ctx->mt_offset, ctx->pairs, ctx->hdr);
+    HIGS_CUDA(ctx, launch_pdl(k_fill, dim3(n_b), dim3(BIN_THREADS), smem, st, ctx->chunk_count, ctx->part_list, ctx->part_desc, lcap, ctx->bin,
+                              ctx->rec, P, ctx->hist, ctx->mt_fill, ctx->mt_offset, ctx->pairs, ctx->hdr));
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }

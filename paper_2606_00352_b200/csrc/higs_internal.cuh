@@ -131,6 +131,24 @@ struct higs_ctx {
 // every kernel launch site of a frame calls this right after the <<<>>> (stats: n_launches)
 #define HIGS_LAUNCHED(ctx) do { HIGS_CUDA(ctx, cudaGetLastError()); ++(ctx)->n_launches; } while (0)
 
+// ---- programmatic dependent launch (PDL): a kernel launched with launch_pdl right behind another kernel on the same
+// stream may be scheduled while its predecessor drains; it must call pdl_wait() before touching anything the
+// predecessor wrote, and calls pdl_trigger() so that its own successor can be scheduled early in turn.
+__device__ __forceinline__ void pdl_wait()    { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KP, typename... A>
+inline cudaError_t launch_pdl(void (*kernel)(KP...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, A&&... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KP(args)...);
+}
+
 // ---- launch entry points, one per pipeline step (defined in the .cu files) ----------------------
 int launch_project(higs_ctx*, const FrameParams&, const float* means, const float* scales, const float* quats,
                    const float* opac, const float* sh, int64_t N, cudaStream_t);

@@ -267,6 +267,7 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
     __shared__ uint32_t s_nvis, s_nlist, s_lbase;
     uint32_t* s_hist = s_dyn;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    pdl_trigger();                                                   // k_plan may be scheduled as this grid drains
     float* q = reinterpret_cast<float*>(s_dyn + ((P.n_m + 3) & ~3)) + w * (PROJ_QF * PROJ_QCAP);
     uint32_t* s_list = s_dyn + ((P.n_m + 3) & ~3) + PROJ_WARPS * PROJ_QF * PROJ_QCAP;   // [lcap] chunks this CTA claimed
     for (int m = threadIdx.x; m < P.n_m; m += PROJ_THREADS) s_hist[m] = 0;

@@ -103,6 +103,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
     RasSmem& S = *reinterpret_cast<RasSmem*>(s_raw);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const uint32_t lt_mask = (1u << lane) - 1u;
+    pdl_trigger();                                                    // k_merge_image may be scheduled as this grid drains
     const uint32_t n_sub = hdr->n_units * HIGS_RASTER_SPLIT;
     const bool use_cut = !(P.flags & HIGS_FLAG_NO_XBATCH_CUT);
     const float fW = (float)P.W, fH = (float)P.H;
@@ -303,6 +304,7 @@ k_merge_image(const float4* __restrict__ partial, const uint32_t* __restrict__ u
               float* __restrict__ out_rgb)
 {
     const int lane = threadIdx.x & 31;
+    pdl_wait();
     const int gw = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const int m = gw >> 5, t = gw & 31;
     if (m >= P.n_m) return;
@@ -360,7 +362,8 @@ int launch_raster(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
 int launch_merge(higs_ctx* ctx, const FrameParams& P, float* out_rgb, cudaStream_t st)
 {
     const int warps = P.n_m * HIGS_MT_TILES;
-    k_merge_image<<<(warps + 7) / 8, 256, 0, st>>>(ctx->partial, ctx->unit_active, ctx->batch_offset, P, ctx->hdr, out_rgb);
+    HIGS_CUDA(ctx, launch_pdl(k_merge_image, dim3((warps + 7) / 8), dim3(256), 0, st, ctx->partial, ctx->unit_active, ctx->batch_offset, P,
+                              ctx->hdr, out_rgb));
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }

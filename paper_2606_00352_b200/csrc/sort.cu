@@ -157,6 +157,7 @@ k_over_split(const SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr, 
     u64* buf = reinterpret_cast<u64*>(s_raw);
     __shared__ uint32_t s_seg;
     const int t = threadIdx.x;
+    pdl_trigger();
     for (;;) {
         __syncthreads();
         if (t == 0) s_seg = atomicAdd(&hdr->split_cursor[0], 1u);
@@ -204,6 +205,7 @@ k_over_buckets(const SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr
     __shared__ uint32_t s_base[HIGS_MAX_SPLIT];
     __shared__ uint32_t s_tile;
     const int t = threadIdx.x;
+    pdl_wait(); pdl_trigger();
     const uint32_t n_over = hdr->n_oversize, n_tiles = hdr->n_split_tiles;
     for (;;) {
         __syncthreads();
@@ -263,6 +265,7 @@ k_bucket_plan(const SplitSeg* __restrict__ split, const uint32_t* __restrict__ b
 {
     __shared__ uint32_t s_warp[33 * 7];
     __shared__ uint32_t s_maxlev;
+    pdl_wait(); pdl_trigger();
     if (threadIdx.x == 0) s_maxlev = 0;
     __syncthreads();
     const uint32_t n_buckets = hdr->n_buckets;
@@ -445,14 +448,14 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, b
     k_over_split<<<ctx->n_sm, SPLIT_THREADS, sort_smem<SPLIT_THREADS>(), st>>>(ctx->split_segs, ctx->hdr, pairs, ctx->splitters,
                                                                               ctx->bucket_count, ctx->bucket_seg);
     HIGS_LAUNCHED(ctx);
-    k_over_buckets<false><<<ctx->n_sm * 2, SCAT_THREADS, 0, st>>>(ctx->split_segs, ctx->hdr, pairs, ctx->splitters, ctx->bucket_count,
-                                                                  ctx->bucket_cursor, alt);
+    HIGS_CUDA(ctx, launch_pdl(k_over_buckets<false>, dim3(ctx->n_sm * 2), dim3(SCAT_THREADS), 0, st, ctx->split_segs, ctx->hdr, pairs,
+                              ctx->splitters, ctx->bucket_count, ctx->bucket_cursor, alt));
     HIGS_LAUNCHED(ctx);
-    k_bucket_plan<<<1, 1024, 0, st>>>(ctx->split_segs, ctx->bucket_count, ctx->bucket_seg, ctx->bucket_cursor, jobs1, (size_t)ctx->max_jobs,
-                                      ctx->over_segs, ctx->hdr);
+    HIGS_CUDA(ctx, launch_pdl(k_bucket_plan, dim3(1), dim3(1024), 0, st, ctx->split_segs, ctx->bucket_count, ctx->bucket_seg, ctx->bucket_cursor,
+                              jobs1, (size_t)ctx->max_jobs, ctx->over_segs, ctx->hdr));
     HIGS_LAUNCHED(ctx);
-    k_over_buckets<true><<<ctx->n_sm * 2, SCAT_THREADS, 0, st>>>(ctx->split_segs, ctx->hdr, pairs, ctx->splitters, ctx->bucket_count,
-                                                                 ctx->bucket_cursor, alt);
+    HIGS_CUDA(ctx, launch_pdl(k_over_buckets<true>, dim3(ctx->n_sm * 2), dim3(SCAT_THREADS), 0, st, ctx->split_segs, ctx->hdr, pairs,
+                              ctx->splitters, ctx->bucket_count, ctx->bucket_cursor, alt));
     HIGS_LAUNCHED(ctx);
     HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_fork2, st));
     for (int k = 1; k < 4; ++k) HIGS_CUDA(ctx, cudaStreamWaitEvent(ctx->aux_stream[k], ctx->ev_fork2, 0));
