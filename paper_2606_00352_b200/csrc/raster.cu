@@ -23,12 +23,15 @@
 
 namespace {
 
-constexpr int RAS_THREADS = 256;                  // 3 CTAs per SM (80 registers, 71 KB shared memory each)
+#ifndef HIGS_RAS_THREADS
+#define HIGS_RAS_THREADS 256
+#endif
+constexpr int RAS_THREADS = HIGS_RAS_THREADS;     // 3 CTAs per SM (71 KB shared memory each)
 constexpr int RAS_WARPS = RAS_THREADS / 32;
 constexpr int RAS_SUB = HIGS_BATCH_CAP / HIGS_RASTER_SPLIT;   // gaussians per sub-unit: a unit is rasterized in parts
 constexpr int RAS_MB = RAS_SUB / 32;              // mini-batches of 32 gaussians per sub-unit
 constexpr int MASK_PITCH = RAS_MB + 1;
-constexpr int RING = 64;                          // per-warp index ring (u16), drained 8 at a time (B_d, 8x unroll)
+constexpr int RING = 64;                          // per-warp ring of staged-record addresses, drained 8 at a time (B_d, 8x unroll)
 constexpr int NULL_IDX = RAS_SUB;                 // index of the "null" gaussian that pads the last drain
 
 // Shared-memory record of one staged gaussian, 64 B, laid out for packed f32x2 math: operands that multiply both
@@ -37,7 +40,7 @@ constexpr int NULL_IDX = RAS_SUB;                 // index of the "null" gaussia
 struct __align__(16) RasSmem {
     float4 rec[(RAS_SUB + 1) * 4];
     uint32_t masks[HIGS_MT_TILES * MASK_PITCH];   // [tile][mini-batch]: bit j = gaussian k*32+j touches the tile
-    uint16_t ring[RAS_WARPS][RING];
+    uint32_t ring[RAS_WARPS][RING];              // shared-window byte addresses of the records: an entry is an LDS operand as it stands
     uint32_t unit, next_tile, n_tiles, active, cut;
     uint8_t order[HIGS_MT_TILES];                 // tile of the i-th tile claim: most gaussians first
 };
@@ -46,6 +49,12 @@ __device__ __forceinline__ void cp_async16(void* smem, const void* gmem)
 {
     const uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(s), "l"(gmem));
+}
+__device__ __forceinline__ float4 lds128(uint32_t saddr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(saddr));
+    return v;
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;\n" ::: "memory"); }
 __device__ __forceinline__ float ex2_approx(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
@@ -91,7 +100,7 @@ __device__ __forceinline__ uint32_t tile_mask_fast(float mux, float muy, float A
 }
 
 template <bool COUNT>
-__global__ void __launch_bounds__(RAS_THREADS, 768 / RAS_THREADS)
+__global__ void __launch_bounds__(RAS_THREADS, 3)
 k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict__ rec,
          const uint32_t* __restrict__ mt_offset, const uint32_t* __restrict__ mt_count,
          const uint32_t* __restrict__ batch_offset, const uint32_t* __restrict__ unit_mt,
@@ -112,7 +121,8 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
         S.rec[NULL_IDX * 4] = make_float4(0.f, 0.f, 0.f, 0.f); S.rec[NULL_IDX * 4 + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
         S.rec[NULL_IDX * 4 + 2] = make_float4(0.f, 0.f, 0.f, 0.f); S.rec[NULL_IDX * 4 + 3] = make_float4(0.f, 0.f, -1.0f, 0.f);
     }
-    uint16_t* ring = S.ring[w];
+    uint32_t* ring = S.ring[w];
+    const uint32_t rec_s = (uint32_t)__cvta_generic_to_shared(S.rec);
 
     for (;;) {
         __syncthreads();                                              // everyone is done with the previous unit's shared state
@@ -229,13 +239,12 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             bool sat = false;
             // one drain: 8 ring entries starting at rd (a multiple of 8), composited in order
             auto drain8 = [&]() {
-                const uint4 pk = *reinterpret_cast<const uint4*>(ring + (rd & (RING - 1)));
-                const uint32_t pkw[4] = { pk.x, pk.y, pk.z, pk.w };
+                const uint4 pk0 = *reinterpret_cast<const uint4*>(ring + (rd & (RING - 1)));
+                const uint4 pk1 = *reinterpret_cast<const uint4*>(ring + (rd & (RING - 1)) + 4);
+                const uint32_t pkw[8] = { pk0.x, pk0.y, pk0.z, pk0.w, pk1.x, pk1.y, pk1.z, pk1.w };
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    const uint32_t idx = (e & 1) ? (pkw[e >> 1] >> 16) : (pkw[e >> 1] & 0xffffu);
-                    const float4* gp = S.rec + 4 * idx;
-                    const float4 a = gp[0], bq = gp[1], cq = gp[2], dq = gp[3];
+                    const float4 a = lds128(pkw[e]), bq = lds128(pkw[e] + 16), cq = lds128(pkw[e] + 32), dq = lds128(pkw[e] + 48);
                     // N-Q, pinned: dx, u = A dx, a0 = u dx, b0 = B2 dx, t = fma(C, dy, b0), q = fma(t, dy, a0)
                     const float dx = __fsub_rn(pxf, a.x);
                     const float uu = __fmul_rn(a.z, dx);
@@ -261,7 +270,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
                 const int k = __ffs(rest) - 1;
                 rest &= rest - 1;
                 const uint32_t bits = __shfl_sync(0xffffffffu, mine, k);
-                if ((bits >> lane) & 1u) ring[(wr + __popc(bits & lt_mask)) & (RING - 1)] = (uint16_t)(k * 32 + lane);
+                if ((bits >> lane) & 1u) ring[(wr + __popc(bits & lt_mask)) & (RING - 1)] = rec_s + (uint32_t)(k * 32 + lane) * 64u;
                 wr += __popc(bits);
                 __syncwarp();
                 while (wr - rd >= 8u) {
@@ -271,7 +280,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
                 if (sat) break;
             }
             if (!sat && wr > rd) {                                    // flush: pad the last drain with the null gaussian
-                if (lane < 8) ring[(wr + lane) & (RING - 1)] = (uint16_t)NULL_IDX;
+                if (lane < 8) ring[(wr + lane) & (RING - 1)] = rec_s + (uint32_t)NULL_IDX * 64u;
                 __syncwarp();
                 drain8();
             }
