@@ -10,9 +10,7 @@
 #define HIGS_HDR_WORDS  64           // 32-bit words reserved for the FrameHeader at the head of its block
 #define HIGS_MAX_NM     32768        // macro-tiles per frame the shared-memory histograms are sized for
 #define HIGS_N_TIERS    4            // block-sort tiers, capacities 1024 / 2048 / 4096 / 8192
-#ifndef HIGS_CHUNK
 #define HIGS_CHUNK      256          // consecutive ids projected by one warp; survivors are stored densely per chunk
-#endif
 #define HIGS_MERGE_TILE 4096         // output items per merge-path tile (overflow path)
 #define HIGS_SPLIT_TILE 4096         // items per CTA pass of the bucket count / scatter kernels
 #define HIGS_BUCKET_TARGET 1536      // mean items per depth bucket of an oversize segment

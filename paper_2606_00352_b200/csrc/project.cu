@@ -16,9 +16,9 @@
 #include <stdio.h>
 #include "higs_internal.cuh"
 
-#ifndef HIGS_LD
+// inputs go through the read-only L1 path: consecutive loads of a warp share sectors (12-byte strides, halves of a
+// 32-byte sector of an SH row), and streaming / L1-bypassing loads were measured to re-fetch them from L2 and DRAM
 #define HIGS_LD __ldg
-#endif
 namespace {
 
 // ln_spec (DESIGN.md N-LN): frexp + atanh series, separate mul and add, x in (1, 255].
