@@ -23,7 +23,7 @@
 
 namespace {
 
-constexpr int RAS_THREADS = 256;                  // 3 CTAs per SM (80 registers, 72 KB shared memory each); 288-512 threads measured no faster
+constexpr int RAS_THREADS = 256;                  // 3 CTAs per SM at 80 registers (4 at 64 registers measured 2 % slower)
 constexpr int RAS_WARPS = RAS_THREADS / 32;
 constexpr int RAS_SUB = HIGS_BATCH_CAP / HIGS_RASTER_SPLIT;   // gaussians per sub-unit: a unit is rasterized in parts
 constexpr int RAS_MB = RAS_SUB / 32;              // mini-batches of 32 gaussians per sub-unit
@@ -31,11 +31,13 @@ constexpr int MASK_PITCH = RAS_MB + 1;
 constexpr int RING = 64;                          // per-warp ring of staged-record addresses, drained 8 at a time (B_d, 8x unroll)
 constexpr int NULL_IDX = RAS_SUB;                 // index of the "null" gaussian that pads the last drain
 
-// Shared-memory record of one staged gaussian, 64 B, laid out for packed f32x2 math: operands that multiply both
-// pixels of a lane sit duplicated in an aligned pair, so an LDS.128 lands them straight in an FFMA2 operand.
-//   f4[0] = mux, muy, A, B2      f4[1] = (C, C), (log2 o, log2 o)      f4[2] = (r, r), (g, g)      f4[3] = (b, b), tau, -
+// Shared-memory record of one staged gaussian: the first 48 B of its global record, as gathered:
+//   f4[0] = mux, muy, A, B2      f4[1] = C, tau, log2 o, r      f4[2] = g, b, -, -
+// Packed f32x2 instructions (FFMA2 / FMUL2 / FADD2) take a plain 32-bit register as a broadcast operand, so the values
+// that multiply both pixels of a lane need no duplicated copy in shared memory.
+constexpr int REC_F4 = 3;
 struct __align__(16) RasSmem {
-    float4 rec[(RAS_SUB + 1) * 4];
+    float4 rec[(RAS_SUB + 1) * REC_F4];
     uint32_t masks[HIGS_MT_TILES * MASK_PITCH];   // [tile][mini-batch]: bit j = gaussian k*32+j touches the tile
     uint32_t ring[RAS_WARPS][RING];              // shared-window byte addresses of the records: an entry is an LDS operand as it stands
     uint32_t unit, next_tile, n_tiles, active, cut;
@@ -115,8 +117,8 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
     const float fW = (float)P.W, fH = (float)P.H;
     unsigned long long n_eval_g = 0, n_tp = 0;
     if (threadIdx.x == 0) {                                           // the null gaussian: tau < 0, never passes q <= tau
-        S.rec[NULL_IDX * 4] = make_float4(0.f, 0.f, 0.f, 0.f); S.rec[NULL_IDX * 4 + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
-        S.rec[NULL_IDX * 4 + 2] = make_float4(0.f, 0.f, 0.f, 0.f); S.rec[NULL_IDX * 4 + 3] = make_float4(0.f, 0.f, -1.0f, 0.f);
+        S.rec[NULL_IDX * REC_F4] = make_float4(0.f, 0.f, 0.f, 0.f); S.rec[NULL_IDX * REC_F4 + 1] = make_float4(0.f, -1.0f, 0.f, 0.f);
+        S.rec[NULL_IDX * REC_F4 + 2] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     uint32_t* ring = S.ring[w];
     const uint32_t rec_s = (uint32_t)__cvta_generic_to_shared(S.rec);
@@ -149,9 +151,9 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
         for (int i = threadIdx.x; i < len; i += RAS_THREADS) {
             const uint32_t id = (uint32_t)pairs[start + i];
             const float4* src = rec + 4 * (size_t)id;
-            cp_async16(&S.rec[4 * i], src);
-            cp_async16(&S.rec[4 * i + 1], src + 1);
-            cp_async16(&S.rec[4 * i + 2], src + 2);
+            cp_async16(&S.rec[REC_F4 * i], src);
+            cp_async16(&S.rec[REC_F4 * i + 1], src + 1);
+            cp_async16(&S.rec[REC_F4 * i + 2], src + 2);
         }
 
         // tiles wholly outside the image are never active (Alg. 1 line 11, InBounds); cross-batch saturation
@@ -186,11 +188,8 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             if (k * 32 >= len) { S.masks[lane * MASK_PITCH + k] = 0; continue; }
             uint32_t gm = 0;
             if (i < len) {
-                const float4 a = S.rec[4 * i], b = S.rec[4 * i + 1], c = S.rec[4 * i + 2];
+                const float4 a = S.rec[REC_F4 * i], b = S.rec[REC_F4 * i + 1];
                 gm = tile_mask_fast(a.x, a.y, a.z, a.w, b.x, b.y, X0, Y0, fW, fH) & ~cut;
-                S.rec[4 * i + 1] = make_float4(b.x, b.x, b.z, b.z);
-                S.rec[4 * i + 2] = make_float4(b.w, b.w, c.x, c.x);
-                S.rec[4 * i + 3] = make_float4(c.y, c.y, b.y, 0.0f);
             }
             uint32_t mine = 0;
 #pragma unroll
@@ -230,6 +229,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             const float pxf = X0 + (float)((t & 7) * HIGS_TILE + (lane & 7)) + 0.5f;
             const float py0 = Y0 + (float)((t >> 3) * HIGS_TILE + (lane >> 3)) + 0.5f;
             const float py1 = py0 + 4.0f;
+            const float2 py2 = make_float2(py0, py1);
             float2 T2 = make_float2(1.0f, 1.0f), r2 = make_float2(0.f, 0.f), g2 = r2, b2 = r2;
             const float2 kexp = make_float2(-0.72134752f, -0.72134752f), neg1 = make_float2(-1.0f, -1.0f);
             uint32_t wr = 0, rd = 0;
@@ -241,24 +241,25 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
                 const uint32_t pkw[8] = { pk0.x, pk0.y, pk0.z, pk0.w, pk1.x, pk1.y, pk1.z, pk1.w };
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                    const float4 a = lds128(pkw[e]), bq = lds128(pkw[e] + 16), cq = lds128(pkw[e] + 32), dq = lds128(pkw[e] + 48);
+                    const float4 a = lds128(pkw[e]), bq = lds128(pkw[e] + 16), cq = lds128(pkw[e] + 32);
                     // N-Q, pinned: dx, u = A dx, a0 = u dx, b0 = B2 dx, t = fma(C, dy, b0), q = fma(t, dy, a0)
                     const float dx = __fsub_rn(pxf, a.x);
                     const float uu = __fmul_rn(a.z, dx);
                     const float a0 = __fmul_rn(uu, dx);
                     const float bb = __fmul_rn(a.w, dx);
-                    const float2 dy = make_float2(__fsub_rn(py0, a.y), __fsub_rn(py1, a.y));
-                    const float2 tq = __ffma2_rn(make_float2(bq.x, bq.y), dy, make_float2(bb, bb));
+                    const float nmy = -a.y;
+                    const float2 dy = __fadd2_rn(py2, make_float2(nmy, nmy));    // py - muy for both rows (same rounding as a subtraction)
+                    const float2 tq = __ffma2_rn(make_float2(bq.x, bq.x), dy, make_float2(bb, bb));
                     const float2 q = __ffma2_rn(tq, dy, make_float2(a0, a0));
-                    const float2 ex = __ffma2_rn(q, kexp, make_float2(bq.z, bq.w));
+                    const float2 ex = __ffma2_rn(q, kexp, make_float2(bq.z, bq.z));
                     float al0 = fminf(HIGS_ALPHA_MAX, ex2_approx(ex.x));
                     float al1 = fminf(HIGS_ALPHA_MAX, ex2_approx(ex.y));
-                    al0 = (q.x <= dq.z) ? al0 : 0.0f;                 // alpha < 1/255: skipped
-                    al1 = (q.y <= dq.z) ? al1 : 0.0f;
+                    al0 = (q.x <= bq.y) ? al0 : 0.0f;                 // alpha < 1/255: skipped
+                    al1 = (q.y <= bq.y) ? al1 : 0.0f;
                     const float2 wgt = __fmul2_rn(T2, make_float2(al0, al1));
-                    r2 = __ffma2_rn(wgt, make_float2(cq.x, cq.y), r2);
-                    g2 = __ffma2_rn(wgt, make_float2(cq.z, cq.w), g2);
-                    b2 = __ffma2_rn(wgt, make_float2(dq.x, dq.y), b2);
+                    r2 = __ffma2_rn(wgt, make_float2(bq.w, bq.w), r2);
+                    g2 = __ffma2_rn(wgt, make_float2(cq.x, cq.x), g2);
+                    b2 = __ffma2_rn(wgt, make_float2(cq.y, cq.y), b2);
                     T2 = __ffma2_rn(wgt, neg1, T2);
                 }
                 rd += 8;
@@ -267,7 +268,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
                 const int k = __ffs(rest) - 1;
                 rest &= rest - 1;
                 const uint32_t bits = __shfl_sync(0xffffffffu, mine, k);
-                if ((bits >> lane) & 1u) ring[(wr + __popc(bits & lt_mask)) & (RING - 1)] = rec_s + (uint32_t)(k * 32 + lane) * 64u;
+                if ((bits >> lane) & 1u) ring[(wr + __popc(bits & lt_mask)) & (RING - 1)] = rec_s + (uint32_t)(k * 32 + lane) * (REC_F4 * 16u);
                 wr += __popc(bits);
                 __syncwarp();
                 while (wr - rd >= 8u) {
@@ -277,7 +278,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
                 if (sat) break;
             }
             if (!sat && wr > rd) {                                    // flush: pad the last drain with the null gaussian
-                if (lane < 8) ring[(wr + lane) & (RING - 1)] = rec_s + (uint32_t)NULL_IDX * 64u;
+                if (lane < 8) ring[(wr + lane) & (RING - 1)] = rec_s + (uint32_t)NULL_IDX * (REC_F4 * 16u);
                 __syncwarp();
                 drain8();
             }
