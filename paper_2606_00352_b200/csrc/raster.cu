@@ -9,7 +9,7 @@
 // word per (tile, mini-batch) says which gaussians touch the tile.  Phase 2 (Alg. 1 lines 9-17,
 // Alg. 2): warps claim render tiles from a shared counter; a warp owns the 8x8 tile (two pixels per
 // lane, rows y and y+4 of one column, so the dx terms are shared), walks the tile's mask words,
-// reads each listed gaussian as three broadcast LDS.128 and composites front to back; after every
+// reads each listed gaussian as three broadcast LDS.128 (48 B, as gathered) and composites front to back; after every
 // mask word a unanimous vote on T < eps ends the tile early (Alg. 2 line 8).  Partial (r,g,b,T) per
 // pixel goes to the dense (unit, tile) buffer, the unit's 32-bit active mask out of band
 // (PAPER.md:284).  The merge kernel gives one warp per render tile and folds the macro-tile's units
@@ -244,9 +244,9 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
                     const float4 a = lds128(pkw[e]), bq = lds128(pkw[e] + 16), cq = lds128(pkw[e] + 32);
                     // N-Q, pinned: dx, u = A dx, a0 = u dx, b0 = B2 dx, t = fma(C, dy, b0), q = fma(t, dy, a0)
                     const float dx = __fsub_rn(pxf, a.x);
-                    const float uu = __fmul_rn(a.z, dx);
-                    const float a0 = __fmul_rn(uu, dx);
-                    const float bb = __fmul_rn(a.w, dx);
+                    const float2 ub = __fmul2_rn(make_float2(a.z, a.w), make_float2(dx, dx));   // u = A dx and b0 = B2 dx in one packed multiply
+                    const float a0 = __fmul_rn(ub.x, dx);
+                    const float bb = ub.y;
                     const float nmy = -a.y;
                     const float2 dy = __fadd2_rn(py2, make_float2(nmy, nmy));    // py - muy for both rows (same rounding as a subtraction)
                     const float2 tq = __ffma2_rn(make_float2(bq.x, bq.x), dy, make_float2(bb, bb));
