@@ -103,7 +103,8 @@ struct higs_ctx {
     uint32_t* bucket_seg;      // [max_buckets]  index into split_segs
     int64_t   max_buckets;
     float4*   partial;         // [max_units * HIGS_RASTER_SPLIT][32 tiles][64 px] (r,g,b,T)
-    float*    tile_maxT;       // [max_units * HIGS_RASTER_SPLIT][32] largest transmittance left in (sub-unit, tile); 0 = unknown
+    int*      tile_logT;       // [max_nm][32] running sum over the finished units of a macro-tile of log2(largest transmittance left in the
+                               //             tile) x 1024, each term rounded towards zero: an upper bound of the transmittance in front of later units
     FrameHeader* hdr;          // device
     FrameHeader* hdr_host;     // pinned
     // resident scene / host staging

@@ -28,6 +28,8 @@ constexpr int RAS_WARPS = RAS_THREADS / 32;
 constexpr int RAS_SUB = HIGS_BATCH_CAP / HIGS_RASTER_SPLIT;   // gaussians per sub-unit: a unit is rasterized in parts
 constexpr int RAS_MB = RAS_SUB / 32;              // mini-batches of 32 gaussians per sub-unit
 constexpr int MASK_PITCH = RAS_MB + 1;
+constexpr float LOGT_SCALE = 1024.0f;             // fixed point of the running log2 transmittance bounds
+constexpr int LOGT_EPS = -13608;                  // floor(log2(1e-4) * 1024): a sum below it proves T < eps
 constexpr int RING = 64;                          // per-warp ring of staged-record addresses, drained 8 at a time (B_d, 8x unroll)
 constexpr int NULL_IDX = RAS_SUB;                 // index of the "null" gaussian that pads the last drain
 
@@ -105,7 +107,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
          const uint32_t* __restrict__ batch_offset, const uint32_t* __restrict__ unit_mt,
          const uint32_t* __restrict__ unit_order,
          const FrameParams P, FrameHeader* __restrict__ hdr,
-         float4* __restrict__ partial, uint32_t* __restrict__ unit_active, float* __restrict__ tile_maxT)
+         float4* __restrict__ partial, uint32_t* __restrict__ unit_active, int* __restrict__ tile_logT)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
     RasSmem& S = *reinterpret_cast<RasSmem*>(s_raw);
@@ -158,20 +160,17 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
 
         // tiles wholly outside the image are never active (Alg. 1 line 11, InBounds); cross-batch saturation
         // cut-off: the product over the earlier units of this macro-tile of the largest transmittance they left
-        // in tile t bounds the transmittance in front of this unit
+        // in tile t bounds the transmittance in front of this unit.  The product is kept as a
+        // running sum of fixed-point log2 values per (macro-tile, tile), each rounded towards zero, so the sum never
+        // understates the bound; units are claimed batch index major, so whatever has been added when this unit
+        // looks comes from batches in front of it.
         if (w == 0) {
             const int tiles_x = min(8, (P.W - mtx * HIGS_MT_W + HIGS_TILE - 1) / HIGS_TILE);
             const int tiles_y = min(4, (P.H - mty * HIGS_MT_H + HIGS_TILE - 1) / HIGS_TILE);
-            float bound = 1.0f;
-            if (use_cut) {
-                for (uint32_t vv = u0 * HIGS_RASTER_SPLIT; vv < v; ++vv) {   // every earlier sub-unit of this macro-tile
-                    const float mt = __ldcg(tile_maxT + (size_t)vv * HIGS_MT_TILES + lane);
-                    bound *= (mt > 0.0f ? mt : 1.0f);                 // 0 = not published (yet, or an empty part)
-                    if (__all_sync(0xffffffffu, bound < HIGS_EPS_T)) break;
-                }
-            }
+            bool saturated = false;
+            if (use_cut && v > u0 * HIGS_RASTER_SPLIT) saturated = __ldcg(tile_logT + (size_t)m * HIGS_MT_TILES + lane) < LOGT_EPS;
             const bool inb = (lane & 7) < tiles_x && (lane >> 3) < tiles_y;
-            const uint32_t cut = __ballot_sync(0xffffffffu, bound < HIGS_EPS_T || !inb);
+            const uint32_t cut = __ballot_sync(0xffffffffu, saturated || !inb);
             if (lane == 0) S.cut = cut;
         }
         cp_async_wait_all();                                          // each thread waits for the records it asked for
@@ -291,7 +290,10 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
 #pragma unroll
             for (int d = 16; d > 0; d >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, d));
             if (lane == 0) {
-                __stcg(tile_maxT + (size_t)v * HIGS_MT_TILES + t, fmaxf(tm, 1e-30f));
+                if (use_cut) {                                        // log2 of the largest transmittance left, rounded towards zero
+                    const int q = min(0, (int)ceilf(__log2f(fmaxf(tm, 1e-30f)) * LOGT_SCALE) + 2);
+                    if (q) atomicAdd(tile_logT + (size_t)m * HIGS_MT_TILES + t, q);
+                }
                 atomicOr(&S.active, 1u << t);
             }
         }
@@ -358,10 +360,10 @@ int launch_raster(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
     const int grid = ctx->n_sm * g_raster_ctas_per_sm;
     if (P.flags & HIGS_FLAG_COUNT_EVALS)
         k_raster<true><<<grid, RAS_THREADS, smem, st>>>(ctx->pairs, ctx->rec, ctx->mt_offset, ctx->mt_count, ctx->batch_offset,
-                                                        ctx->unit_mt, ctx->unit_order, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_maxT);
+                                                        ctx->unit_mt, ctx->unit_order, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_logT);
     else
         k_raster<false><<<grid, RAS_THREADS, smem, st>>>(ctx->pairs, ctx->rec, ctx->mt_offset, ctx->mt_count, ctx->batch_offset,
-                                                         ctx->unit_mt, ctx->unit_order, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_maxT);
+                                                         ctx->unit_mt, ctx->unit_order, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_logT);
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }
