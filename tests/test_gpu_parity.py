@@ -347,3 +347,20 @@ def test_frame_captures_into_a_cuda_graph(hg):
     assert np.abs(img.cpu().numpy() - oracle.render(pr)).max() <= PIX_TOL
     del g
     hg.higs_destroy(ctx)
+
+
+def test_8k_image_16200_macro_tiles(hg):
+    """A 7680x4320 frame: 16,200 macro-tiles, so the per-CTA histograms (65 KB) and the plan's shared tables leave their
+    default shared-memory budget; most gaussians span several macro-tiles.  Lists bit-exact, a 1600x800 window of pixels."""
+    s = hs.retarget(hs.scene_cfg1(N=50_000), 7680, 4320)
+    cam = s.cameras[0]
+    r, img = _render(hg, s, cam, max_pairs=6_000_000)
+    st = r.stats()
+    assert st["overflow"] == 0
+    pr = oracle.project(s, cam)
+    ols = oracle.bin_lists(pr)
+    assert st["n_visible"] == pr.n_vis
+    _check_lists(r.lists(), ols)
+    ref = oracle.render(pr, window=(3000, 1800, 4600, 2600))
+    assert np.abs(img[1800:2600, 3000:4600] - ref).max() <= PIX_TOL
+    r.close()
