@@ -127,14 +127,48 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
 
     for (;;) {
         __syncthreads();                                              // everyone is done with the previous unit's shared state
-        if (threadIdx.x == 0) {
-            const uint32_t c = atomicAdd(&hdr->raster_cursor, 1u);
-            S.unit = c < n_sub ? unit_order[c] : 0xffffffffu;
-            S.next_tile = 0; S.active = 0; S.cut = 0;
+        // Warp 0 claims units until one has something left to show.  Tiles wholly outside the image are never active
+        // (Alg. 1 line 11, InBounds).  Cross-batch saturation cut-off: the product over the earlier units of this
+        // macro-tile of the largest transmittance they left in tile t (lane = tile) bounds the transmittance in front of
+        // this unit.  The product is kept as a running sum of fixed-point log2 values per
+        // (macro-tile, tile), each rounded towards zero, so the sum never understates the bound; units are claimed batch
+        // index major, so whatever has been added when this unit looks comes from batches in front of it.  A unit with
+        // every tile cut costs one atomic and four loads: it is never gathered.
+        if (w == 0) {
+            uint32_t v_sel = 0xffffffffu, cut_sel = 0;
+            for (;;) {
+                uint32_t c = 0;
+                if (lane == 0) c = atomicAdd(&hdr->raster_cursor, 1u);
+                c = __shfl_sync(0xffffffffu, c, 0);
+                if (c >= n_sub) break;
+                const uint32_t vc = unit_order[c];
+                const uint32_t uc = vc / HIGS_RASTER_SPLIT, hc = vc % HIGS_RASTER_SPLIT;
+                const uint32_t mc = unit_mt[uc];
+                const uint32_t u0c = batch_offset[mc];
+                const int lenc = min(RAS_SUB, (int)min((uint32_t)P.batch_cap, mt_count[mc] - (uc - u0c) * (uint32_t)P.batch_cap) - (int)(hc * RAS_SUB));
+                uint32_t cut = 0xffffffffu;
+                if (lenc > 0) {                                       // else: the unit ends in an earlier part
+                    const int mtx = (int)(mc % (uint32_t)P.n_mx), mty = (int)(mc / (uint32_t)P.n_mx);
+                    const int tiles_x = min(8, (P.W - mtx * HIGS_MT_W + HIGS_TILE - 1) / HIGS_TILE);
+                    const int tiles_y = min(4, (P.H - mty * HIGS_MT_H + HIGS_TILE - 1) / HIGS_TILE);
+                    bool saturated = false;
+                    if (use_cut && vc > u0c * HIGS_RASTER_SPLIT) saturated = __ldcg(tile_logT + (size_t)mc * HIGS_MT_TILES + lane) < LOGT_EPS;
+                    const bool inb = (lane & 7) < tiles_x && (lane >> 3) < tiles_y;
+                    cut = __ballot_sync(0xffffffffu, saturated || !inb);
+                }
+                if (cut == 0xffffffffu) {                             // nothing left to see behind the earlier batches
+                    if (lane == 0) unit_active[vc] = 0;
+                    continue;
+                }
+                v_sel = vc; cut_sel = cut;
+                break;
+            }
+            if (lane == 0) { S.unit = v_sel; S.cut = cut_sel; S.next_tile = 0; S.active = 0; }
         }
         __syncthreads();
         const uint32_t v = S.unit;                                    // sub-unit: part h of unit u; outputs are indexed by v
         if (v == 0xffffffffu) break;
+        const uint32_t cut = S.cut;
         const uint32_t u = v / HIGS_RASTER_SPLIT, h = v % HIGS_RASTER_SPLIT;
         const uint32_t m = unit_mt[u];
         const uint32_t u0 = batch_offset[m];
@@ -142,14 +176,10 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
         const uint32_t seg_n = mt_count[m];
         const uint32_t start = mt_offset[m] + j * (uint32_t)P.batch_cap + h * RAS_SUB;
         const int len = min(RAS_SUB, (int)min((uint32_t)P.batch_cap, seg_n - j * (uint32_t)P.batch_cap) - (int)(h * RAS_SUB));
-        if (len <= 0) {                                               // the unit ends in an earlier part
-            if (threadIdx.x == 0) unit_active[v] = 0;
-            continue;
-        }
         const int mtx = (int)(m % (uint32_t)P.n_mx), mty = (int)(m / (uint32_t)P.n_mx);
         const float X0 = (float)(mtx * HIGS_MT_W), Y0 = (float)(mty * HIGS_MT_H);
 
-        // ---- Phase 1a: start the gather of this unit's records (Alg. 1 line 4), first 48 B of each, by sorted id ----
+        // ---- Phase 1a: gather of this unit's records (Alg. 1 line 4), first 48 B of each, by sorted id ----
         for (int i = threadIdx.x; i < len; i += RAS_THREADS) {
             const uint32_t id = (uint32_t)pairs[start + i];
             const float4* src = rec + 4 * (size_t)id;
@@ -157,29 +187,8 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             cp_async16(&S.rec[REC_F4 * i + 1], src + 1);
             cp_async16(&S.rec[REC_F4 * i + 2], src + 2);
         }
-
-        // tiles wholly outside the image are never active (Alg. 1 line 11, InBounds); cross-batch saturation
-        // cut-off: the product over the earlier units of this macro-tile of the largest transmittance they left
-        // in tile t bounds the transmittance in front of this unit.  The product is kept as a
-        // running sum of fixed-point log2 values per (macro-tile, tile), each rounded towards zero, so the sum never
-        // understates the bound; units are claimed batch index major, so whatever has been added when this unit
-        // looks comes from batches in front of it.
-        if (w == 0) {
-            const int tiles_x = min(8, (P.W - mtx * HIGS_MT_W + HIGS_TILE - 1) / HIGS_TILE);
-            const int tiles_y = min(4, (P.H - mty * HIGS_MT_H + HIGS_TILE - 1) / HIGS_TILE);
-            bool saturated = false;
-            if (use_cut && v > u0 * HIGS_RASTER_SPLIT) saturated = __ldcg(tile_logT + (size_t)m * HIGS_MT_TILES + lane) < LOGT_EPS;
-            const bool inb = (lane & 7) < tiles_x && (lane >> 3) < tiles_y;
-            const uint32_t cut = __ballot_sync(0xffffffffu, saturated || !inb);
-            if (lane == 0) S.cut = cut;
-        }
         cp_async_wait_all();                                          // each thread waits for the records it asked for
         __syncthreads();
-        const uint32_t cut = S.cut;
-        if (cut == 0xffffffffu) {                                     // nothing left to see behind the earlier batches
-            if (threadIdx.x == 0) unit_active[v] = 0;
-            continue;
-        }
 
         // ---- Phase 1b: per-gaussian tile masks (Alg. 1 lines 5-6), transposed by ballot; records re-laid for f32x2 ----
         for (int k = w; k < RAS_MB; k += RAS_WARPS) {
