@@ -186,7 +186,7 @@ def workload_config(scene, args, world) -> dict:
     return {"workload": "configs[3]: large scene, paper scale (heavy-tailed planes/shells + 20% background + 10% hot region)",
             "n_gaussians": scene.N, "sh_degree": scene.degree, "image": "1920x1080", "fov_x_deg": 60,
             "views": f"orbit of {len(scene.cameras)} poses, step i -> view (i*{world}+rank) % {len(scene.cameras)}; view 0 = configs[3]'s pose",
-            "tiles": "8x8 px render tiles, 8x4 macro-tiles (64x32 px), B_r=1024, partition batches = 2 persistent CTAs per SM over 512-id chunks",
+            "tiles": f"8x8 px render tiles, 8x4 macro-tiles (64x32 px), B_r={args.batch_cap}, partition batches = 2 persistent CTAs per SM over 512-id chunks",
             "l2": "inputs (1.37 GB) and per-frame records (0.46 GB) exceed the 126 MB L2; no flush between frames",
             "parallelism": f"replicas x{world} (views sharded, no collective)"}
 
@@ -212,6 +212,8 @@ def run_higs(args) -> int:
     dev = hg.scene_to_device(scene, f"cuda:{local}")
     max_w, max_h = (3840, 2160) if not args.no_4k else (1920, 1080)
     ctx = hg.higs_create(local, scene.N, max_w, max_h, 0)
+    if args.batch_cap != 1024:
+        hg.higs_set_batch_cap(ctx, args.batch_cap)
     ccams_1080 = [hg.make_camera(c) for c in cams_1080]
     ccams_4k = [hg.make_camera(c) for c in cams_4k]
     img = torch.empty((1080, 1920, 3), dtype=torch.float32, device=f"cuda:{local}")
@@ -408,6 +410,7 @@ def main() -> int:
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="higs", choices=["higs", "reference"])
     ap.add_argument("--n", type=int, default=N_PAPER, help="gaussians in the scene (default: the paper-scale 5.8 M)")
+    ap.add_argument("--batch-cap", type=int, default=1024, help="B_r, gaussians per rasterizer work unit (PAPER.md:81 fixes 1,024; smaller values for the sweep)")
     ap.add_argument("--no-4k", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=16)
