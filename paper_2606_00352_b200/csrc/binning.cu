@@ -15,6 +15,7 @@
 
 namespace {
 
+constexpr int FILL_QCAP = 1024;      // wide-span gaussians a fill CTA can defer (more are handled in place)
 constexpr int BIN_THREADS = 1024;   // two CTAs per SM at 32 registers: the pass is latency-bound, so warps in flight decide
 
 // exclusive block scan of NV values per thread position (1024 threads), with a running carry
@@ -163,6 +164,9 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
     extern __shared__ uint32_t s_cursor[];
     uint32_t* s_chunk = s_cursor + P.n_m;           // [lcap]
     uint32_t* s_pref = s_chunk + lcap;              // [lcap + 1] exclusive prefix of the chunk counts
+    uint32_t* s_queue = s_pref + lcap + 1;          // [2 * FILL_QCAP] (slot, key) of the gaussians with wide spans
+    __shared__ uint32_t s_nq;
+    if (threadIdx.x == 0) s_nq = 0;
     pdl_wait(); pdl_trigger();
     if (hdr->overflow) return;                      // capacity exceeded: write nothing (HIGS_E_CAPACITY)
     const uint32_t b = blockIdx.x;
@@ -196,6 +200,23 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
         while (lo < hi) { const uint32_t mid = (lo + hi + 1) >> 1; if (s_pref[mid] <= k) lo = mid; else hi = mid - 1; }
         return (size_t)s_chunk[lo] * HIGS_CHUNK + (k - s_pref[lo]);
     };
+    // A gaussian whose span did not fit the descriptor (more than 4 macro-tile rows: 0.8 % of the survivors at 1080p,
+    // 4.5 % at 4K) redoes the row scan, some hundreds of instructions.  Done in place it would run with one lane of the
+    // warp active in a quarter (1080p) to three quarters (4K) of all warp iterations, so such gaussians are queued and
+    // handled after the main loop, one per lane.
+    auto emit_wide = [&](size_t slot, uint32_t key) {
+        const unsigned long long item = ((unsigned long long)key << 32) | (unsigned long long)(uint32_t)slot;
+        const float4 s0 = __ldcs(rec + 4 * slot), s1 = __ldcs(rec + 4 * slot + 1), s2 = __ldcs(rec + 4 * slot + 2),
+                     s3 = __ldcs(rec + 4 * slot + 3);
+        RowScan rs;
+        rs.init(s0.x, s0.y, s2.z, s2.w, s3.x, s1.y, (float)HIGS_MT_H, P.n_my);
+        const float fW = (float)P.W, fH = (float)P.H;
+        for (int r = rs.r0; r <= rs.r1; ++r) {
+            int m0, m1;
+            if (!rs.row(r, (float)HIGS_MT_W, (float)HIGS_MT_H, fW, fH, P.n_mx, m0, m1)) continue;
+            for (int m = m0; m <= m1; ++m) pairs[atomicAdd(&s_cursor[r * P.n_mx + m], 1u)] = item;
+        }
+    };
     auto emit = [&](size_t slot, const uint4 bn) {  // bn = key, desc lo, desc hi, id
         const unsigned long long item = ((unsigned long long)bn.x << 32) | (unsigned long long)(uint32_t)slot;
         const unsigned long long desc = ((unsigned long long)bn.z << 32) | bn.y;
@@ -208,23 +229,19 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
                 const int cell0 = (r0 + rr) * P.n_mx + m0, wd = (int)(f >> 9);
                 for (int m = 0; m <= wd; ++m) pairs[atomicAdd(&s_cursor[cell0 + m], 1u)] = item;
             }
-        } else {                                    // span too large for the descriptor: redo the row scan
-            const float4 s0 = __ldcs(rec + 4 * slot), s1 = __ldcs(rec + 4 * slot + 1), s2 = __ldcs(rec + 4 * slot + 2),
-                         s3 = __ldcs(rec + 4 * slot + 3);
-            RowScan rs;
-            rs.init(s0.x, s0.y, s2.z, s2.w, s3.x, s1.y, (float)HIGS_MT_H, P.n_my);
-            const float fW = (float)P.W, fH = (float)P.H;
-            for (int r = rs.r0; r <= rs.r1; ++r) {
-                int m0, m1;
-                if (!rs.row(r, (float)HIGS_MT_W, (float)HIGS_MT_H, fW, fH, P.n_mx, m0, m1)) continue;
-                for (int m = m0; m <= m1; ++m) pairs[atomicAdd(&s_cursor[r * P.n_mx + m], 1u)] = item;
-            }
+        } else {                                    // span too large for the descriptor: queue it (or, queue full, do it here)
+            const uint32_t qpos = atomicAdd(&s_nq, 1u);
+            if (qpos < (uint32_t)FILL_QCAP) { s_queue[2 * qpos] = (uint32_t)slot; s_queue[2 * qpos + 1] = bn.x; }
+            else emit_wide(slot, bn.x);
         }
     };
     for (uint32_t k = threadIdx.x; k < total; k += BIN_THREADS) {
         const size_t slot = slot_of(k);
         emit(slot, __ldcs(bin + slot));
     }
+    __syncthreads();
+    const uint32_t n_wide = min(s_nq, (uint32_t)FILL_QCAP);
+    for (uint32_t k = threadIdx.x; k < n_wide; k += BIN_THREADS) emit_wide((size_t)s_queue[2 * k], s_queue[2 * k + 1]);
 }
 
 // test-facing exports (higs_get_lists / higs_get_records; never part of a frame)
@@ -270,7 +287,7 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
         return HIGS_OK;
     }
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, n_b);
-    const size_t smem = sizeof(uint32_t) * ((size_t)P.n_m + 2 * (size_t)lcap + 1);
+    const size_t smem = sizeof(uint32_t) * ((size_t)P.n_m + 2 * (size_t)lcap + 1 + 2 * FILL_QCAP);
     if (ev_count) cudaEventRecord(ev_count, st);    // the count pass ran inside k_project: this stage is empty
     HIGS_CUDA(ctx, launch_pdl(k_plan, dim3(1), dim3(1024), sizeof(uint32_t) * ((size_t)P.n_m + 1), st, P, ctx->mt_count, ctx->mt_offset,
                               ctx->batch_offset, ctx->unit_mt, ctx->unit_order, ctx->level_hist, ctx->level_cur, ctx->sort_jobs,
@@ -302,7 +319,7 @@ int higs_binning_smem_setup(higs_ctx* ctx)
 {
     int lcap_max = higs_part_lcap(ctx->n_chunks_max, ctx->n_sm);
     if (lcap_max < 96) lcap_max = 96;
-    const int bytes = (int)(sizeof(uint32_t) * ((size_t)ctx->max_nm + 2 * (size_t)lcap_max + 1));
+    const int bytes = (int)(sizeof(uint32_t) * ((size_t)ctx->max_nm + 2 * (size_t)lcap_max + 1 + 2 * FILL_QCAP));
     if (bytes > 48 * 1024) {
         HIGS_CUDA(ctx, cudaFuncSetAttribute(k_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     }
