@@ -289,7 +289,7 @@ def run_higs(args) -> int:
     }
     # DRAM bytes per launch (read + write) from the committed ncu --set full capture of this workload
     # (profiles/r01_final.md); measured once per round under the profiler, not in this run
-    NCU_TRAFFIC = {"project": 1.357e9, "fill": 1.18e8, "sort": 1.30e8, "raster": 3.10e8}
+    NCU_TRAFFIC = {"project": 1.357e9, "fill": 1.19e8, "sort": 1.30e8, "raster": 3.10e8}
     def hbm_roof(stage, nbytes):
         ms = stage_ms[stage]
         ach = nbytes / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
