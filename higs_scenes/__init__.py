@@ -252,6 +252,23 @@ def stack_gaussians(means, scales, quats, opacities, rgbs, W=129, H=129) -> Scen
     return Scene("handmade", means, scales, quats, opac, sh, 0, [make_camera(W, H)])
 
 
+def needle_scene(n: int = 300, W: int = 1920, H: int = 1080, seed: int = 6, sigma_lo_px: float = 60.0,
+                 sigma_hi_px: float = 350.0) -> Scene:
+    """Near-camera needles: one long axis (log-uniform screen-space sigma in [lo, hi] px), two axes of 1e-5,
+    rotated about the view axis by a random angle, centres spread over the image; degree-0 colours.  The conic
+    of such a gaussian is ill-conditioned (a c / det up to 1e5-1e7): the stress case for the conservative
+    bounding box / row scan (reading Q8)."""
+    rng = np.random.default_rng(seed)
+    fx = (W / 2.0) / np.tan(np.pi / 6.0)
+    z = rng.uniform(0.5, 1.5, n)
+    means = np.stack([rng.uniform(-0.4, 0.4, n) * z, rng.uniform(-0.25, 0.25, n) * z, z], axis=1)
+    sig_px = np.exp(rng.uniform(np.log(sigma_lo_px), np.log(sigma_hi_px), n))
+    scales = np.stack([sig_px * z / fx, np.full(n, 1e-5), np.full(n, 1e-5)], axis=1)
+    th = rng.uniform(0.0, np.pi, n)
+    quats = np.stack([np.cos(th / 2), np.zeros(n), np.zeros(n), np.sin(th / 2)], axis=1)
+    return stack_gaussians(means, scales, quats, rng.uniform(0.3, 0.99, n), rng.uniform(0, 1, (n, 3)), W, H)
+
+
 CONFIGS = {0: scene_cfg0, 1: scene_cfg1, 2: scene_cfg2, 3: scene_cfg3, 4: scene_cfg4}
 
 

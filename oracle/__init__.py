@@ -101,7 +101,7 @@ class Projected:
     valid: np.ndarray    # (N,) uint8
     reason: np.ndarray   # (N,) uint8 cull reason (0 = kept)
     key: np.ndarray      # (N,) uint32 depth key = bits(z_cam)
-    geo: np.ndarray      # (N,8) float32: mux, muy, a, b, c, tau, hx, hy
+    geo: np.ndarray      # (N,9) float32: mux, muy, a, b, c, tau, hx, hy, tau_s (scan / bbox threshold)
     conic: np.ndarray    # (N,3) float32: A, B2, C
     rgb: np.ndarray      # (N,3) float64
     opac: np.ndarray     # (N,) float32 (input opacities)
@@ -147,7 +147,7 @@ def project(scene, cam) -> Projected:
     sh = np.ascontiguousarray(scene.sh, dtype=np.float32)
     camf = cam.as_floats()
     valid = np.zeros(N, np.uint8); reason = np.zeros(N, np.uint8); key = np.zeros(N, np.uint32)
-    geo = np.zeros((N, 8), np.float32); conic = np.zeros((N, 3), np.float32); rgb = np.zeros((N, 3), np.float64)
+    geo = np.zeros((N, 9), np.float32); conic = np.zeros((N, 3), np.float32); rgb = np.zeros((N, 3), np.float64)
     nvis = lib().orc_project(N, _p(means, C.c_float), _p(scales, C.c_float), _p(quats, C.c_float),
                              _p(opac, C.c_float), _p(sh, C.c_float), scene.degree, _p(camf, C.c_float),
                              cam.W, cam.H, _p(valid, C.c_uint8), _p(reason, C.c_uint8), _p(key, C.c_uint32),

@@ -49,8 +49,10 @@
 #define ORC_EPS_T 1e-4   /* transmittance threshold epsilon, reading Q1 */
 #define ORC_ALPHA_MAX 0.99
 
-/* geo record, 8 floats per gaussian: mux, muy, a, b, c (2D covariance), tau, hx, hy */
-enum { G_MUX = 0, G_MUY, G_A, G_B, G_C, G_TAU, G_HX, G_HY, G_STRIDE };
+/* geo record, 9 floats per gaussian: mux, muy, a, b, c (2D covariance), tau, hx, hy, tau_s.
+ * tau decides the per-pixel 1/255 skip; tau_s >= tau is the same threshold with the margin the
+ * bounding box and the row scan need to stay conservative (see project_one step 9). */
+enum { G_MUX = 0, G_MUY, G_A, G_B, G_C, G_TAU, G_HX, G_HY, G_TAUS, G_STRIDE };
 
 static inline uint32_t f2u(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
 
@@ -134,7 +136,7 @@ static void sh_colour(const float* mean, const float* cam_pos, const float* sh, 
  *   valid[i]   1 / 0          reason[i] (may be NULL): 0 ok, 1 near, 2 quaternion, 3 det,
  *                              4 opacity, 5 off-screen
  *   key[i]     bits(z_cam)    (raw IEEE-754 bits, unsigned order = depth order)
- *   geo[i][8]  mux, muy, a, b, c, tau, hx, hy
+ *   geo[i][9]  mux, muy, a, b, c, tau, hx, hy, tau_s
  *   conic[i][3] A, B2, C      (q = A dx^2 + B2 dx dy + C dy^2)
  *   rgb[i][3]  fp64 colour
  * Returns the number of valid gaussians.
@@ -204,14 +206,24 @@ static int project_one(const float* m, const float* s, const float* qt, float o,
     if (!(x255 > 1.0f) || !(x255 <= FLT_MAX)) return 4;
     float tau = 2.0f * orc_ln_spec(x255);
     if (!(tau > 0.0f)) return 4;
-    float hx = sqrtf(tau * a), hy = sqrtf(tau * c);
+    /* The bounding box and the macro-tile row scan must be CONSERVATIVE with respect to the pixel
+     * test q <= tau ("conservative per-row ellipse-contour scan"; DESIGN.md reading
+     * Q8).  q is evaluated in fp32 from the conic (A, B2, C), whose cross term cancels for elongated
+     * gaussians (the hazard PAPER.md:180-226 describes): the region the pixel test accepts differs
+     * from the ellipse of the covariance (a, b, c) by a relative ~3 * 2^-24 * cond in tau, with
+     * cond = a c / det (measured over needles up to cond = 1e7).  The box and the scan therefore use
+     * tau_s = tau * (1 + 2^-20 cond), five times that; for ordinary gaussians (cond < 100) the
+     * margin is below 1e-4 of tau. */
+    float cond = (a * c) * rd;
+    float tau_s = tau * fmaf(cond, 9.5367431640625e-07f, 1.0f);
+    float hx = sqrtf(tau_s * a), hy = sqrtf(tau_s * c);
     /* 10. off-screen cull on the threshold ellipse's bounding box */
     float fW = (float)W, fH = (float)H;
     if (!(mux + hx > 0.0f) || !(mux - hx < fW) || !(muy + hy > 0.0f) || !(muy - hy < fH)) return 5;
     /* 11. depth key */
     *key = f2u(zc);
     geo[G_MUX] = mux; geo[G_MUY] = muy; geo[G_A] = a; geo[G_B] = b; geo[G_C] = c;
-    geo[G_TAU] = tau; geo[G_HX] = hx; geo[G_HY] = hy;
+    geo[G_TAU] = tau; geo[G_HX] = hx; geo[G_HY] = hy; geo[G_TAUS] = tau_s;
     conic[0] = A; conic[1] = B2; conic[2] = C;
     return 0;
 }
@@ -300,7 +312,7 @@ int orc_scan(const float* g, int W, int H, int cw, int ch, int32_t* out, int cap
 {
     const int ncx = (W + cw - 1) / cw, ncy = (H + ch - 1) / ch;
     const float mux = g[G_MUX], muy = g[G_MUY], a = g[G_A], b = g[G_B], c = g[G_C];
-    const float tau = g[G_TAU], hx = g[G_HX], hy = g[G_HY];
+    const float tau = g[G_TAUS], hx = g[G_HX], hy = g[G_HY];   /* the scan runs on tau_s (project_one step 9) */
     const float fcw = (float)cw, fch = (float)ch, fW = (float)W, fH = (float)H;
     const float ytop_e = muy - hy, ybot_e = muy + hy;
     int r0 = (int)clampf(floorf(ytop_e / fch), 0.0f, (float)(ncy - 1));

@@ -1,8 +1,11 @@
 """Pins for the oracle's integer lists (O-LIST) and for the three renderers agreeing.
 
 * row scan (N-SCAN) against an independent exact test written here in fp64 numpy: a cell is hit
-  iff the minimum of the quadratic form over the (clipped) cell rectangle is <= tau;
-* conservativeness by brute force: every pixel centre with q <= tau lies in a listed macro-tile;
+  iff the minimum of the quadratic form over the (clipped) cell rectangle is <= tau_s (the scan
+  threshold: tau with the conditioning margin of DESIGN.md reading Q8);
+* conservativeness by brute force: every pixel centre with q <= tau lies in a listed macro-tile; for
+  ill-conditioned needles: every pixel the fp32 test accepts lies inside the ellipse of tau_s, which
+  the scan covers exactly by the previous pin;
 * counts / offsets / sorted segments against numpy (bincount, cumsum, lexsort);
 * orc_render == orc_brute (bounding box logic) and == orc_render_batched (Eq. (1)),
   with B_r = 16 forcing many batches per macro-tile.
@@ -33,7 +36,8 @@ def _min_q_over_rect(mux, muy, A, B2, C, x0, x1, y0, y1):
 
 
 def _cells_by_rect_test(geo, W, H, cw, ch):
-    mux, muy, a, b, c, tau = (float(v) for v in geo[:6])
+    mux, muy, a, b, c = (float(v) for v in geo[:5])
+    tau = float(geo[8])                      # the scan runs on tau_s
     det = a * c - b * b
     A, B2, C = c / det, -2 * b / det, a / det
     ncx, ncy = (W + cw - 1) // cw, (H + ch - 1) // ch
@@ -83,6 +87,63 @@ def test_row_scan_is_conservative_for_pixel_centres():
         inside = q <= float(tau) * (1 + 1e-5)
         need = set(((ys[inside] // 32) * nmx + xs[inside] // 64).tolist())
         assert need <= cells, i
+
+
+def _fp32_pixel_test(pr, i, xs, ys):
+    """The pinned fp32 sequence N-Q on every pixel centre (numpy float32 ops, fma through float64)."""
+    A, B2, C = (np.float32(v) for v in pr.conic[i])
+    dx = (xs + 0.5).astype(np.float32) - pr.geo[i, 0]
+    dy = (ys + 0.5).astype(np.float32) - pr.geo[i, 1]
+    u = A * dx
+    a0 = u * dx
+    b0 = B2 * dx
+    t = (np.float64(C) * dy.astype(np.float64) + b0.astype(np.float64)).astype(np.float32)
+    q = (t.astype(np.float64) * dy.astype(np.float64) + a0.astype(np.float64)).astype(np.float32)
+    return q <= pr.geo[i, 5]
+
+
+def test_scan_threshold_covers_the_fp32_pixel_test_of_needles():
+    """Elongated gaussians: the region the fp32 conic test accepts leaves the ellipse {q_cov <= tau} of the
+    covariance by up to ~3 * 2^-24 * cond in tau (cancellation in the cross term).  tau_s
+    must cover it with room to spare; without the margin 60-odd of these 500 needles fail."""
+    W, H = 960, 540
+    s = hs.needle_scene(500, W, H, seed=11, sigma_lo_px=20, sigma_hi_px=600)
+    pr = oracle.project(s, s.cameras[0])
+    ys, xs = np.mgrid[0:H, 0:W]
+    outside_plain, worst = 0, 0.0
+    for i in np.nonzero(pr.valid)[0]:
+        ins = _fp32_pixel_test(pr, i, xs, ys)
+        if not ins.any():
+            continue
+        a, b, c = (np.float64(pr.geo[i, k]) for k in (2, 3, 4))
+        det = a * c - b * b
+        dx = (xs[ins] + 0.5) - np.float64(pr.geo[i, 0])
+        dy = (ys[ins] + 0.5) - np.float64(pr.geo[i, 1])
+        q_cov = ((c * dx * dx - 2 * b * dx * dy + a * dy * dy) / det).max()
+        tau, tau_s = float(pr.geo[i, 5]), float(pr.geo[i, 8])
+        assert tau_s >= tau
+        det32 = np.float32(a * c - np.float64(np.float32(b) * np.float32(b)))     # fma(a, c, -(b*b)) as N-PROJ rounds it
+        assert tau_s / tau - 1 == pytest.approx(2.0 ** -20 * a * c / np.float64(det32), rel=1e-3, abs=1e-7)
+        outside_plain += q_cov > tau
+        if q_cov > tau:
+            worst = max(worst, (q_cov / tau - 1) / (tau_s / tau - 1))
+        assert q_cov <= tau + 0.5 * (tau_s - tau), i       # at most half of the margin is ever used
+    assert outside_plain > 20                               # the hazard is real on this scene
+    assert worst < 0.5
+
+
+def test_render_equals_brute_equals_batched_on_needles():
+    """Same three renderers on ill-conditioned needles at 1080p: before the margin one pixel of this frame
+    differed between the bounding-box renderer and brute force."""
+    s = hs.needle_scene(300, 1920, 1080, seed=6)
+    pr = oracle.project(s, s.cameras[0])
+    assert pr.n_vis == 300
+    brute = oracle.brute(pr)
+    assert np.array_equal(oracle.render(pr), brute)
+    ls = oracle.bin_lists(pr)
+    batched = oracle.render_batched(pr, ls)
+    assert np.abs(batched - brute).max() < 1e-4 * float(pr.rgb.max())     # only the termination point is free (Q2)
+    assert np.abs(oracle.render_batched(pr, ls, terminate=False) - oracle.brute(pr, terminate=False)).max() < 1e-12
 
 
 @pytest.mark.parametrize("B_r", [1024, 16])

@@ -51,6 +51,23 @@ def test_golden_ewa_is_the_closed_form():
     assert g["mux"] == pytest.approx(fx * x / z + 64.5, rel=1e-12)
 
 
+def test_golden_ewa_clamp_active_is_the_closed_form():
+    g = load_golden("ewa_clamp_active.txt")
+    fx = float(np.float32(64.5 / math.tan(math.radians(30.0))))
+    sx, sy, sz, z = 0.05, 0.03, 0.6, 3.0
+    lim = 0.65 * 129 / fx
+    assert g["lim"] == pytest.approx(lim, rel=1e-12) and 0.9 > lim
+    assert g["A_a"] == pytest.approx(fx * fx * (sx * sx + lim * lim * sz * sz) / z ** 2 + 0.3, rel=1e-12)
+    assert g["A_c"] == pytest.approx((fx * sy / z) ** 2 + 0.3, rel=1e-12)
+    assert g["A_mux"] == pytest.approx(fx * 0.9 + 64.5, rel=1e-12)
+    assert g["A_a_if_unclamped"] == pytest.approx(fx * fx * (sx * sx + 0.81 * sz * sz) / z ** 2 + 0.3, rel=1e-12)
+    assert g["B_a"] == pytest.approx((fx * sx / z) ** 2 + 0.3, rel=1e-12)
+    assert g["B_c"] == pytest.approx(fx * fx * (sy * sy + lim * lim * sz * sz) / z ** 2 + 0.3, rel=1e-12)
+    assert g["B_muy"] == pytest.approx(-fx * 0.9 + 64.5, rel=1e-12)
+    assert g["C_b"] == pytest.approx(-(fx * lim / z) ** 2 * sz * sz, rel=1e-12)
+    assert g["C_a"] == g["A_a"] and g["C_c"] == g["B_c"]
+
+
 def test_golden_grid_counts():
     g = load_golden("grid.txt")
     assert oracle.MT_W == g["mt_w"] and oracle.MT_H == g["mt_h"] and oracle.B_R == g["batch_cap"]
@@ -198,6 +215,34 @@ def test_ewa_off_axis_golden():
     d = oracle.project_f64((1, 0, 3), (0.05, 0.03, 0.2), (1, 0, 0, 0), 0.8, cam)
     # the fp64 definition still sees the fp32-rounded inputs (0.05f, 0.2f, ...): 3e-8 relative
     assert d["a"] == pytest.approx(g["a"], rel=2e-7) and d["c"] == pytest.approx(g["c"], rel=2e-7)
+
+
+def test_ewa_frustum_clamp_active_golden():
+    """The Jacobian clamp (reading Q11) with the clamp ACTIVE, against the hand-worked closed form - not against the
+    oracle's own fp64 twin: a wrong limit, a clamp that also moves the centre, a clamp on the wrong axis or with
+    the wrong sign each fail here."""
+    g = load_golden("ewa_clamp_active.txt")
+    sc = (0.05, 0.03, 0.6)
+    for name, mean in (("A", (2.7, 0.0, 3.0)), ("B", (0.0, -2.7, 3.0)), ("C", (2.7, -2.7, 3.0))):
+        s, cam = _one(mean=mean, scale=sc)
+        pr = oracle.project(s, cam)
+        assert pr.n_vis == 1, name                        # centre 36 px outside, ellipse (55 px) still reaches the image
+        assert pr.geo[0, 2] == pytest.approx(g[name + "_a"], rel=3e-6), name
+        assert pr.geo[0, 4] == pytest.approx(g[name + "_c"], rel=3e-6), name
+        if g[name + "_b"] == 0.0:
+            assert abs(pr.geo[0, 3]) < 1e-4, name
+        else:
+            assert pr.geo[0, 3] == pytest.approx(g[name + "_b"], rel=3e-6), name
+        if name + "_mux" in g:                            # the centre itself is never clamped
+            assert pr.geo[0, 0] == pytest.approx(g[name + "_mux"], rel=1e-6), name
+            assert pr.geo[0, 1] == pytest.approx(g[name + "_muy"], rel=1e-6), name
+    s, cam = _one(mean=(2.7, 0.0, 3.0), scale=sc)
+    assert abs(float(oracle.project(s, cam).geo[0, 2]) - g["A_a_if_unclamped"]) > 100.0
+    # just inside the limit the clamp is inactive and the plain closed form holds
+    fx = float(np.float32(64.5 / math.tan(math.radians(30.0))))
+    x = 0.74 * 3.0
+    s, cam = _one(mean=(x, 0.0, 3.0), scale=sc)
+    assert oracle.project(s, cam).geo[0, 2] == pytest.approx(fx * fx * (0.05 ** 2 + (0.74 * 0.6) ** 2) / 9.0 + 0.3, rel=3e-6)
 
 
 def test_ewa_monte_carlo_small_scale_limit():
