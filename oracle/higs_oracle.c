@@ -405,15 +405,17 @@ float orc_pixel_q(float px, float py, float mux, float muy, float A, float B2, f
     return fmaf(t, dy, a0);
 }
 
-/* alpha of gaussian g at pixel (i,j), or a negative value if it is skipped.  Smooth part fp64. */
+/* alpha of gaussian g at pixel (i,j), or a negative value if it is skipped.  O-IMG: "q = N-Q(p, g); if
+ * q > tau skip; alpha = min(0.99, o exp(-q/2))" - ONE q, the pinned fp32 one, decides the skip and gives alpha; exp and
+ * the product are fp64.  (For an elongated gaussian the conic form cancels, and a second, fp64
+ * evaluation of q would differ from the pinned one by ~2^-24 a c/det relative: two renderers that agree on every skip
+ * decision would then disagree on alpha by that much.) */
 static inline double pixel_alpha(int i, int j, const float* geo, const float* conic, float o)
 {
     float px = (float)i + 0.5f, py = (float)j + 0.5f;
     float q32 = orc_pixel_q(px, py, geo[G_MUX], geo[G_MUY], conic[0], conic[1], conic[2]);
     if (!(q32 <= geo[G_TAU])) return -1.0;          /* alpha < 1/255: skipped */
-    double dx = (double)px - (double)geo[G_MUX], dy = (double)py - (double)geo[G_MUY];
-    double q = (double)conic[0] * dx * dx + (double)conic[1] * dx * dy + (double)conic[2] * dy * dy;
-    double alpha = (double)o * exp(-0.5 * q);
+    double alpha = (double)o * exp(-0.5 * (double)q32);
     return alpha < ORC_ALPHA_MAX ? alpha : ORC_ALPHA_MAX;   /* min(0.99, alpha) */
 }
 
