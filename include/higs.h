@@ -43,11 +43,6 @@ extern "C" {
 #define HIGS_MT_H        32     /* macro-tile height, px (4 tiles)  */
 #define HIGS_MT_TILES    32     /* M: render tiles per macro-tile  */
 #define HIGS_BATCH_CAP   1024   /* B_r: gaussians per rasterizer work unit  */
-#ifndef HIGS_RASTER_SPLIT
-#define HIGS_RASTER_SPLIT 1     /* the rasterizer composites a unit in this many consecutive parts ("sub-units"), each with
-                                   its own partial (r,g,b,T) and active mask; Eq. (1) is associative, so the image is the same.
-                                   1 = whole units (measured best on B200: parts of 512 cost more in fixed work than they balance) */
-#endif
 #define HIGS_PART_BATCH  8192   /* B_p: gaussians per partitioning batch  */
 #define HIGS_SORT_BLOCK  8192   /* largest segment sorted by one CTA */
 
@@ -102,7 +97,7 @@ typedef struct {
     const uint32_t* mt_offset;       /* [N_M+1]   exclusive prefix sum = segment bounds           */
     const uint32_t* batch_offset;    /* [N_M+1]   exclusive prefix sum of ceil(n_m/B_r)           */
     const uint64_t* pairs;           /* [n_pairs] (key << 32 | id), each segment ascending        */
-    const uint32_t* unit_active;     /* [n_units * HIGS_RASTER_SPLIT] 32-bit active-tile mask per sub-unit */
+    const uint32_t* unit_active;     /* [n_units] 32-bit active-tile mask per unit  */
 } higs_lists;
 
 /* Per-gaussian records of the last frame.  DEVICE pointers owned by the context. */

@@ -20,7 +20,7 @@ from . import build as _build
 
 HIGS_OK, HIGS_E_ARG, HIGS_E_CUDA, HIGS_E_CAPACITY, HIGS_E_NOMEM = 0, -1, -2, -3, -4
 HIGS_FLAG_STAGE_TIMERS, HIGS_FLAG_COUNT_EVALS, HIGS_FLAG_NO_XBATCH_CUT = 1, 2, 4
-HIGS_TILE, HIGS_MT_W, HIGS_MT_H, HIGS_MT_TILES, HIGS_BATCH_CAP, HIGS_RASTER_SPLIT = 8, 64, 32, 32, 1024, 1
+HIGS_TILE, HIGS_MT_W, HIGS_MT_H, HIGS_MT_TILES, HIGS_BATCH_CAP = 8, 64, 32, 32, 1024
 
 EXPORTS = ["higs_abi_version", "higs_strerror", "higs_last_error", "higs_create", "higs_destroy", "higs_set_flags",
            "higs_set_batch_cap", "higs_render", "higs_render_host", "higs_scene_upload", "higs_render_view_host",
@@ -219,7 +219,7 @@ def higs_get_lists(ctx) -> dict:
             "mt_offset": _dev_to_numpy(ctx, ls.mt_offset, nm + 1, np.uint32),
             "batch_offset": _dev_to_numpy(ctx, ls.batch_offset, nm + 1, np.uint32),
             "keys": (pairs >> np.uint64(32)).astype(np.uint32), "ids": (pairs & np.uint64(0xffffffff)).astype(np.uint32),
-            "unit_active": _dev_to_numpy(ctx, ls.unit_active, nun * HIGS_RASTER_SPLIT, np.uint32)}
+            "unit_active": _dev_to_numpy(ctx, ls.unit_active, nun, np.uint32)}
 
 
 def higs_get_records(ctx) -> dict:

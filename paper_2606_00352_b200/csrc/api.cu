@@ -34,15 +34,16 @@ template <typename T> void dev_free(T*& p) { if (p) cudaFree(p); p = nullptr; }
 int alloc_unit_buffers(higs_ctx* ctx)
 {
     dev_free(ctx->unit_mt); dev_free(ctx->unit_active); dev_free(ctx->partial);
-    dev_free(ctx->unit_order); dev_free(ctx->level_hist); dev_free(ctx->level_cur);
+    dev_free(ctx->unit_order); dev_free(ctx->level_hist); dev_free(ctx->level_cur); dev_free(ctx->cut_term);
     ctx->max_units = ctx->max_nm + (ctx->max_pairs + ctx->batch_cap - 1) / ctx->batch_cap + 1;
     int rc;
     if ((rc = dev_alloc(ctx, &ctx->unit_mt, (size_t)ctx->max_units))) return rc;
-    if ((rc = dev_alloc(ctx, &ctx->unit_active, (size_t)ctx->max_units * HIGS_RASTER_SPLIT))) return rc;
-    if ((rc = dev_alloc(ctx, &ctx->unit_order, (size_t)ctx->max_units * HIGS_RASTER_SPLIT))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->unit_active, (size_t)ctx->max_units))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->unit_order, (size_t)ctx->max_units))) return rc;
     if ((rc = dev_alloc(ctx, &ctx->level_hist, (size_t)ctx->max_units + 2))) return rc;
-    if ((rc = dev_alloc(ctx, &ctx->level_cur, 3 * ((size_t)ctx->max_units + 2)))) return rc;
-    if ((rc = dev_alloc(ctx, &ctx->partial, (size_t)ctx->max_units * HIGS_RASTER_SPLIT * HIGS_MT_TILES * 64))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->level_cur, (size_t)ctx->max_units + 2))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->partial, (size_t)ctx->max_units * HIGS_MT_TILES * 64))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->cut_term, (size_t)ctx->max_units * HIGS_MT_TILES))) return rc;
     return HIGS_OK;
 }
 
@@ -77,8 +78,6 @@ int render_impl(higs_ctx* ctx, const float* means, const float* scales, const fl
     ctx->n_launches = 0;
     // one memset: frame header, per-macro-tile pair counts and fill cursors (one allocation)
     HIGS_CUDA(ctx, cudaMemsetAsync(ctx->hdr, 0, sizeof(uint32_t) * (HIGS_HDR_WORDS + 2 * ((size_t)ctx->max_nm + 1)), st));
-    if (!(ctx->flags & HIGS_FLAG_NO_XBATCH_CUT))
-        HIGS_CUDA(ctx, cudaMemsetAsync(ctx->tile_logT, 0, sizeof(int) * (size_t)P.n_m * HIGS_MT_TILES, st));
     if (timers) cudaEventRecord(ev[0], st);
     if ((rc = launch_project(ctx, P, means, scales, quats, opac, sh, N, st))) return rc;
     if (timers) cudaEventRecord(ev[1], st);
@@ -183,7 +182,7 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     if ((rc = dev_alloc(ctx, &ctx->part_list, (size_t)ctx->n_chunks_max))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->part_desc, (size_t)ctx->n_part_max))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->hist, (size_t)ctx->n_part_max * nm))) return fail(rc);
-    if ((rc = dev_alloc(ctx, &ctx->tile_logT, (size_t)nm * HIGS_MT_TILES))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->cut_word, (size_t)nm * HIGS_MT_TILES))) return fail(rc);
     static_assert(sizeof(FrameHeader) <= sizeof(uint32_t) * HIGS_HDR_WORDS, "frame header outgrew its block");
     if ((rc = dev_alloc(ctx, &ctx->hdr_block, HIGS_HDR_WORDS + 2 * ((size_t)nm + 1)))) return fail(rc);
     ctx->hdr = reinterpret_cast<FrameHeader*>(ctx->hdr_block);
@@ -232,7 +231,7 @@ void higs_destroy(higs_ctx* ctx)
     dev_free(ctx->mt_offset); dev_free(ctx->batch_offset); dev_free(ctx->unit_mt);
     dev_free(ctx->unit_active); dev_free(ctx->pairs); dev_free(ctx->pairs_alt); dev_free(ctx->sort_jobs);
     dev_free(ctx->over_segs); dev_free(ctx->split_segs); dev_free(ctx->splitters); dev_free(ctx->bucket_count);
-    dev_free(ctx->bucket_cursor); dev_free(ctx->bucket_seg); dev_free(ctx->partial); dev_free(ctx->tile_logT);
+    dev_free(ctx->bucket_cursor); dev_free(ctx->bucket_seg); dev_free(ctx->partial); dev_free(ctx->cut_word); dev_free(ctx->cut_term);
     dev_free(ctx->unit_order); dev_free(ctx->level_hist); dev_free(ctx->level_cur);
     dev_free(ctx->s_means); dev_free(ctx->s_scales); dev_free(ctx->s_quats); dev_free(ctx->s_opac); dev_free(ctx->s_sh);
     dev_free(ctx->s_img);

@@ -2,11 +2,11 @@
 // PAPER.md:247-257 section 4.3, section 3.1).  The count pass (a2) lives in project.cu.
 //
 // Count and fill each run one CTA per partitioning batch.  Here a batch is the set of
-// 512-id chunks one persistent projection CTA claimed (project.cu), so N_B = a whole number of CTAs per SM;
+// HIGS_CHUNK-id chunks one persistent projection CTA claimed (project.cu), so N_B = a whole number of CTAs per SM;
 // fill only touches the dense survivor slots, so culled gaussians never reach it.  The
-// count CTA's histogram is one row of the N_B x N_M matrix; the scan turns it into write bases in two
-// levels (groups of 32 batches);
-// the fill CTA replays the intersection -- from the 64-bit span descriptor the count left in the
+// count CTA's histogram is one row of the N_B x N_M matrix and is also added to mt_count[m] by atomics, so the
+// segment bounds are one scan over m (k_plan); a fill CTA reserves its share of a segment with one atomic on
+// mt_fill[m].  The fill CTA replays the intersection -- from the 64-bit span descriptor the count left in the
 // record, or by redoing the row scan N-SCAN when the span did not fit -- and drops
 // (depth key << 32 | id) at base + local rank.
 #include <stdio.h>
@@ -17,42 +17,6 @@ namespace {
 
 constexpr int FILL_QCAP = 1024;      // wide-span gaussians a fill CTA can defer (more are handled in place)
 constexpr int BIN_THREADS = 1024;   // two CTAs per SM at 32 registers: the pass is latency-bound, so warps in flight decide
-
-// exclusive block scan of NV values per thread position (1024 threads), with a running carry
-template <int NV>
-__device__ __forceinline__ void block_scan_excl(uint32_t (&v)[NV], uint32_t (&carry)[NV], uint32_t* s_warp /* [32*NV] */)
-{
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    uint32_t incl[NV];
-#pragma unroll
-    for (int q = 0; q < NV; ++q) {
-        uint32_t x = v[q];
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
-        incl[q] = x;
-        if (lane == 31) s_warp[wid * NV + q] = x;
-    }
-    __syncthreads();
-    if (wid == 0) {
-#pragma unroll
-        for (int q = 0; q < NV; ++q) {
-            uint32_t x = s_warp[lane * NV + q];
-            uint32_t t = x;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, t, d); if (lane >= d) t += y; }
-            s_warp[lane * NV + q] = t - x;               // exclusive warp base
-            if (lane == 31) s_warp[32 * NV + q] = t;     // block total
-        }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int q = 0; q < NV; ++q) {
-        const uint32_t excl = carry[q] + s_warp[wid * NV + q] + incl[q] - v[q];
-        carry[q] += s_warp[32 * NV + q];
-        v[q] = excl;
-    }
-    __syncthreads();
-}
 
 // Scan (a3) + batch schedule (a6) + sort plan, one CTA of 1024 threads:
 //   mt_count[m] was accumulated by the projection CTAs (one atomicAdd per touched macro-tile per CTA);
@@ -68,9 +32,12 @@ k_plan(const FrameParams P,
     extern __shared__ uint32_t s_bo[];                            // [n_m + 1] copy of batch_offset for the unit -> macro-tile search
     __shared__ uint32_t s_warp[33 * 8];
     __shared__ uint32_t s_max;
+    __shared__ unsigned long long s_total;
+    if (threadIdx.x == 0) { s_max = 0; s_total = 0ull; }
     pdl_wait(); pdl_trigger();
-    if (threadIdx.x == 0) s_max = 0;
+    __syncthreads();
     uint32_t carry[2] = {0, 0};
+    unsigned long long my_total = 0;
     const uint32_t br = (uint32_t)P.batch_cap;
     // pass 1: totals and offsets
     for (int m0 = 0; m0 < P.n_m; m0 += 1024) {
@@ -78,15 +45,20 @@ k_plan(const FrameParams P,
         uint32_t n = 0;
         if (m < P.n_m) {
             n = mt_count[m];
+            my_total += n;
             if (n) atomicMax(&s_max, n);
         }
         uint32_t v[2] = { n, (n + br - 1) / br };
-        block_scan_excl<2>(v, carry, s_warp);
+        plan_scan<2>(v, carry, s_warp);
         if (m < P.n_m) { mt_offset[m] = v[0]; batch_offset[m] = v[1]; s_bo[m] = v[1]; }
     }
+    // the 32-bit scan wraps beyond 2^32 pairs: the capacity check is on a 64-bit total (one shared atomic per warp)
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) my_total += __shfl_xor_sync(0xffffffffu, my_total, d);
+    if ((threadIdx.x & 31) == 0 && my_total) atomicAdd(&s_total, my_total);
     __syncthreads();
     const uint32_t n_pairs = carry[0], n_units = carry[1];
-    const bool overflow = n_pairs > P.max_pairs || n_units > P.max_units;
+    const bool overflow = s_total > (unsigned long long)P.max_pairs || n_units > P.max_units;
     if (threadIdx.x == 0) {
         mt_offset[P.n_m] = n_pairs; batch_offset[P.n_m] = n_units; s_bo[P.n_m] = n_units;
         hdr->n_pairs = overflow ? 0u : n_pairs;
@@ -98,8 +70,6 @@ k_plan(const FrameParams P,
     sort_plan_body(mt_offset, P.n_m, overflow, sort_jobs, max_jobs, split, hdr, s_warp);
     if (overflow) return;
     __syncthreads();
-    uint32_t* level_base = level_cur + (P.max_units + 2);
-    uint32_t* level_cnt = level_base + (P.max_units + 2);
     // pass 2: unit table, and the order the rasterizer claims (sub-)units in: batch index j major ("level" j =
     // the j-th batch of every macro-tile that has one), so that by the time a deep batch starts the batches
     // in front of it have published their transmittance bounds (cross-batch cut).
@@ -128,11 +98,11 @@ k_plan(const FrameParams P,
             const uint32_t j = j0 + threadIdx.x;
             const uint32_t h = (j < max_nb) ? level_hist[j + 1] : 0u;       // hist[0] is unused (nb = 0 is never counted)
             uint32_t v[1] = { h };
-            block_scan_excl<1>(v, c_hist, s_warp);                        // v = #{1 <= nb <= j}
+            plan_scan<1>(v, c_hist, s_warp);                        // v = #{1 <= nb <= j}
             const uint32_t cnt = (j < max_nb) ? n_nonempty - v[0] : 0u;     // macro-tiles with nb > j
             uint32_t b[1] = { cnt };
-            block_scan_excl<1>(b, c_base, s_warp);
-            if (j < max_nb) { level_cur[j] = b[0]; level_base[j] = b[0]; level_cnt[j] = cnt; }
+            plan_scan<1>(b, c_base, s_warp);
+            if (j < max_nb) level_cur[j] = b[0];
         }
     }
     __syncthreads();
@@ -140,12 +110,8 @@ k_plan(const FrameParams P,
         int lo = 0, hi = P.n_m - 1;                                       // last m with batch_offset[m] <= u and a batch there
         while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_bo[mid] <= u) lo = mid; else hi = mid - 1; }
         unit_mt[u] = (uint32_t)lo;
-        // sub-unit (u, h) = part h of unit u (HIGS_RASTER_SPLIT parts): level j's first parts, then its second parts, ...
         const uint32_t lvl = u - s_bo[lo];
-        const uint32_t p = atomicAdd(&level_cur[lvl], 1u) - level_base[lvl];
-#pragma unroll
-        for (uint32_t h = 0; h < HIGS_RASTER_SPLIT; ++h)
-            unit_order[HIGS_RASTER_SPLIT * level_base[lvl] + h * level_cnt[lvl] + p] = u * HIGS_RASTER_SPLIT + h;
+        unit_order[atomicAdd(&level_cur[lvl], 1u)] = u;
     }
 }
 
@@ -159,7 +125,8 @@ __global__ void __launch_bounds__(BIN_THREADS, 2)
 k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ part_list, const uint2* __restrict__ part_desc, int lcap,
        const uint4* __restrict__ bin, const float4* __restrict__ rec,
        const FrameParams P, const uint32_t* __restrict__ hist, uint32_t* __restrict__ mt_fill, const uint32_t* __restrict__ mt_offset,
-       unsigned long long* __restrict__ pairs, const FrameHeader* __restrict__ hdr)
+       unsigned long long* __restrict__ pairs, const FrameHeader* __restrict__ hdr,
+       unsigned long long* __restrict__ cut_word, int* __restrict__ cut_term)
 {
     extern __shared__ uint32_t s_cursor[];
     uint32_t* s_chunk = s_cursor + P.n_m;           // [lcap]
@@ -169,6 +136,14 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
     if (threadIdx.x == 0) s_nq = 0;
     pdl_wait(); pdl_trigger();
     if (hdr->overflow) return;                      // capacity exceeded: write nothing (HIGS_E_CAPACITY)
+    // the rasterizer's cross-batch cut state starts every frame at zero (raster.cu): cleared here, where the grid is wide
+    // and the unit count is known, instead of by a memset sized for the capacity
+    if (!(P.flags & HIGS_FLAG_NO_XBATCH_CUT)) {
+        const size_t n_word = (size_t)P.n_m * HIGS_MT_TILES, n_term = (size_t)hdr->n_units * HIGS_MT_TILES;
+        const size_t stride = (size_t)gridDim.x * BIN_THREADS;
+        for (size_t i = (size_t)blockIdx.x * BIN_THREADS + threadIdx.x; i < n_word; i += stride) cut_word[i] = 0ull;
+        for (size_t i = (size_t)blockIdx.x * BIN_THREADS + threadIdx.x; i < n_term; i += stride) cut_term[i] = 0;
+    }
     const uint32_t b = blockIdx.x;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const uint2 pd = part_desc[b];
@@ -209,7 +184,7 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
         const float4 s0 = __ldcs(rec + 4 * slot), s1 = __ldcs(rec + 4 * slot + 1), s2 = __ldcs(rec + 4 * slot + 2),
                      s3 = __ldcs(rec + 4 * slot + 3);
         RowScan rs;
-        rs.init(s0.x, s0.y, s2.z, s2.w, s3.x, s1.y, (float)HIGS_MT_H, P.n_my);
+        rs.init(s0.x, s0.y, s2.z, s2.w, s3.x, tau_scan(s2.z, s2.w, s3.x, s1.y), (float)HIGS_MT_H, P.n_my);
         const float fW = (float)P.W, fH = (float)P.H;
         for (int r = rs.r0; r <= rs.r1; ++r) {
             int m0, m1;
@@ -295,7 +270,7 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
     HIGS_CUDA(ctx, launch_pdl(k_fill, dim3(n_b), dim3(BIN_THREADS), smem, st, ctx->chunk_count, ctx->part_list, ctx->part_desc, lcap, ctx->bin,
-                              ctx->rec, P, ctx->hist, ctx->mt_fill, ctx->mt_offset, ctx->pairs, ctx->hdr));
+                              ctx->rec, P, ctx->hist, ctx->mt_fill, ctx->mt_offset, ctx->pairs, ctx->hdr, ctx->cut_word, ctx->cut_term));
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }

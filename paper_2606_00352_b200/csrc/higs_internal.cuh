@@ -71,8 +71,8 @@ struct higs_ctx {
     // scratch (device)
     uint32_t* valid_bits;      // [ceil(maxN/32)]
     float4*   rec;             // [slots][4]  mux,muy,A,B2 | C,tau,log2o,r | g,b,a,b | c,bits(key),id,-   (64 B; the rasterizer gathers the
-                               //             first 40 B).  A slot is the dense position of a surviving gaussian: survivor k of the
-                               //             512-id chunk c sits at c*512 + k (monotone in the id)
+                               //             first 48 B).  A slot is the dense position of a surviving gaussian: survivor k of the
+                               //             HIGS_CHUNK-id chunk c sits at c*HIGS_CHUNK + k (monotone in the id)
     uint4*    bin;             // [slots]     bits(key), span descriptor lo, hi, id   (16 B, read by fill)
     uint32_t* chunk_count;     // [chunks]    survivors of the chunk
     uint32_t* part_list;       // [chunks]    chunk ids grouped by the partition CTA that claimed them
@@ -85,11 +85,10 @@ struct higs_ctx {
     uint32_t* mt_offset;       // [max_nm+1]
     uint32_t* batch_offset;    // [max_nm+1]
     uint32_t* unit_mt;         // [max_units] macro-tile of unit u
-    uint32_t* unit_active;     // [max_units * HIGS_RASTER_SPLIT] per sub-unit
-    uint32_t* unit_order;      // [max_units * HIGS_RASTER_SPLIT] sub-units in the order the rasterizer claims them: batch index j major,
-                               //             within a level all first parts, then all second parts
+    uint32_t* unit_active;     // [max_units] 32-bit active-tile mask per unit
+    uint32_t* unit_order;      // [max_units] units in the order the rasterizer claims them: batch index j major
     uint32_t* level_hist;      // [max_units+2] scratch of k_plan: macro-tiles per batch count, then level cursors
-    uint32_t* level_cur;       // [3][max_units+2] level cursors, level bases, level sizes
+    uint32_t* level_cur;       // [max_units+2] write cursor of each level in unit_order
     unsigned long long* pairs; // [max_pairs]
     unsigned long long* pairs_alt; // [max_pairs] ping-pong buffer of the overflow merge
     SortJob*  sort_jobs;       // [2][HIGS_N_TIERS][max_jobs]  list 0: whole segments, list 1: buckets
@@ -102,9 +101,10 @@ struct higs_ctx {
     uint32_t* bucket_cursor;   // [max_buckets]  write position of the scatter pass
     uint32_t* bucket_seg;      // [max_buckets]  index into split_segs
     int64_t   max_buckets;
-    float4*   partial;         // [max_units * HIGS_RASTER_SPLIT][32 tiles][64 px] (r,g,b,T)
-    int*      tile_logT;       // [max_nm][32] running sum over the finished units of a macro-tile of log2(largest transmittance left in the
-                               //             tile) x 1024, each term rounded towards zero: an upper bound of the transmittance in front of later units
+    float4*   partial;         // [max_units][32 tiles][64 px] (r,g,b,T)
+    unsigned long long* cut_word;  // [max_nm][32] cross-batch cut: (k << 32 | sum of the terms of batches 0 .. k-1), a cached prefix (raster.cu)
+    int*      cut_term;        // [max_units][32] log2(largest transmittance the unit left in the tile) x 1024, rounded towards zero, minus 1;
+                               //             0 = not published.  Both are zeroed every frame by k_fill
     FrameHeader* hdr;          // device
     FrameHeader* hdr_host;     // pinned
     // resident scene / host staging
@@ -120,6 +120,8 @@ struct higs_ctx {
     cudaEvent_t ev[9];
     bool timers_valid;
     int n_launches;            // kernels enqueued by the current / last frame
+    // resident CTAs per SM of the persistent kernels (occupancy queried at create time, per device)
+    int raster_ctas_per_sm, merge_ctas_per_sm, tier_ctas_per_sm[HIGS_N_TIERS];
     char err[512];
 };
 
@@ -162,8 +164,21 @@ int launch_merge(higs_ctx*, const FrameParams&, float* out_rgb, cudaStream_t);
 // ---- device helpers ----------------------------------------------------------------------------
 __device__ __forceinline__ float clampf_(float v, float lo, float hi) { return fminf(fmaxf(v, lo), hi); }
 
+// Threshold of the bounding box and of the macro-tile row scan (N-PROJ step 9):
+//   tau_s = tau * fma(cond, 2^-20, 1),  cond = (a c) / det,  det = fma(a, c, -(b b)).
+// The fp32 pixel test q <= tau is evaluated on the conic, whose cross term cancels for elongated gaussians
+// (PAPER.md:180-226), so the region it accepts leaves the covariance ellipse of tau by ~3 * 2^-24 * cond in tau;
+// everything that must be conservative with respect to the pixel test runs on tau_s.  Pinned: same ops as the oracle.
+__device__ __forceinline__ float tau_scan(float a, float b, float c, float tau)
+{
+    const float det = __fmaf_rn(a, c, -__fmul_rn(b, b));
+    const float cond = __fmul_rn(__fmul_rn(a, c), __frcp_rn(det));
+    return __fmul_rn(tau, __fmaf_rn(cond, 9.5367431640625e-07f, 1.0f));
+}
+
 // The row scan of DESIGN.md section 3 (N-SCAN): exact x-extent of the threshold ellipse
-// {q <= tau} inside each row band of a grid of cw x ch cells, clipped to [0,W] x [0,H].
+// {q <= tau_s} inside each row band of a grid of cw x ch cells, clipped to [0,W] x [0,H]; the caller passes
+// tau_s = tau_scan(a, b, c, tau).
 // Every operation is a single correctly rounded fp32 op in the written order (no contraction):
 // the set of cells it yields is part of the bit-exact contract with the oracle.
 struct RowScan {

@@ -1,6 +1,6 @@
 // project.cu -- steps a1 + a2: fused EWA projection + cull + SH colour (section 4.2), with the
 // count pass of the partitioning folded in: every persistent CTA is one partition batch
-// (the chunks of 512 consecutive ids its warps claim), keeps the private shared-memory histogram with one counter
+// (the chunks of HIGS_CHUNK = 256 consecutive ids its warps claim), keeps the private shared-memory histogram with one counter
 // per macro-tile and flushes it as one row of the N_B x N_M matrix (N_B = CTAs = a whole number per SM).  The kernel is HBM-latency-bound, so the row scan runs in issue
 // slots that were idle; the macro-tile span it finds is also packed into a 64-bit descriptor in the record, so
 // the fill pass replays it without redoing the arithmetic.  (Section 4.2:
@@ -198,8 +198,9 @@ __device__ __forceinline__ bool project_cull(const RawIn& in, const FrameParams&
     if (!((x255 > 1.0f) && (x255 <= 3.402823466e+38f))) return false;
     const float tau = __fmul_rn(2.0f, ln_spec(x255));
     if (!(tau > 0.0f)) return false;
-    // 10. off-screen cull on the threshold ellipse's bounding box
-    const float hx = __fsqrt_rn(__fmul_rn(tau, a)), hy = __fsqrt_rn(__fmul_rn(tau, c));
+    // 10. off-screen cull on the bounding box of the threshold ellipse, on tau_s (conservative for the fp32 pixel test)
+    const float tau_s = __fmul_rn(tau, __fmaf_rn(__fmul_rn(__fmul_rn(a, c), rd), 9.5367431640625e-07f, 1.0f));
+    const float hx = __fsqrt_rn(__fmul_rn(tau_s, a)), hy = __fsqrt_rn(__fmul_rn(tau_s, c));
     if (!((__fadd_rn(mux, hx) > 0.0f) && (__fsub_rn(mux, hx) < (float)P.W) &&
           (__fadd_rn(muy, hy) > 0.0f) && (__fsub_rn(muy, hy) < (float)P.H))) return false;
     s.mux = mux; s.muy = muy; s.a = a; s.b = b; s.c = c; s.A = A; s.B2 = B2; s.C = C; s.tau = tau; s.zc = zc; s.o = o;
@@ -217,7 +218,7 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
     unsigned long long desc = 0;
     {
         RowScan rs;
-        rs.init(s.mux, s.muy, s.a, s.b, s.c, s.tau, (float)HIGS_MT_H, P.n_my);
+        rs.init(s.mux, s.muy, s.a, s.b, s.c, tau_scan(s.a, s.b, s.c, s.tau), (float)HIGS_MT_H, P.n_my);
         const float fW = (float)P.W, fH = (float)P.H;
         bool fits = (rs.r1 - rs.r0) <= 3 && P.n_mx <= 511 && rs.r0 <= 511;
         desc = (unsigned long long)(uint32_t)rs.r0 | ((unsigned long long)(uint32_t)((rs.r1 - rs.r0) & 3) << 9);
@@ -248,12 +249,12 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
     bin[slot] = make_uint4(key, (uint32_t)desc, (uint32_t)(desc >> 32), (uint32_t)i);
 }
 
-// Persistent CTAs (a whole number per SM), one histogram row per CTA.  A warp claims chunks of HIGS_CHUNK = 512
+// Persistent CTAs (a whole number per SM), one histogram row per CTA.  A warp claims chunks of HIGS_CHUNK = 256
 // consecutive ids from a device counter, so the load balances itself and the grid never has a partial wave; the
 // paper's fixed partition batch of B_p consecutive ids becomes "the chunks one CTA happened to
-// claim", recorded in chunk_count's high half for the fill pass.  A warp runs phase A on 32 gaussians at a time
+// claim", listed in part_list / part_desc for the fill pass.  A warp runs phase A on 32 gaussians at a time
 // and queues the survivors (about 4 in 10 at paper scale) in shared memory; whenever 32 are queued it runs phase B
-// on them with every lane busy.  Survivor k of chunk c gets dense slot c*512 + k: slots are monotone in the
+// on them with every lane busy.  Survivor k of chunk c gets dense slot c*HIGS_CHUNK + k: slots are monotone in the
 // gaussian id, so (key, slot) order = (key, id) order (Q7).
 template <int DEG>
 __global__ void __launch_bounds__(PROJ_THREADS, 2)
@@ -374,8 +375,6 @@ static size_t project_smem_bytes(int n_m, int lcap)
 // retires early always leaves others with room (sum of capacities > chunks: every chunk finds a taker)
 int higs_part_lcap(int64_t n_chunks, int grid) { return (int)(4 * ((n_chunks + grid - 1) / grid) + 2 * PROJ_WARPS); }
 
-static int g_proj_ctas_per_sm = 2;
-
 // CTAs of the partition passes (project+count, fill) for N gaussians: a whole number per SM, fewer only when
 // there are not enough chunks to give every warp one
 int higs_part_grid(const higs_ctx* ctx, int64_t N)
@@ -417,7 +416,6 @@ int higs_project_smem_setup(higs_ctx* ctx)
     HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     int occ = 0;
     HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3>, PROJ_THREADS, (size_t)bytes));
-    g_proj_ctas_per_sm = occ < 1 ? 1 : occ;
-    ctx->n_part_max = ctx->n_sm * g_proj_ctas_per_sm;
+    ctx->n_part_max = ctx->n_sm * (occ < 1 ? 1 : occ);
     return HIGS_OK;
 }

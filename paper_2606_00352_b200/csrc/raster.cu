@@ -25,8 +25,8 @@ namespace {
 
 constexpr int RAS_THREADS = 256;                  // 3 CTAs per SM at 80 registers (4 at 64 registers measured 2 % slower)
 constexpr int RAS_WARPS = RAS_THREADS / 32;
-constexpr int RAS_SUB = HIGS_BATCH_CAP / HIGS_RASTER_SPLIT;   // gaussians per sub-unit: a unit is rasterized in parts
-constexpr int RAS_MB = RAS_SUB / 32;              // mini-batches of 32 gaussians per sub-unit
+constexpr int RAS_SUB = HIGS_BATCH_CAP;           // gaussians per unit
+constexpr int RAS_MB = RAS_SUB / 32;              // mini-batches of 32 gaussians per unit
 constexpr int MASK_PITCH = RAS_MB + 1;
 constexpr float LOGT_SCALE = 1024.0f;             // fixed point of the running log2 transmittance bounds
 constexpr int LOGT_EPS = -13608;                  // floor(log2(1e-4) * 1024): a sum below it proves T < eps
@@ -34,7 +34,7 @@ constexpr int RING = 64;                          // per-warp ring of staged-rec
 constexpr int NULL_IDX = RAS_SUB;                 // index of the "null" gaussian that pads the last drain
 
 // Shared-memory record of one staged gaussian: the first 48 B of its global record, as gathered:
-//   f4[0] = mux, muy, A, B2      f4[1] = C, tau, log2 o, r      f4[2] = g, b, -, -
+//   f4[0] = mux, muy, A, B2      f4[1] = C, tau, log2 o, r      f4[2] = g, b, cov a, cov b
 // Packed f32x2 instructions (FFMA2 / FMUL2 / FADD2) take a plain 32-bit register as a broadcast operand, so the values
 // that multiply both pixels of a lane need no duplicated copy in shared memory.
 constexpr int REC_F4 = 3;
@@ -63,22 +63,24 @@ __device__ __forceinline__ float rcp_approx(float x) { float y; asm("rcp.approx.
 __device__ __forceinline__ float sqrt_approx(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 // Conservative render-tile overlap mask of one gaussian inside macro-tile (X0, Y0) (reading Q9:
-// internal, never compared with the oracle).  Row scan of the ellipse {q <= tau} written on the conic itself:
-//   dx(dy) = -h dy +- sqrt(tau/A - D dy^2),  h = B2/(2A),  D = det/A^2,  det = A C - B2^2/4,
-// with approximate rcp/sqrt; tau is inflated by 1e-3 and every pixel centre sits 0.5 px inside its tile, which
-// dwarfs the ~1e-6 relative error of the approximations.
-__device__ __forceinline__ uint32_t tile_mask_fast(float mux, float muy, float A, float B2, float C, float tau,
-                                                   float X0, float Y0, float fW, float fH)
+// internal, never compared with the oracle).  N-SCAN at 8-px cells on the COVARIANCE (a, b, c), on the threshold
+//   tau_m = tau (1.002 + 2^-20 cond),  cond = a c / det,
+// i.e. the oracle's tau_s (the region the fp32 pixel test accepts stays inside the ellipse of tau_s, see tau_scan)
+// with 0.2 % on top.  The staged record has a, b and the conic; c and det come from the identities det = a / C,
+// c = A det, cond = A a, which do not cancel - recomputing det from the conic as A C - B2^2/4 loses all digits for
+// elongated gaussians (cond ~ 1/eps).  With approximate rcp / sqrt every extent is good to ~1e-6 relative; extents are
+// widened by 0.25 px on top, pixel centres sit 0.5 px inside their tile, and gaussians larger than 3e4 px take every tile.
+__device__ __forceinline__ uint32_t tile_mask_cov(float mux, float muy, float A, float C, float tau, float a, float b,
+                                                  float X0, float Y0, float fW, float fH)
 {
-    const float det = A * C - 0.25f * B2 * B2;
-    if (!(det > 0.0f) || !(A > 0.0f)) return 0xffffffffu;
-    tau *= 1.001f;
-    const float rA = rcp_approx(A), rdet = rcp_approx(det);
-    const float h = 0.5f * B2 * rA;
-    const float D = det * rA * rA;
-    const float tA = tau * rA;
-    const float hx = sqrt_approx(tau * C * rdet), hy = sqrt_approx(tau * A * rdet);
-    const float yR = -0.5f * B2 * sqrt_approx(tau * rdet * rcp_approx(C));   // dy of the rightmost point
+    const float det = a * rcp_approx(C);
+    const float c = A * det;
+    const float tau_m = tau * fmaf(A * a, 9.5367431640625e-07f, 1.002f);
+    const float hx = sqrt_approx(tau_m * a) + 0.25f, hy = sqrt_approx(tau_m * c) + 0.25f;
+    if (!(det > 0.0f) || !(c > 0.0f) || !(hx < 3.0e4f) || !(hy < 3.0e4f)) return 0xffffffffu;
+    const float rc = rcp_approx(c);
+    const float boc = b * rc, sdet = det * rc;
+    const float yR = b * sqrt_approx(tau_m * rcp_approx(a));          // dy of the rightmost point
     const float ytop = muy - hy, ybot = muy + hy;
     uint32_t mask = 0;
 #pragma unroll
@@ -87,10 +89,10 @@ __device__ __forceinline__ uint32_t tile_mask_fast(float mux, float muy, float A
         const float y1 = fminf(y0 + 8.0f, fH);
         const float ylo = fmaxf(y0, ytop) - muy, yhi = fminf(y1, ybot) - muy;
         if (!(yhi >= ylo)) continue;
-        const float rlo = sqrt_approx(fmaxf(0.0f, tA - D * ylo * ylo));
-        const float rhi = sqrt_approx(fmaxf(0.0f, tA - D * yhi * yhi));
-        float xmax = (ylo <= yR && yR <= yhi) ? hx : fmaxf(rlo - h * ylo, rhi - h * yhi);
-        float xmin = (ylo <= -yR && -yR <= yhi) ? -hx : fminf(-rlo - h * ylo, -rhi - h * yhi);
+        const float rlo = sqrt_approx(fmaxf(0.0f, sdet * fmaf(-ylo * ylo, rc, tau_m)));
+        const float rhi = sqrt_approx(fmaxf(0.0f, sdet * fmaf(-yhi * yhi, rc, tau_m)));
+        float xmax = (ylo <= yR && yR <= yhi) ? hx : fmaxf(fmaf(boc, ylo, rlo), fmaf(boc, yhi, rhi)) + 0.25f;
+        float xmin = (ylo <= -yR && -yR <= yhi) ? -hx : fminf(fmaf(boc, ylo, -rlo), fmaf(boc, yhi, -rhi)) - 0.25f;
         xmax = fminf(xmax + mux, fW) - X0; xmin = fmaxf(xmin + mux, 0.0f) - X0;
         if (!(xmax >= 0.0f) || !(xmin < 64.0f) || !(xmax >= xmin)) continue;
         const int c0 = max(0, (int)floorf(xmin * 0.125f)), c1 = min(7, (int)floorf(xmax * 0.125f));
@@ -100,6 +102,31 @@ __device__ __forceinline__ uint32_t tile_mask_fast(float mux, float muy, float A
     return mask;
 }
 
+// ---- cross-batch cut (not in the paper, which lets the batches behind an opaque one run) -------------
+// Every (unit, tile) publishes a TERM: log2 of the largest transmittance it left in the tile, fixed point, rounded
+// towards zero (so a sum of terms never understates the product of the transmittances).  cut_term[u][t] holds it as
+// term - 1 (< 0); 0 = not published (the buffer is zeroed every frame by k_fill).  Unit (m, j) may skip tile t when
+// the terms of batches 0 .. j-1 of macro-tile m sum below log2(eps): everything it could add sits behind T < eps.
+// The sum is taken IN BATCH ORDER and only over j' < j by construction: cut_word[m][t] = (k << 32 | sum of the terms
+// of batches 0 .. k-1) is a cache of a prefix; a reader starts from it, walks terms k, k+1, ... < j until one is
+// not published yet, and writes the longer prefix back with atomicMax (equal k means equal sum, so the largest word is
+// the longest prefix).  No ordering between units is assumed: a term that is not visible yet only loses some cut.
+__device__ __forceinline__ int cut_prefix(unsigned long long* __restrict__ word, const int* __restrict__ term_mt /* cut_term + u0*32 + t */,
+                                          uint32_t j)
+{
+    const unsigned long long w0 = __ldcg(word);
+    uint32_t k = (uint32_t)(w0 >> 32);
+    int sum = (int)(uint32_t)w0;
+    const uint32_t k0 = k;
+    while (k < j && sum >= LOGT_EPS) {
+        const int tk = __ldcg(term_mt + (size_t)k * HIGS_MT_TILES);
+        if (tk == 0) break;
+        sum += tk + 1; ++k;
+    }
+    if (k != k0) atomicMax(word, ((unsigned long long)k << 32) | (unsigned long long)(uint32_t)sum);
+    return sum;
+}
+
 template <bool COUNT>
 __global__ void __launch_bounds__(RAS_THREADS, 3)
 k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict__ rec,
@@ -107,14 +134,15 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
          const uint32_t* __restrict__ batch_offset, const uint32_t* __restrict__ unit_mt,
          const uint32_t* __restrict__ unit_order,
          const FrameParams P, FrameHeader* __restrict__ hdr,
-         float4* __restrict__ partial, uint32_t* __restrict__ unit_active, int* __restrict__ tile_logT)
+         float4* __restrict__ partial, uint32_t* __restrict__ unit_active,
+         unsigned long long* __restrict__ cut_word, int* __restrict__ cut_term)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
     RasSmem& S = *reinterpret_cast<RasSmem*>(s_raw);
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const uint32_t lt_mask = (1u << lane) - 1u;
     pdl_trigger();                                                    // k_merge_image may be scheduled as this grid drains
-    const uint32_t n_sub = hdr->n_units * HIGS_RASTER_SPLIT;
+    const uint32_t n_units = hdr->n_units;
     const bool use_cut = !(P.flags & HIGS_FLAG_NO_XBATCH_CUT);
     const float fW = (float)P.W, fH = (float)P.H;
     unsigned long long n_eval_g = 0, n_tp = 0;
@@ -128,54 +156,46 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
     for (;;) {
         __syncthreads();                                              // everyone is done with the previous unit's shared state
         // Warp 0 claims units until one has something left to show.  Tiles wholly outside the image are never active
-        // (Alg. 1 line 11, InBounds).  Cross-batch saturation cut-off: the product over the earlier units of this
-        // macro-tile of the largest transmittance they left in tile t (lane = tile) bounds the transmittance in front of
-        // this unit.  The product is kept as a running sum of fixed-point log2 values per
-        // (macro-tile, tile), each rounded towards zero, so the sum never understates the bound; units are claimed batch
-        // index major, so whatever has been added when this unit looks comes from batches in front of it.  A unit with
-        // every tile cut costs one atomic and four loads: it is never gathered.
+        // (Alg. 1 line 11, InBounds); tiles whose bound from the batches in front is below eps are cut (lane = tile).
+        // A unit with every tile cut costs one atomic and a few loads: it is never gathered.
         if (w == 0) {
-            uint32_t v_sel = 0xffffffffu, cut_sel = 0;
+            uint32_t u_sel = 0xffffffffu, cut_sel = 0;
             for (;;) {
                 uint32_t c = 0;
                 if (lane == 0) c = atomicAdd(&hdr->raster_cursor, 1u);
                 c = __shfl_sync(0xffffffffu, c, 0);
-                if (c >= n_sub) break;
-                const uint32_t vc = unit_order[c];
-                const uint32_t uc = vc / HIGS_RASTER_SPLIT, hc = vc % HIGS_RASTER_SPLIT;
+                if (c >= n_units) break;
+                const uint32_t uc = unit_order[c];
                 const uint32_t mc = unit_mt[uc];
                 const uint32_t u0c = batch_offset[mc];
-                const int lenc = min(RAS_SUB, (int)min((uint32_t)P.batch_cap, mt_count[mc] - (uc - u0c) * (uint32_t)P.batch_cap) - (int)(hc * RAS_SUB));
-                uint32_t cut = 0xffffffffu;
-                if (lenc > 0) {                                       // else: the unit ends in an earlier part
-                    const int mtx = (int)(mc % (uint32_t)P.n_mx), mty = (int)(mc / (uint32_t)P.n_mx);
-                    const int tiles_x = min(8, (P.W - mtx * HIGS_MT_W + HIGS_TILE - 1) / HIGS_TILE);
-                    const int tiles_y = min(4, (P.H - mty * HIGS_MT_H + HIGS_TILE - 1) / HIGS_TILE);
-                    bool saturated = false;
-                    if (use_cut && vc > u0c * HIGS_RASTER_SPLIT) saturated = __ldcg(tile_logT + (size_t)mc * HIGS_MT_TILES + lane) < LOGT_EPS;
-                    const bool inb = (lane & 7) < tiles_x && (lane >> 3) < tiles_y;
-                    cut = __ballot_sync(0xffffffffu, saturated || !inb);
-                }
+                const uint32_t jc = uc - u0c;
+                const int mtx = (int)(mc % (uint32_t)P.n_mx), mty = (int)(mc / (uint32_t)P.n_mx);
+                const int tiles_x = min(8, (P.W - mtx * HIGS_MT_W + HIGS_TILE - 1) / HIGS_TILE);
+                const int tiles_y = min(4, (P.H - mty * HIGS_MT_H + HIGS_TILE - 1) / HIGS_TILE);
+                bool saturated = false;
+                if (use_cut && jc > 0)
+                    saturated = cut_prefix(cut_word + (size_t)mc * HIGS_MT_TILES + lane, cut_term + (size_t)u0c * HIGS_MT_TILES + lane, jc) < LOGT_EPS;
+                const bool inb = (lane & 7) < tiles_x && (lane >> 3) < tiles_y;
+                const uint32_t cut = __ballot_sync(0xffffffffu, saturated || !inb);
                 if (cut == 0xffffffffu) {                             // nothing left to see behind the earlier batches
-                    if (lane == 0) unit_active[vc] = 0;
+                    if (lane == 0) unit_active[uc] = 0;
                     continue;
                 }
-                v_sel = vc; cut_sel = cut;
+                u_sel = uc; cut_sel = cut;
                 break;
             }
-            if (lane == 0) { S.unit = v_sel; S.cut = cut_sel; S.next_tile = 0; S.active = 0; }
+            if (lane == 0) { S.unit = u_sel; S.cut = cut_sel; S.next_tile = 0; S.active = 0; }
         }
         __syncthreads();
-        const uint32_t v = S.unit;                                    // sub-unit: part h of unit u; outputs are indexed by v
-        if (v == 0xffffffffu) break;
+        const uint32_t u = S.unit;
+        if (u == 0xffffffffu) break;
         const uint32_t cut = S.cut;
-        const uint32_t u = v / HIGS_RASTER_SPLIT, h = v % HIGS_RASTER_SPLIT;
         const uint32_t m = unit_mt[u];
         const uint32_t u0 = batch_offset[m];
         const uint32_t j = u - u0;
         const uint32_t seg_n = mt_count[m];
-        const uint32_t start = mt_offset[m] + j * (uint32_t)P.batch_cap + h * RAS_SUB;
-        const int len = min(RAS_SUB, (int)min((uint32_t)P.batch_cap, seg_n - j * (uint32_t)P.batch_cap) - (int)(h * RAS_SUB));
+        const uint32_t start = mt_offset[m] + j * (uint32_t)P.batch_cap;
+        const int len = (int)min((uint32_t)P.batch_cap, seg_n - j * (uint32_t)P.batch_cap);
         const int mtx = (int)(m % (uint32_t)P.n_mx), mty = (int)(m / (uint32_t)P.n_mx);
         const float X0 = (float)(mtx * HIGS_MT_W), Y0 = (float)(mty * HIGS_MT_H);
 
@@ -190,14 +210,14 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
         cp_async_wait_all();                                          // each thread waits for the records it asked for
         __syncthreads();
 
-        // ---- Phase 1b: per-gaussian tile masks (Alg. 1 lines 5-6), transposed by ballot; records re-laid for f32x2 ----
+        // ---- Phase 1b: per-gaussian tile masks (Alg. 1 lines 5-6), transposed by ballot ----
         for (int k = w; k < RAS_MB; k += RAS_WARPS) {
             const int i = k * 32 + lane;                              // == threadIdx.x + RAS_THREADS*(k/RAS_WARPS): the slot this thread gathered
             if (k * 32 >= len) { S.masks[lane * MASK_PITCH + k] = 0; continue; }
             uint32_t gm = 0;
             if (i < len) {
-                const float4 a = S.rec[REC_F4 * i], b = S.rec[REC_F4 * i + 1];
-                gm = tile_mask_fast(a.x, a.y, a.z, a.w, b.x, b.y, X0, Y0, fW, fH) & ~cut;
+                const float4 a = S.rec[REC_F4 * i], b = S.rec[REC_F4 * i + 1], c = S.rec[REC_F4 * i + 2];
+                gm = tile_mask_cov(a.x, a.y, a.z, b.x, b.y, c.z, c.w, X0, Y0, fW, fH) & ~cut;
             }
             uint32_t mine = 0;
 #pragma unroll
@@ -209,7 +229,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
         }
         __syncthreads();
         // tiles are handed out most-gaussians-first (the longest tile bounds the unit's tail); tiles nobody touches get
-        // no claim at all.  lane = tile.
+        // no claim at all: they publish the term of T = 1 here so that the prefix of later batches runs through.  lane = tile.
         if (w == 0) {
             uint32_t cnt = 0;
 #pragma unroll
@@ -219,6 +239,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
 #pragma unroll
             for (int o = 0; o < 32; ++o) rank += __shfl_sync(0xffffffffu, key, o) > key ? 1u : 0u;
             if (cnt) S.order[rank] = (uint8_t)lane;
+            else if (use_cut && !((cut >> lane) & 1u)) cut_term[(size_t)u * HIGS_MT_TILES + lane] = -1;
             const uint32_t nt = __popc(__ballot_sync(0xffffffffu, cnt != 0u));
             if (lane == 0) S.n_tiles = nt;
         }
@@ -292,7 +313,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             }
             __syncwarp();                                             // ring reads done before the next tile's writes
             if (COUNT) { n_tp += wr; n_eval_g += min(rd, wr); }
-            float4* out = partial + ((size_t)v * HIGS_MT_TILES + t) * 64;
+            float4* out = partial + ((size_t)u * HIGS_MT_TILES + t) * 64;
             __stcs(out + lane, make_float4(r2.x, g2.x, b2.x, T2.x));
             __stcs(out + 32 + lane, make_float4(r2.y, g2.y, b2.y, T2.y));
             float tm = fmaxf(T2.x, T2.y);
@@ -300,14 +321,14 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             for (int d = 16; d > 0; d >>= 1) tm = fmaxf(tm, __shfl_xor_sync(0xffffffffu, tm, d));
             if (lane == 0) {
                 if (use_cut) {                                        // log2 of the largest transmittance left, rounded towards zero
-                    const int q = min(0, (int)ceilf(__log2f(fmaxf(tm, 1e-30f)) * LOGT_SCALE) + 2);
-                    if (q) atomicAdd(tile_logT + (size_t)m * HIGS_MT_TILES + t, q);
+                    const int q = max(-32768, min(0, (int)ceilf(__log2f(fmaxf(tm, 1e-30f)) * LOGT_SCALE) + 2));
+                    cut_term[(size_t)u * HIGS_MT_TILES + t] = q - 1;
                 }
                 atomicOr(&S.active, 1u << t);
             }
         }
         __syncthreads();
-        if (threadIdx.x == 0) unit_active[v] = S.active;
+        if (threadIdx.x == 0) unit_active[u] = S.active;
     }
     if (COUNT && lane == 0) {                                         // both counters are warp-uniform
         atomicAdd(&hdr->n_evals, n_eval_g * 64ull);
@@ -331,7 +352,7 @@ k_merge_image(const float4* __restrict__ partial, const uint32_t* __restrict__ u
     const int y0 = mty * HIGS_MT_H + (t >> 3) * HIGS_TILE + (lane >> 3);
     if (mtx * HIGS_MT_W + (t & 7) * HIGS_TILE >= P.W || mty * HIGS_MT_H + (t >> 3) * HIGS_TILE >= P.H) return;
     uint32_t u0 = 0, nb = 0;
-    if (!hdr->overflow) { u0 = batch_offset[m] * HIGS_RASTER_SPLIT; nb = batch_offset[m + 1] * HIGS_RASTER_SPLIT - u0; }   // sub-units, in depth order
+    if (!hdr->overflow) { u0 = batch_offset[m]; nb = batch_offset[m + 1] - u0; }   // this macro-tile's units, in depth order
     float T0 = 1.0f, T1 = 1.0f, r0 = 0, g0 = 0, b0 = 0, r1 = 0, g1 = 0, b1 = 0;
     for (uint32_t j = 0; j < nb; ++j) {
         const uint32_t act = __ldg(unit_active + u0 + j);
@@ -350,8 +371,6 @@ k_merge_image(const float4* __restrict__ partial, const uint32_t* __restrict__ u
 
 } // namespace
 
-static int g_raster_ctas_per_sm = 0;
-
 int higs_raster_setup(higs_ctx* ctx)
 {
     const int smem = (int)sizeof(RasSmem);
@@ -359,20 +378,20 @@ int higs_raster_setup(higs_ctx* ctx)
     HIGS_CUDA(ctx, cudaFuncSetAttribute(k_raster<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     int occ = 0;
     HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_raster<false>, RAS_THREADS, smem));
-    g_raster_ctas_per_sm = occ > 0 ? occ : 1;
+    ctx->raster_ctas_per_sm = occ > 0 ? occ : 1;
     return HIGS_OK;
 }
 
 int launch_raster(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
 {
     const int smem = (int)sizeof(RasSmem);
-    const int grid = ctx->n_sm * g_raster_ctas_per_sm;
+    const int grid = ctx->n_sm * ctx->raster_ctas_per_sm;
     if (P.flags & HIGS_FLAG_COUNT_EVALS)
         k_raster<true><<<grid, RAS_THREADS, smem, st>>>(ctx->pairs, ctx->rec, ctx->mt_offset, ctx->mt_count, ctx->batch_offset,
-                                                        ctx->unit_mt, ctx->unit_order, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_logT);
+                                                        ctx->unit_mt, ctx->unit_order, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->cut_word, ctx->cut_term);
     else
         k_raster<false><<<grid, RAS_THREADS, smem, st>>>(ctx->pairs, ctx->rec, ctx->mt_offset, ctx->mt_count, ctx->batch_offset,
-                                                         ctx->unit_mt, ctx->unit_order, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->tile_logT);
+                                                         ctx->unit_mt, ctx->unit_order, P, ctx->hdr, ctx->partial, ctx->unit_active, ctx->cut_word, ctx->cut_term);
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }

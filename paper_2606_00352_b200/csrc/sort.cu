@@ -401,16 +401,13 @@ k_merge_levels(const OverSeg* __restrict__ over, const FrameHeader* __restrict__
     }
 }
 
-int g_merge_ctas_per_sm = 1;
-int g_tier_ctas_per_sm[HIGS_N_TIERS] = {1, 1, 1, 1};
-
 template <int THREADS>
 constexpr size_t sort_smem() { return (size_t)(THREADS * IPT + THREADS) * sizeof(u64); }
 
 template <int THREADS>
 int launch_tier(higs_ctx* ctx, int list, int tier, u64* pairs, cudaStream_t st)
 {
-    const int ctas = ctx->n_sm * g_tier_ctas_per_sm[tier];
+    const int ctas = ctx->n_sm * ctx->tier_ctas_per_sm[tier];
     k_block_sort<THREADS><<<ctas, THREADS, sort_smem<THREADS>(), st>>>(
         ctx->sort_jobs + (size_t)(list * HIGS_N_TIERS + tier) * ctx->max_jobs, ctx->hdr, list, tier, pairs, ctx->pairs_alt);
     HIGS_LAUNCHED(ctx);
@@ -423,7 +420,7 @@ int setup_tier(higs_ctx* ctx, int tier)
     HIGS_CUDA(ctx, cudaFuncSetAttribute(k_block_sort<THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_smem<THREADS>()));
     int occ = 0;
     HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_block_sort<THREADS>, THREADS, sort_smem<THREADS>()));
-    g_tier_ctas_per_sm[tier] = occ < 1 ? 1 : occ;
+    ctx->tier_ctas_per_sm[tier] = occ < 1 ? 1 : occ;
     return HIGS_OK;
 }
 
@@ -465,7 +462,7 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, b
     if ((rc = launch_tier<64>(ctx, 1, 0, pairs, ctx->aux_stream[3]))) return rc;
     const OverSeg* over = ctx->over_segs; const FrameHeader* hdr = ctx->hdr;
     void* args[] = { (void*)&over, (void*)&hdr, (void*)&pairs, (void*)&alt };
-    HIGS_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)k_merge_levels, dim3(ctx->n_sm * g_merge_ctas_per_sm), dim3(MERGE_THREADS), args, 0, st));
+    HIGS_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)k_merge_levels, dim3(ctx->n_sm * ctx->merge_ctas_per_sm), dim3(MERGE_THREADS), args, 0, st));
     ++ctx->n_launches;
     for (int k = 0; k < 4; ++k) {
         HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_join[k], ctx->aux_stream[k]));
@@ -486,7 +483,7 @@ int higs_sort_smem_setup(higs_ctx* ctx)
     HIGS_CUDA(ctx, cudaFuncSetAttribute(k_over_split, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_smem<SPLIT_THREADS>()));
     int occ = 0;
     HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_merge_levels, MERGE_THREADS, 0));
-    g_merge_ctas_per_sm = occ < 1 ? 1 : (occ > 2 ? 2 : occ);
+    ctx->merge_ctas_per_sm = occ < 1 ? 1 : (occ > 2 ? 2 : occ);
     return HIGS_OK;
 }
 
