@@ -231,7 +231,7 @@ def run_higs(args) -> int:
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    hg.higs_set_flags(ctx, 0)
+    hg.higs_set_flags(ctx, args.flags)
     for i in range(args.warmup):
         frame(i)
     barrier()
@@ -254,7 +254,7 @@ def run_higs(args) -> int:
     clocks = sampler.summary(t_mark0, t_mark1) if rank == 0 else None
 
     # -- per-stage pass: the same K views with stage events on, one sync per frame --
-    hg.higs_set_flags(ctx, hg.HIGS_FLAG_STAGE_TIMERS)
+    hg.higs_set_flags(ctx, args.flags | hg.HIGS_FLAG_STAGE_TIMERS)
     stage_names = ["project", "count", "scan", "fill", "sort", "raster", "merge", "total"]
     rows, frames_stats = [], []
     for i in range(args.steps):
@@ -267,13 +267,13 @@ def run_higs(args) -> int:
     mean_of = lambda k: float(np.mean([s[k] for s in frames_stats]))
 
     # -- instrumented pass: evaluations actually executed by the rasterizer (same views) --
-    hg.higs_set_flags(ctx, hg.HIGS_FLAG_COUNT_EVALS)
+    hg.higs_set_flags(ctx, args.flags | hg.HIGS_FLAG_COUNT_EVALS)
     evals, tile_pairs = [], []
     for i in range(min(args.steps, 8)):
         frame(args.warmup + i)
         s = hg.higs_get_stats(ctx)
         evals.append(s["n_evals"]); tile_pairs.append(s["n_tile_pairs"])
-    hg.higs_set_flags(ctx, 0)
+    hg.higs_set_flags(ctx, args.flags)
     n_evals, n_tile_pairs = float(np.mean(evals)), float(np.mean(tile_pairs))
 
     # -- rooflines (algorithmic work per launch / mean CUDA-event duration of that stage) --
@@ -348,7 +348,7 @@ def run_higs(args) -> int:
     fps_4k = None
     if not args.no_4k:
         img4 = torch.empty((2160, 3840, 3), dtype=torch.float32, device=f"cuda:{local}")
-        hg.higs_set_flags(ctx, hg.HIGS_FLAG_STAGE_TIMERS)
+        hg.higs_set_flags(ctx, args.flags | hg.HIGS_FLAG_STAGE_TIMERS)
         per_view, st4 = [], []
         my_views = [v for v in range(n_views) if v % world == rank]
         for v in my_views:
@@ -360,7 +360,7 @@ def run_higs(args) -> int:
                     ms.append(s["ms_total"])
             per_view.append(1000.0 / float(np.median(ms)))
             st4.append(s)
-        hg.higs_set_flags(ctx, 0)
+        hg.higs_set_flags(ctx, args.flags)
         pv = np.array(per_view)
         fps_4k = {"workload": "configs[4]: same scene at 3840x2160, 32 orbit views", "views": len(my_views),
                   "median": float(np.median(pv)), "min": float(pv.min()), "max": float(pv.max()),
@@ -411,6 +411,7 @@ def main() -> int:
     ap.add_argument("--impl", default="higs", choices=["higs", "reference"])
     ap.add_argument("--n", type=int, default=N_PAPER, help="gaussians in the scene (default: the paper-scale 5.8 M)")
     ap.add_argument("--batch-cap", type=int, default=1024, help="B_r, gaussians per rasterizer work unit (PAPER.md:81 fixes 1,024; smaller values for the sweep)")
+    ap.add_argument("--flags", type=int, default=0, help="extra HIGS_FLAG_* bits for every frame (4 = no cross-batch cut, 8 = merge-sort tiers)")
     ap.add_argument("--no-4k", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=16)

@@ -113,6 +113,8 @@ typedef struct {
 #define HIGS_FLAG_COUNT_EVALS   2u   /* rasterizer counts evaluations (slower; for the roofline)  */
 #define HIGS_FLAG_NO_XBATCH_CUT 4u   /* disable the cross-batch saturation cut-off:
                                         every unit then rasterizes every tile it touches          */
+#define HIGS_FLAG_RADIX_SORT    8u   /* tier kernels run the block radix sort (8-bit passes) instead of
+                                        the block merge sort; same result, measured slower on B200 (profiles/)   */
 
 /* Create a context on CUDA device `device` and preallocate all scratch (PAPER.md:83, 284:
  * "preallocated up front").  max_pairs bounds N_pairs (<= 2^31-1; 0 selects 4*max_gaussians + 65536).

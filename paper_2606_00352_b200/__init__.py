@@ -19,7 +19,7 @@ import numpy as np
 from . import build as _build
 
 HIGS_OK, HIGS_E_ARG, HIGS_E_CUDA, HIGS_E_CAPACITY, HIGS_E_NOMEM = 0, -1, -2, -3, -4
-HIGS_FLAG_STAGE_TIMERS, HIGS_FLAG_COUNT_EVALS, HIGS_FLAG_NO_XBATCH_CUT = 1, 2, 4
+HIGS_FLAG_STAGE_TIMERS, HIGS_FLAG_COUNT_EVALS, HIGS_FLAG_NO_XBATCH_CUT, HIGS_FLAG_RADIX_SORT = 1, 2, 4, 8
 HIGS_TILE, HIGS_MT_W, HIGS_MT_H, HIGS_MT_TILES, HIGS_BATCH_CAP = 8, 64, 32, 32, 1024
 
 EXPORTS = ["higs_abi_version", "higs_strerror", "higs_last_error", "higs_create", "higs_destroy", "higs_set_flags",

@@ -12,9 +12,9 @@
 #define HIGS_N_TIERS    4            // block-sort tiers, capacities 1024 / 2048 / 4096 / 8192
 #define HIGS_CHUNK      256          // consecutive ids projected by one warp; survivors are stored densely per chunk
 #define HIGS_MERGE_TILE 4096         // output items per merge-path tile (overflow path)
-#define HIGS_SPLIT_TILE 4096         // items per CTA pass of the bucket count / scatter kernels
+#define HIGS_SPLIT_TILE 2048         // items per CTA pass of the bucket count / scatter kernels
 #define HIGS_BUCKET_TARGET 1536      // mean items per depth bucket of an oversize segment
-#define HIGS_MAX_SPLIT  512          // most buckets per oversize segment (splitters live in shared memory)
+#define HIGS_MAX_SPLIT  256          // most buckets per oversize segment (splitters live in shared memory)
 
 // ---- per-frame device header: every data-dependent size lives here, never on the host ----------
 struct FrameHeader {
@@ -25,18 +25,19 @@ struct FrameHeader {
     uint32_t n_oversize;       // segments > HIGS_SORT_BLOCK: split into depth buckets first (sort.cu)
     uint32_t n_split_tiles;    // sum over oversize segments of ceil(n / HIGS_SPLIT_TILE)
     uint32_t n_buckets;        // buckets of all oversize segments
-    uint32_t n_fallback;       // buckets that still exceed HIGS_SORT_BLOCK: block sort + merge levels
-    uint32_t n_merge_tiles;    // sum over fallback buckets of ceil(n / HIGS_MERGE_TILE)
     uint32_t max_levels;       // merge levels needed by the longest fallback bucket
+    uint32_t pad0;
     uint32_t n_sort_jobs[2][HIGS_N_TIERS];   // [0] whole segments, [1] buckets of oversize segments
     uint32_t sort_cursor[2][HIGS_N_TIERS];   // work counters (persistent kernels)
-    uint32_t split_cursor[3];  // work counters of the split / count / scatter kernels
+    uint32_t split_cursor[3];  // k_oversize: work items claimed per phase (segments, tiles, tiles)
+    uint32_t split_done[3];    // k_oversize: work items finished per phase
     uint32_t raster_cursor;
     uint32_t merge_barrier;    // software grid barrier of the merge kernel
     uint32_t n_visible;
     uint32_t proj_cursor;      // chunk counter of the projection kernel
     uint32_t part_list_cursor; // entries of part_list handed out
     uint32_t pad1;
+    unsigned long long fallback_pack;   // (buckets that still exceed HIGS_SORT_BLOCK << 32 | their merge tiles): block sort + merge levels
     unsigned long long n_evals;
     unsigned long long n_tile_pairs;
 };
@@ -99,7 +100,6 @@ struct higs_ctx {
     unsigned long long* splitters;   // [max_buckets]  bucket b of a segment holds items in [splitter[b-1], splitter[b])
     uint32_t* bucket_count;    // [max_buckets]
     uint32_t* bucket_cursor;   // [max_buckets]  write position of the scatter pass
-    uint32_t* bucket_seg;      // [max_buckets]  index into split_segs
     int64_t   max_buckets;
     float4*   partial;         // [max_units][32 tiles][64 px] (r,g,b,T)
     unsigned long long* cut_word;  // [max_nm][32] cross-batch cut: (k << 32 | sum of the terms of batches 0 .. k-1), a cached prefix (raster.cu)
@@ -121,7 +121,7 @@ struct higs_ctx {
     bool timers_valid;
     int n_launches;            // kernels enqueued by the current / last frame
     // resident CTAs per SM of the persistent kernels (occupancy queried at create time, per device)
-    int raster_ctas_per_sm, merge_ctas_per_sm, tier_ctas_per_sm[HIGS_N_TIERS];
+    int raster_ctas_per_sm, merge_ctas_per_sm, over_ctas_per_sm, tier_ctas_per_sm[2][HIGS_N_TIERS];   // tiers: [0] radix, [1] merge sort
     char err[512];
 };
 

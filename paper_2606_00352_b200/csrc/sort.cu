@@ -146,41 +146,194 @@ k_block_sort(const SortJob* __restrict__ jobs, FrameHeader* __restrict__ hdr, in
     }
 }
 
-// ---- oversize segments, step 1: splitters from a sorted strided sample -------------------------------
-constexpr int SPLIT_THREADS = 512;
+// ---- block radix sort ("4 x 8-bit radix passes") ------------------------------------------
+// LSD passes of 8 bits over the bits of the depth key that actually vary inside the job (depth inside one
+// macro-tile spans a narrow range: the top bits are common, typically 3 passes instead of 4).  Ranking is
+// warp-private: a warp owns a contiguous chunk of the items and walks it 32 at a time; match.any finds the lanes
+// with the same digit, the lowest of them bumps the warp's counter of that digit, so an item's rank inside
+// (warp, digit) follows item order and the pass is stable.  A column scan over the NW x 256 counters gives the
+// global bases.  Required order is the whole 64-bit item (key, slot) (reading Q7): equal keys are rare,
+// so after the key passes runs of two equal keys are fixed by one compare-exchange; a job with a longer run of
+// equal keys (duplicate depths) is sorted again, stably, by the varying bits of the slot and then by the key.
+template <int THREADS, int IPT>
+struct RadixLayout {
+    static constexpr int NW = THREADS / 32;
+    static constexpr int CAP = THREADS * IPT;
+    static constexpr int G = THREADS >= 256 ? THREADS / 256 : 1;   // thread groups of the column scan
+    static constexpr size_t bytes = sizeof(u64) * CAP + sizeof(uint32_t) * (NW * 256 + 256 + G * 256 + 4 * NW + 4);
+    u64* buf; uint32_t* cnt; uint32_t* tot; uint32_t* grp; uint32_t* red;
+    __device__ explicit RadixLayout(unsigned char* raw)
+    {
+        buf = reinterpret_cast<u64*>(raw);
+        cnt = reinterpret_cast<uint32_t*>(buf + CAP);
+        tot = cnt + NW * 256;
+        grp = tot + 256;
+        red = grp + G * 256;
+    }
+};
 
-__global__ void __launch_bounds__(SPLIT_THREADS)
-k_over_split(const SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr, const u64* __restrict__ pairs,
-             u64* __restrict__ splitters, uint32_t* __restrict__ bucket_count, uint32_t* __restrict__ bucket_seg)
+// one stable counting pass on digit (x >> shift) & 255 of the n items in L.buf; cpw = items per warp chunk (multiple of 32)
+template <int THREADS, int IPT>
+__device__ __forceinline__ void radix_pass(const RadixLayout<THREADS, IPT>& L, int n, int cpw, int shift)
 {
-    extern __shared__ __align__(16) unsigned char s_raw[];
-    u64* buf = reinterpret_cast<u64*>(s_raw);
-    __shared__ uint32_t s_seg;
-    const int t = threadIdx.x;
-    pdl_trigger();
-    for (;;) {
-        __syncthreads();
-        if (t == 0) s_seg = atomicAdd(&hdr->split_cursor[0], 1u);
-        __syncthreads();
-        const uint32_t si = s_seg;
-        if (si >= hdr->n_oversize) return;
-        const SplitSeg sg = split[si];
-        const int m = (int)(sg.oversample * sg.nb);              // sample size, <= 8192 <= len
-        const int m_pad = ((m + IPT - 1) / IPT) * IPT;
-        const u64* src = pairs + sg.start;
-        for (int i = t; i < m_pad; i += SPLIT_THREADS)
-            buf[sidx(i)] = i < m ? src[(uint32_t)(((u64)i * sg.len) / (uint32_t)m)] : ~0ull;
-        __syncthreads();
-        block_sort_smem<SPLIT_THREADS>(buf, m, m_pad);
-        for (uint32_t b = t; b < sg.nb; b += SPLIT_THREADS) {
-            if (b + 1 < sg.nb) splitters[sg.bucket_base + b] = buf[sidx((int)((b + 1) * sg.oversample))];
-            bucket_count[sg.bucket_base + b] = 0;
-            bucket_seg[sg.bucket_base + b] = si;
+    constexpr int NW = THREADS / 32;
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    const uint32_t lt = (1u << lane) - 1u;
+    for (int i = t; i < NW * 256; i += THREADS) L.cnt[i] = 0;
+    __syncthreads();
+    const int wbeg = w * cpw, wend = min(n, wbeg + cpw);
+    uint32_t* my_cnt = L.cnt + w * 256;
+    const int kpw = cpw >> 5;                                        // items per lane (warp-uniform)
+    u64 x[IPT];
+    uint32_t off[IPT];                                               // first the peer mask, then the rank inside (warp, digit)
+#pragma unroll
+    for (int k = 0; k < IPT; ++k) {                                  // the matches of a chunk are independent: issued back to back
+        if (k < kpw) {
+            const int i = wbeg + k * 32 + lane;
+            x[k] = i < wend ? L.buf[i] : ~0ull;
+            const uint32_t dgt = i < wend ? (uint32_t)(x[k] >> shift) & 255u : 256u + (uint32_t)lane;
+            off[k] = __match_any_sync(0xffffffffu, dgt);
         }
+    }
+#pragma unroll
+    for (int k = 0; k < IPT; ++k) {                                  // in item order: the lowest lane of a digit bumps the warp's counter
+        if (k < kpw) {
+            const uint32_t peers = off[k];
+            const int leader = __ffs(peers) - 1;
+            const uint32_t dgt = (uint32_t)(x[k] >> shift) & 255u;
+            uint32_t old = 0;
+            if (lane == leader && wbeg + k * 32 + lane < wend) { old = my_cnt[dgt]; my_cnt[dgt] = old + __popc(peers); }
+            old = __shfl_sync(0xffffffffu, old, leader);
+            off[k] = old + __popc(peers & lt);
+            __syncwarp();
+        }
+    }
+    __syncthreads();
+    if constexpr (THREADS >= 256) {                                  // per digit: exclusive prefix over the warps, 8 warps per thread
+        constexpr int G = THREADS / 256;
+        const int d = t & 255, g = t >> 8;
+        uint32_t c[8], run = 0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) c[q] = L.cnt[(g * 8 + q) * 256 + d];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { const uint32_t v = c[q]; c[q] = run; run += v; }
+        if (G > 1) { L.grp[g * 256 + d] = run; __syncthreads(); }
+        uint32_t base = 0;
+#pragma unroll
+        for (int gg = 0; gg < G - 1; ++gg) if (gg < g) base += L.grp[gg * 256 + d];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) L.cnt[(g * 8 + q) * 256 + d] = base + c[q];
+        if (g == G - 1) L.tot[d] = base + run;
+    } else {
+        for (int d = t; d < 256; d += THREADS) {
+            uint32_t run = 0;
+#pragma unroll
+            for (int ww = 0; ww < NW; ++ww) { const uint32_t c = L.cnt[ww * 256 + d]; L.cnt[ww * 256 + d] = run; run += c; }
+            L.tot[d] = run;
+        }
+    }
+    __syncthreads();
+    if (w == 0) {                                                    // exclusive scan of the 256 digit totals
+        uint32_t v[8], sum = 0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { v[q] = L.tot[lane * 8 + q]; sum += v[q]; }
+        uint32_t incl = sum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += y; }
+        uint32_t run = incl - sum;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { L.tot[lane * 8 + q] = run; run += v[q]; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < IPT; ++k) {
+        if (k < kpw && wbeg + k * 32 + lane < wend) {
+            const uint32_t dgt = (uint32_t)(x[k] >> shift) & 255u;
+            L.buf[L.tot[dgt] + my_cnt[dgt] + off[k]] = x[k];
+        }
+    }
+    __syncthreads();
+}
+
+// Sorts L.buf[0 .. n) ascending as 64-bit integers, in place.  Every thread of the CTA calls it; n <= THREADS*IPT.
+template <int THREADS, int IPT>
+__device__ __forceinline__ void block_radix_sort(const RadixLayout<THREADS, IPT>& L, int n)
+{
+    constexpr int NW = THREADS / 32;
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    uint32_t kmin = 0xffffffffu, kmax = 0u;
+    for (int i = t; i < n; i += THREADS) { const uint32_t k = (uint32_t)(L.buf[i] >> 32); kmin = min(kmin, k); kmax = max(kmax, k); }
+    kmin = __reduce_min_sync(0xffffffffu, kmin); kmax = __reduce_max_sync(0xffffffffu, kmax);
+    if (lane == 0) { L.red[w] = kmin; L.red[NW + w] = kmax; }
+    __syncthreads();
+    for (int ww = 0; ww < NW; ++ww) { kmin = min(kmin, L.red[ww]); kmax = max(kmax, L.red[NW + ww]); }
+    const uint32_t kdiff = kmin ^ kmax;
+    const int nk = kdiff ? (32 - __clz(kdiff) + 7) >> 3 : 0;       // 8-bit passes over the varying key bits
+    const int cpw = ((n + NW * 32 - 1) / (NW * 32)) * 32;
+    int ns = 0;                                                      // slot passes: none in the first round
+    for (int round = 0; ; ++round) {
+#pragma unroll 1
+        for (int p = 0; p < ns + nk; ++p) radix_pass<THREADS, IPT>(L, n, cpw, p < ns ? 8 * p : 32 + 8 * (p - ns));
+        if (round == 1) return;
+        // equal keys: the thread at the start of a run of up to MAXRUN equal keys puts it in slot order by insertion
+        // (runs are disjoint); a longer run (duplicate depths) needs the slot passes
+        constexpr int MAXRUN = 16;
+        int longrun = 0;
+        for (int i = t; i + 1 < n; i += THREADS) {
+            const uint32_t k0 = (uint32_t)(L.buf[i] >> 32);
+            if (k0 != (uint32_t)(L.buf[i + 1] >> 32) || (i > 0 && (uint32_t)(L.buf[i - 1] >> 32) == k0)) continue;
+            int e = i + 2;
+            while (e < n && e - i <= MAXRUN && (uint32_t)(L.buf[e] >> 32) == k0) ++e;
+            if (e - i > MAXRUN) { longrun = 1; continue; }
+            for (int a = i + 1; a < e; ++a) {
+                const u64 v = L.buf[a];
+                int b = a - 1;
+                while (b >= i && L.buf[b] > v) { L.buf[b + 1] = L.buf[b]; --b; }
+                L.buf[b + 1] = v;
+            }
+        }
+        longrun = __syncthreads_or(longrun);
+        if (!longrun) return;
+        // second round: stable LSD over the varying slot bits, then the key bits again
+        uint32_t smin = 0xffffffffu, smax = 0u;
+        for (int i = t; i < n; i += THREADS) { const uint32_t sl = (uint32_t)L.buf[i]; smin = min(smin, sl); smax = max(smax, sl); }
+        smin = __reduce_min_sync(0xffffffffu, smin); smax = __reduce_max_sync(0xffffffffu, smax);
+        if (lane == 0) { L.red[2 * NW + w] = smin; L.red[3 * NW + w] = smax; }
+        __syncthreads();
+        for (int ww = 0; ww < NW; ++ww) { smin = min(smin, L.red[2 * NW + ww]); smax = max(smax, L.red[3 * NW + ww]); }
+        const uint32_t sdiff = smin ^ smax;
+        ns = sdiff ? (32 - __clz(sdiff) + 7) >> 3 : 0;
     }
 }
 
-// ---- oversize segments, steps 2 and 4: bucket count and scatter ----------------------------------------
+// ---- radix tier kernel: one CTA sorts one segment, one bucket, or one 8192-item block ------------------
+template <int THREADS, int IPT>
+__global__ void __launch_bounds__(THREADS)
+k_tier_radix(const SortJob* __restrict__ jobs, FrameHeader* __restrict__ hdr, int list, int tier,
+             u64* __restrict__ pairs, u64* __restrict__ pairs_alt)
+{
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    const RadixLayout<THREADS, IPT> L(s_raw);
+    __shared__ uint32_t s_job;
+    const int t = threadIdx.x;
+    for (;;) {
+        __syncthreads();
+        if (t == 0) s_job = atomicAdd(&hdr->sort_cursor[list][tier], 1u);
+        __syncthreads();
+        const uint32_t jb = s_job;
+        if (jb >= hdr->n_sort_jobs[list][tier]) return;
+        const SortJob job = jobs[jb];
+        const int n = (int)job.len;
+        const u64* gsrc = ((job.flags & 2u) ? pairs_alt : pairs) + job.start;
+        for (int i = t; i < n; i += THREADS) L.buf[i] = gsrc[i];
+        __syncthreads();
+        block_radix_sort<THREADS, IPT>(L, n);
+        u64* gdst = ((job.flags & 1u) ? pairs_alt : pairs) + job.start;
+        for (int i = t; i < n; i += THREADS) gdst[i] = L.buf[i];
+    }
+}
+
+// ---- oversize segments: one kernel, three phases ------------------------------------------
 // bucket of item x = number of splitters <= x (splitters ascending, nb - 1 of them)
 __device__ __forceinline__ uint32_t bucket_of(const u64* s_split, uint32_t n_split, u64 x)
 {
@@ -189,126 +342,164 @@ __device__ __forceinline__ uint32_t bucket_of(const u64* s_split, uint32_t n_spl
     return lo;
 }
 
-constexpr int SCAT_THREADS = 512;
-constexpr int SCAT_ITEMS = HIGS_SPLIT_TILE / SCAT_THREADS;
+constexpr int OVER_THREADS = 256;
+constexpr int SCAT_ITEMS = HIGS_SPLIT_TILE / OVER_THREADS;
+static_assert(HIGS_MAX_SPLIT <= OVER_THREADS, "one thread per bucket in the bucket scan");
+constexpr size_t OVER_BUF = sizeof(u64) * (OVER_THREADS * IPT + OVER_THREADS);    // sidx(4096) items of the sample sort
+constexpr size_t OVER_SMEM = OVER_BUF + sizeof(u64) * HIGS_MAX_SPLIT + sizeof(uint32_t) * (2 * HIGS_MAX_SPLIT + 64);
 
-// SCATTER = false: per-bucket totals.  SCATTER = true: every tile reserves its share of each bucket with one atomic
-// on the bucket cursor and writes its items there (order inside a bucket is arbitrary: the tier sort follows).
-template <bool SCATTER>
-__global__ void __launch_bounds__(SCAT_THREADS)
-k_over_buckets(const SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr, const u64* __restrict__ pairs,
-               const u64* __restrict__ splitters, uint32_t* __restrict__ bucket_count, uint32_t* __restrict__ bucket_cursor,
-               u64* __restrict__ pairs_alt)
+// last segment with tile_base <= tile
+__device__ __forceinline__ int seg_of_tile(const SplitSeg* __restrict__ split, uint32_t n_over, uint32_t tile)
 {
-    __shared__ u64 s_split[HIGS_MAX_SPLIT];
-    __shared__ uint32_t s_hist[HIGS_MAX_SPLIT];
-    __shared__ uint32_t s_base[HIGS_MAX_SPLIT];
-    __shared__ uint32_t s_tile;
-    const int t = threadIdx.x;
-    pdl_wait(); pdl_trigger();
-    const uint32_t n_over = hdr->n_oversize, n_tiles = hdr->n_split_tiles;
-    for (;;) {
-        __syncthreads();
-        if (t == 0) s_tile = atomicAdd(&hdr->split_cursor[SCATTER ? 2 : 1], 1u);
-        __syncthreads();
-        const uint32_t tile = s_tile;
-        if (tile >= n_tiles) return;
-        int lo = 0, hi = (int)n_over - 1;                         // last segment with tile_base <= tile
-        while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (split[mid].tile_base <= tile) lo = mid; else hi = mid - 1; }
-        const SplitSeg sg = split[lo];
-        for (uint32_t b = t; b < sg.nb; b += SCAT_THREADS) {
-            if (b + 1 < sg.nb) s_split[b] = splitters[sg.bucket_base + b];
-            s_hist[b] = 0;
-        }
-        __syncthreads();
-        const uint32_t o0 = (tile - sg.tile_base) * HIGS_SPLIT_TILE;
-        const u64* src = pairs + sg.start;
-        u64 x[SCAT_ITEMS]; uint32_t bk[SCAT_ITEMS], rk[SCAT_ITEMS];
-#pragma unroll
-        for (int k = 0; k < SCAT_ITEMS; ++k) {
-            const uint32_t i = o0 + k * SCAT_THREADS + t;
-            x[k] = i < sg.len ? src[i] : 0ull;
-        }
-#pragma unroll
-        for (int k = 0; k < SCAT_ITEMS; ++k) {
-            const uint32_t i = o0 + k * SCAT_THREADS + t;
-            bk[k] = 0; rk[k] = 0;
-            if (i < sg.len) {
-                bk[k] = bucket_of(s_split, sg.nb - 1, x[k]);
-                rk[k] = atomicAdd(&s_hist[bk[k]], 1u);
-            }
-        }
-        __syncthreads();
-        for (uint32_t b = t; b < sg.nb; b += SCAT_THREADS) {
-            const uint32_t h = s_hist[b];
-            if (h) {
-                if (SCATTER) s_base[b] = atomicAdd(&bucket_cursor[sg.bucket_base + b], h);
-                else atomicAdd(&bucket_count[sg.bucket_base + b], h);
-            }
-        }
-        if (SCATTER) {
-            __syncthreads();
-#pragma unroll
-            for (int k = 0; k < SCAT_ITEMS; ++k) {
-                const uint32_t i = o0 + k * SCAT_THREADS + t;
-                if (i < sg.len) pairs_alt[s_base[bk[k]] + rk[k]] = x[k];
-            }
-        }
-    }
+    int lo = 0, hi = (int)n_over - 1;
+    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (split[mid].tile_base <= tile) lo = mid; else hi = mid - 1; }
+    return lo;
 }
 
-// ---- plan B: buckets -> tier job lists (list 1), scatter cursors, fallback merge plan -------------------
-__global__ void __launch_bounds__(1024)
-k_bucket_plan(const SplitSeg* __restrict__ split, const uint32_t* __restrict__ bucket_count, const uint32_t* __restrict__ bucket_seg,
-              uint32_t* __restrict__ bucket_cursor, SortJob* __restrict__ jobs /* list 1 */, size_t max_jobs,
-              OverSeg* __restrict__ over, FrameHeader* __restrict__ hdr)
+// Phase 0: splitters of every oversize segment from a sorted strided sample.  Phase 1: per-bucket totals.
+// Phase 2: every tile reserves its share of each bucket with one atomic on the bucket cursor and writes its items
+// there in the alternate buffer (order inside a bucket is arbitrary: the tier sort follows); the CTA that owns a
+// segment's first tile turns its buckets into tier jobs (list 1).  The phases are separated by completion counters
+// (see below); the kernel replaces a chain of four dependent launches.
+__global__ void __launch_bounds__(OVER_THREADS)
+k_oversize(const SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr, const u64* __restrict__ pairs, u64* __restrict__ pairs_alt,
+           u64* __restrict__ splitters, uint32_t* __restrict__ bucket_count, uint32_t* __restrict__ bucket_cursor,
+           SortJob* __restrict__ jobs /* list 1 */, size_t max_jobs, OverSeg* __restrict__ over)
 {
-    __shared__ uint32_t s_warp[33 * 7];
-    __shared__ uint32_t s_maxlev;
-    pdl_wait(); pdl_trigger();
-    if (threadIdx.x == 0) s_maxlev = 0;
-    __syncthreads();
-    const uint32_t n_buckets = hdr->n_buckets;
-    uint32_t carry[7] = {0, 0, 0, 0, 0, 0, 0};          // tiers 0-3 (3 counts fallback blocks too), fallback buckets, merge tiles, items
-    for (uint32_t b0 = 0; b0 < n_buckets; b0 += 1024) {
-        const uint32_t b = b0 + threadIdx.x;
-        uint32_t n = 0, seg_start = 0, seg_before = 0;
-        if (b < n_buckets) {
-            n = bucket_count[b];
-            const SplitSeg sg = split[bucket_seg[b]];
-            seg_start = sg.start; seg_before = sg.items_before;
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    __shared__ uint32_t s_claim;
+    u64* buf = reinterpret_cast<u64*>(s_raw);
+    u64* s_split = reinterpret_cast<u64*>(s_raw + OVER_BUF);
+    uint32_t* s_hist = reinterpret_cast<uint32_t*>(s_split + HIGS_MAX_SPLIT);
+    uint32_t* s_base = s_hist + HIGS_MAX_SPLIT;
+    uint32_t* s_scan = s_base + HIGS_MAX_SPLIT;                     // [33] warp totals of the bucket scan
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    pdl_wait();
+    const uint32_t n_over = hdr->n_oversize, n_tiles = hdr->n_split_tiles;
+    if (n_over == 0) return;
+    // Work items of a phase are claimed from a device counter and counted when done; a CTA enters the next phase once
+    // every item of the previous one is done.  Whoever holds an item is running, so the wait cannot deadlock whether or
+    // not the whole grid is resident (the tier kernels of the whole segments share the SMs with this kernel).
+    auto claim = [&](int phase) -> uint32_t {
+        __syncthreads();
+        if (t == 0) s_claim = atomicAdd(&hdr->split_cursor[phase], 1u);
+        __syncthreads();
+        return s_claim;
+    };
+    auto done = [&](int phase) {
+        __syncthreads();
+        if (t == 0) { __threadfence(); atomicAdd(&hdr->split_done[phase], 1u); }
+    };
+    auto wait_all = [&](int phase, uint32_t n_work) {
+        if (t == 0) {
+            while (*reinterpret_cast<volatile uint32_t*>(&hdr->split_done[phase]) < n_work) __nanosleep(200);
+            __threadfence();
         }
-        uint32_t v[7] = {0, 0, 0, 0, 0, 0, n};
-        const bool fall = n > HIGS_SORT_BLOCK;
-        const int t = n >= 1 ? (fall ? 3 : tier_of(n)) : -1;     // a one-item bucket still has to travel back from the alternate buffer
-        uint32_t nc = 0, levels = 0;
-        if (fall) {
-            nc = (n + HIGS_SORT_BLOCK - 1) / HIGS_SORT_BLOCK;
-            levels = 32 - __clz(nc - 1);
-            v[3] = nc; v[4] = 1; v[5] = (n + HIGS_MERGE_TILE - 1) / HIGS_MERGE_TILE;
-            atomicMax(&s_maxlev, levels);
-        } else if (t >= 0) v[t] = 1;
-        plan_scan<7>(v, carry, s_warp);
-        if (b < n_buckets) {
-            const uint32_t start = seg_start + (v[6] - seg_before);   // buckets of a segment are consecutive, in depth order
-            bucket_cursor[b] = start;
-            if (fall) {
-                for (uint32_t c = 0; c < nc; ++c) {
-                    const uint32_t cs = c * HIGS_SORT_BLOCK;
-                    jobs[(size_t)3 * max_jobs + v[3] + c] = SortJob{start + cs, min((uint32_t)HIGS_SORT_BLOCK, n - cs), 2u | (levels & 1u), 0u};
-                }
-                over[v[4]] = OverSeg{start, n, levels, v[5]};
-            } else if (t >= 0) {
-                jobs[(size_t)t * max_jobs + v[t]] = SortJob{start, n, 2u, 0u};
-            }
+        __syncthreads();
+    };
+
+    for (;;) {
+        const uint32_t si = claim(0);
+        if (si >= n_over) break;
+        const SplitSeg sg = split[si];
+        const int m = (int)(sg.oversample * sg.nb);                  // sample size, <= 4096 <= len
+        const u64* src = pairs + sg.start;
+        __syncthreads();
+        const int m_pad = ((m + IPT - 1) / IPT) * IPT;
+        for (int i = t; i < m_pad; i += OVER_THREADS) buf[sidx(i)] = i < m ? src[(uint32_t)(((u64)i * sg.len) / (uint32_t)m)] : ~0ull;
+        __syncthreads();
+        block_sort_smem<OVER_THREADS>(buf, m, m_pad);
+        for (uint32_t b = t; b < sg.nb; b += OVER_THREADS) {
+            if (b + 1 < sg.nb) splitters[sg.bucket_base + b] = buf[sidx((int)((b + 1) * sg.oversample))];
+            bucket_count[sg.bucket_base + b] = 0;
+            bucket_cursor[sg.bucket_base + b] = 0;
         }
+        done(0);
     }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int t = 0; t < HIGS_N_TIERS; ++t) hdr->n_sort_jobs[1][t] = carry[t];
-        hdr->n_fallback = carry[4];
-        hdr->n_merge_tiles = carry[5];
-        hdr->max_levels = s_maxlev;
+    wait_all(0, n_over);
+
+    for (int phase = 1; phase <= 2; ++phase) {
+        for (;;) {
+            const uint32_t tile = claim(phase);
+            if (tile >= n_tiles) break;
+            const int si = seg_of_tile(split, n_over, tile);
+            const SplitSeg sg = split[si];
+            __syncthreads();                                          // previous tile's shared state is free
+            for (uint32_t b = t; b < sg.nb; b += OVER_THREADS) {
+                if (b + 1 < sg.nb) s_split[b] = splitters[sg.bucket_base + b];
+                s_hist[b] = 0;
+            }
+            uint32_t my_count = 0, my_start = 0;
+            if (phase == 2) {                                         // bucket b starts at the exclusive prefix of the totals (thread = bucket)
+                my_count = (uint32_t)t < sg.nb ? bucket_count[sg.bucket_base + t] : 0u;
+                uint32_t incl = my_count;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, incl, d); if (lane >= d) incl += y; }
+                if (lane == 31) s_scan[w] = incl;
+                __syncthreads();
+                if (w == 0) {
+                    const uint32_t x = lane < OVER_THREADS / 32 ? s_scan[lane] : 0u;
+                    uint32_t sc = x;
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, sc, d); if (lane >= d) sc += y; }
+                    if (lane < OVER_THREADS / 32) s_scan[lane] = sc - x;
+                }
+                __syncthreads();
+                my_start = sg.start + s_scan[w] + incl - my_count;
+            }
+            __syncthreads();
+            const uint32_t o0 = (tile - sg.tile_base) * HIGS_SPLIT_TILE;
+            const u64* src = pairs + sg.start;
+            u64 x[SCAT_ITEMS]; uint32_t bk[SCAT_ITEMS], rk[SCAT_ITEMS];
+#pragma unroll
+            for (int k = 0; k < SCAT_ITEMS; ++k) {
+                const uint32_t i = o0 + k * OVER_THREADS + t;
+                x[k] = i < sg.len ? src[i] : 0ull;
+            }
+#pragma unroll
+            for (int k = 0; k < SCAT_ITEMS; ++k) {
+                const uint32_t i = o0 + k * OVER_THREADS + t;
+                bk[k] = 0; rk[k] = 0;
+                if (i < sg.len) {
+                    bk[k] = bucket_of(s_split, sg.nb - 1, x[k]);
+                    rk[k] = atomicAdd(&s_hist[bk[k]], 1u);
+                }
+            }
+            __syncthreads();
+            if ((uint32_t)t < sg.nb) {
+                const uint32_t h = s_hist[t];
+                if (phase == 1) { if (h) atomicAdd(&bucket_count[sg.bucket_base + t], h); }
+                else s_base[t] = my_start + (h ? atomicAdd(&bucket_cursor[sg.bucket_base + t], h) : 0u);
+            }
+            if (phase == 2) {
+                __syncthreads();
+#pragma unroll
+                for (int k = 0; k < SCAT_ITEMS; ++k) {
+                    const uint32_t i = o0 + k * OVER_THREADS + t;
+                    if (i < sg.len) pairs_alt[s_base[bk[k]] + rk[k]] = x[k];
+                }
+                if (tile == sg.tile_base && (uint32_t)t < sg.nb && my_count) {   // this segment's buckets -> tier jobs
+                    const uint32_t n = my_count;
+                    if (n <= HIGS_SORT_BLOCK) {
+                        const int tr = tier_of(n);                   // a one-item bucket still has to travel back from the alternate buffer
+                        jobs[(size_t)tr * max_jobs + atomicAdd(&hdr->n_sort_jobs[1][tr], 1u)] = SortJob{my_start, n, 2u, 0u};
+                    } else {                                         // still too large: 8192-blocks + merge levels (k_merge_levels)
+                        const uint32_t nc = (n + HIGS_SORT_BLOCK - 1) / HIGS_SORT_BLOCK, levels = 32 - __clz(nc - 1);
+                        const uint32_t j0 = atomicAdd(&hdr->n_sort_jobs[1][3], nc);
+                        for (uint32_t c = 0; c < nc; ++c) {
+                            const uint32_t cs = c * HIGS_SORT_BLOCK;
+                            jobs[(size_t)3 * max_jobs + j0 + c] = SortJob{my_start + cs, min((uint32_t)HIGS_SORT_BLOCK, n - cs), 2u | (levels & 1u), 0u};
+                        }
+                        // (index, first merge tile) handed out together, so that tile_base grows with the index
+                        const unsigned long long fp = atomicAdd(&hdr->fallback_pack, (1ull << 32) | (unsigned long long)((n + HIGS_MERGE_TILE - 1) / HIGS_MERGE_TILE));
+                        over[(uint32_t)(fp >> 32)] = OverSeg{my_start, n, levels, (uint32_t)fp};
+                        atomicMax(&hdr->max_levels, levels);
+                    }
+                }
+            }
+            done(phase);
+        }
+        if (phase == 1) wait_all(1, n_tiles);
     }
 }
 
@@ -350,7 +541,8 @@ k_merge_levels(const OverSeg* __restrict__ over, const FrameHeader* __restrict__
     cg::grid_group grid = cg::this_grid();
     __shared__ u64 s_in[HIGS_MERGE_TILE];
     __shared__ int s_part[4];
-    const uint32_t n_tiles = hdr->n_merge_tiles, n_over = hdr->n_fallback, max_levels = hdr->max_levels;
+    const unsigned long long fp = hdr->fallback_pack;                 // (fallback buckets << 32 | merge tiles)
+    const uint32_t n_tiles = (uint32_t)fp, n_over = (uint32_t)(fp >> 32), max_levels = hdr->max_levels;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     for (uint32_t lev = 0; lev < max_levels; ++lev) {
         for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
@@ -404,23 +596,39 @@ k_merge_levels(const OverSeg* __restrict__ over, const FrameHeader* __restrict__
 template <int THREADS>
 constexpr size_t sort_smem() { return (size_t)(THREADS * IPT + THREADS) * sizeof(u64); }
 
-template <int THREADS>
-int launch_tier(higs_ctx* ctx, int list, int tier, u64* pairs, cudaStream_t st)
+// tier t: segments / buckets of up to 1024 << t items
+template <int TIER> struct TierCfg;
+template <> struct TierCfg<0> { static constexpr int R_THREADS = 128, R_IPT = 8,  M_THREADS = 64; };
+template <> struct TierCfg<1> { static constexpr int R_THREADS = 256, R_IPT = 8,  M_THREADS = 128; };
+template <> struct TierCfg<2> { static constexpr int R_THREADS = 512, R_IPT = 8,  M_THREADS = 256; };
+template <> struct TierCfg<3> { static constexpr int R_THREADS = 1024, R_IPT = 8, M_THREADS = 512; };
+
+template <int TIER>
+int launch_tier(higs_ctx* ctx, int list, u64* pairs, bool merge_sort, cudaStream_t st)
 {
-    const int ctas = ctx->n_sm * ctx->tier_ctas_per_sm[tier];
-    k_block_sort<THREADS><<<ctas, THREADS, sort_smem<THREADS>(), st>>>(
-        ctx->sort_jobs + (size_t)(list * HIGS_N_TIERS + tier) * ctx->max_jobs, ctx->hdr, list, tier, pairs, ctx->pairs_alt);
+    typedef TierCfg<TIER> C;
+    const SortJob* jobs = ctx->sort_jobs + (size_t)(list * HIGS_N_TIERS + TIER) * ctx->max_jobs;
+    const int ctas = ctx->n_sm * ctx->tier_ctas_per_sm[merge_sort ? 1 : 0][TIER];
+    if (merge_sort)
+        k_block_sort<C::M_THREADS><<<ctas, C::M_THREADS, sort_smem<C::M_THREADS>(), st>>>(jobs, ctx->hdr, list, TIER, pairs, ctx->pairs_alt);
+    else
+        k_tier_radix<C::R_THREADS, C::R_IPT><<<ctas, C::R_THREADS, RadixLayout<C::R_THREADS, C::R_IPT>::bytes, st>>>(jobs, ctx->hdr, list, TIER, pairs, ctx->pairs_alt);
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }
 
-template <int THREADS>
-int setup_tier(higs_ctx* ctx, int tier)
+template <int TIER>
+int setup_tier(higs_ctx* ctx)
 {
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_block_sort<THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_smem<THREADS>()));
+    typedef TierCfg<TIER> C;
     int occ = 0;
-    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_block_sort<THREADS>, THREADS, sort_smem<THREADS>()));
-    ctx->tier_ctas_per_sm[tier] = occ < 1 ? 1 : occ;
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_block_sort<C::M_THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_smem<C::M_THREADS>()));
+    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_block_sort<C::M_THREADS>, C::M_THREADS, sort_smem<C::M_THREADS>()));
+    ctx->tier_ctas_per_sm[1][TIER] = occ < 1 ? 1 : occ;
+    constexpr size_t rb = RadixLayout<C::R_THREADS, C::R_IPT>::bytes;
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_tier_radix<C::R_THREADS, C::R_IPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb));
+    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_tier_radix<C::R_THREADS, C::R_IPT>, C::R_THREADS, rb));
+    ctx->tier_ctas_per_sm[0][TIER] = occ < 1 ? 1 : occ;
     return HIGS_OK;
 }
 
@@ -429,6 +637,7 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, b
     SortJob* jobs0 = ctx->sort_jobs;
     SortJob* jobs1 = ctx->sort_jobs + (size_t)HIGS_N_TIERS * ctx->max_jobs;
     u64* alt = ctx->pairs_alt;
+    const bool ms = (ctx->flags & HIGS_FLAG_RADIX_SORT) == 0;
     int rc;
     if (!plan_done) {                                             // inside a frame k_plan has already done this (binning.cu)
         k_sort_plan<<<1, 1024, 0, st>>>(seg_offset, n_seg, jobs0, (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr);
@@ -438,33 +647,31 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, b
     // while the main stream splits the oversize segments into buckets
     HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_fork, st));
     for (int k = 0; k < 4; ++k) HIGS_CUDA(ctx, cudaStreamWaitEvent(ctx->aux_stream[k], ctx->ev_fork, 0));
-    if ((rc = launch_tier<512>(ctx, 0, 3, pairs, ctx->aux_stream[0]))) return rc;
-    if ((rc = launch_tier<256>(ctx, 0, 2, pairs, ctx->aux_stream[1]))) return rc;
-    if ((rc = launch_tier<128>(ctx, 0, 1, pairs, ctx->aux_stream[2]))) return rc;
-    if ((rc = launch_tier<64>(ctx, 0, 0, pairs, ctx->aux_stream[3]))) return rc;
-    k_over_split<<<ctx->n_sm, SPLIT_THREADS, sort_smem<SPLIT_THREADS>(), st>>>(ctx->split_segs, ctx->hdr, pairs, ctx->splitters,
-                                                                              ctx->bucket_count, ctx->bucket_seg);
-    HIGS_LAUNCHED(ctx);
-    HIGS_CUDA(ctx, launch_pdl(k_over_buckets<false>, dim3(ctx->n_sm * 2), dim3(SCAT_THREADS), 0, st, ctx->split_segs, ctx->hdr, pairs,
-                              ctx->splitters, ctx->bucket_count, ctx->bucket_cursor, alt));
-    HIGS_LAUNCHED(ctx);
-    HIGS_CUDA(ctx, launch_pdl(k_bucket_plan, dim3(1), dim3(1024), 0, st, ctx->split_segs, ctx->bucket_count, ctx->bucket_seg, ctx->bucket_cursor,
-                              jobs1, (size_t)ctx->max_jobs, ctx->over_segs, ctx->hdr));
-    HIGS_LAUNCHED(ctx);
-    HIGS_CUDA(ctx, launch_pdl(k_over_buckets<true>, dim3(ctx->n_sm * 2), dim3(SCAT_THREADS), 0, st, ctx->split_segs, ctx->hdr, pairs,
-                              ctx->splitters, ctx->bucket_count, ctx->bucket_cursor, alt));
-    HIGS_LAUNCHED(ctx);
+    {
+        const SplitSeg* split = ctx->split_segs; FrameHeader* hdr = ctx->hdr; const u64* src = pairs;
+        u64* splitters = ctx->splitters; uint32_t* bc = ctx->bucket_count; uint32_t* bcur = ctx->bucket_cursor;
+        size_t mj = (size_t)ctx->max_jobs; OverSeg* over = ctx->over_segs;
+        HIGS_CUDA(ctx, launch_pdl(k_oversize, dim3(ctx->n_sm * ctx->over_ctas_per_sm), dim3(OVER_THREADS), OVER_SMEM, st, split, hdr, src, alt, splitters, bc, bcur,
+                                  jobs1, mj, over));
+        HIGS_LAUNCHED(ctx);
+    }
+    if ((rc = launch_tier<3>(ctx, 0, pairs, ms, ctx->aux_stream[0]))) return rc;
+    if ((rc = launch_tier<2>(ctx, 0, pairs, ms, ctx->aux_stream[1]))) return rc;
+    if ((rc = launch_tier<1>(ctx, 0, pairs, ms, ctx->aux_stream[2]))) return rc;
+    if ((rc = launch_tier<0>(ctx, 0, pairs, ms, ctx->aux_stream[3]))) return rc;
     HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_fork2, st));
     for (int k = 1; k < 4; ++k) HIGS_CUDA(ctx, cudaStreamWaitEvent(ctx->aux_stream[k], ctx->ev_fork2, 0));
-    if ((rc = launch_tier<512>(ctx, 1, 3, pairs, st))) return rc;
-    if ((rc = launch_tier<256>(ctx, 1, 2, pairs, ctx->aux_stream[1]))) return rc;
-    if ((rc = launch_tier<128>(ctx, 1, 1, pairs, ctx->aux_stream[2]))) return rc;
-    if ((rc = launch_tier<64>(ctx, 1, 0, pairs, ctx->aux_stream[3]))) return rc;
+    if ((rc = launch_tier<1>(ctx, 1, pairs, ms, st))) return rc;              // buckets average HIGS_BUCKET_TARGET items: tier 1 carries most
+    if ((rc = launch_tier<0>(ctx, 1, pairs, ms, ctx->aux_stream[1]))) return rc;
+    if ((rc = launch_tier<2>(ctx, 1, pairs, ms, ctx->aux_stream[2]))) return rc;
+    if ((rc = launch_tier<3>(ctx, 1, pairs, ms, ctx->aux_stream[3]))) return rc;
+    HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_join[3], ctx->aux_stream[3]));     // the merge levels follow the 8192-blocks of tier 3
+    HIGS_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_join[3], 0));
     const OverSeg* over = ctx->over_segs; const FrameHeader* hdr = ctx->hdr;
     void* args[] = { (void*)&over, (void*)&hdr, (void*)&pairs, (void*)&alt };
     HIGS_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)k_merge_levels, dim3(ctx->n_sm * ctx->merge_ctas_per_sm), dim3(MERGE_THREADS), args, 0, st));
     ++ctx->n_launches;
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < 3; ++k) {
         HIGS_CUDA(ctx, cudaEventRecord(ctx->ev_join[k], ctx->aux_stream[k]));
         HIGS_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_join[k], 0));
     }
@@ -476,12 +683,14 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, b
 int higs_sort_smem_setup(higs_ctx* ctx)
 {
     int rc;
-    if ((rc = setup_tier<64>(ctx, 0))) return rc;
-    if ((rc = setup_tier<128>(ctx, 1))) return rc;
-    if ((rc = setup_tier<256>(ctx, 2))) return rc;
-    if ((rc = setup_tier<512>(ctx, 3))) return rc;
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_over_split, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sort_smem<SPLIT_THREADS>()));
+    if ((rc = setup_tier<0>(ctx))) return rc;
+    if ((rc = setup_tier<1>(ctx))) return rc;
+    if ((rc = setup_tier<2>(ctx))) return rc;
+    if ((rc = setup_tier<3>(ctx))) return rc;
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_oversize, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)OVER_SMEM));
     int occ = 0;
+    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_oversize, OVER_THREADS, OVER_SMEM));
+    ctx->over_ctas_per_sm = occ < 1 ? 1 : (occ > 4 ? 4 : occ);
     HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_merge_levels, MERGE_THREADS, 0));
     ctx->merge_ctas_per_sm = occ < 1 ? 1 : (occ > 2 ? 2 : occ);
     return HIGS_OK;

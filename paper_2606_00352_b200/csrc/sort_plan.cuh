@@ -67,8 +67,8 @@ __device__ __forceinline__ void sort_plan_body(const uint32_t* __restrict__ seg_
         plan_scan<8>(v, carry, s_warp);
         if (t >= 0) jobs[(size_t)t * max_jobs + v[t]] = SortJob{start, n, 0u, 0u};
         if (over) {
-            uint32_t a = 8192u / nb;                    // sample = a * nb <= 8192 items, sorted by one CTA
-            a = a > 16u ? 16u : a;                      // 16 sample items per bucket: bucket sizes within about +-25 % (1 sigma)
+            const uint32_t a = nb > 64u ? 8u : 16u;     // sample = a * nb <= 2048 items, sorted by one CTA; 16 sample items per
+                                                        // bucket keep bucket sizes within about +-25 % (1 sigma), 8 within +-35 %
             split[v[4]] = SplitSeg{start, n, nb, v[6], v[5], v[7], a, 0u};
         }
     }
@@ -80,8 +80,8 @@ __device__ __forceinline__ void sort_plan_body(const uint32_t* __restrict__ seg_
         hdr->n_oversize = carry[4];
         hdr->n_split_tiles = carry[5];
         hdr->n_buckets = carry[6];
-        hdr->n_fallback = 0; hdr->n_merge_tiles = 0; hdr->max_levels = 0;
-        hdr->split_cursor[0] = 0; hdr->split_cursor[1] = 0; hdr->split_cursor[2] = 0;
+        hdr->fallback_pack = 0ull; hdr->max_levels = 0;
+        for (int q = 0; q < 3; ++q) { hdr->split_cursor[q] = 0; hdr->split_done[q] = 0; }
     }
 }
 

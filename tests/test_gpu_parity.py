@@ -208,19 +208,27 @@ def test_host_buffer_entry_points(hg):
     hg.higs_destroy(ctx)
 
 
-def test_sort_segments_alone_against_numpy(hg):
-    """Teacher forcing of a5: random (key, id) pairs in segments of every tier size, incl. oversize and ties."""
+@pytest.mark.parametrize("flags", [0, 8])
+def test_sort_segments_alone_against_numpy(hg, flags):
+    """Teacher forcing of a5: random (key, id) pairs in segments of every tier size, incl. oversize and ties; with the
+    block merge sort (default) and with the block radix sort (HIGS_FLAG_RADIX_SORT)."""
     import torch
     rng = np.random.default_rng(9)
-    sizes = [0, 1, 2, 31, 32, 33, 1000, 1024, 1025, 2048, 3000, 4096, 5000, 8192, 8193, 20000, 70000, 7, 0, 500]
+    sizes = [0, 1, 2, 31, 32, 33, 1000, 1024, 1025, 2048, 3000, 4096, 5000, 8192, 8193, 20000, 70000, 7, 0, 500, 3000, 6000, 40000]
     off = np.concatenate([[0], np.cumsum(sizes)]).astype(np.uint32)
     n = int(off[-1])
     keys = rng.integers(0, 2 ** 32, n, dtype=np.uint64)
     keys[rng.random(n) < 0.3] = np.uint64(0x40400000)            # 30 % ties on one key
     keys[:2000] &= np.uint64(0xff)                                 # a segment whose high digits are constant
+    off_l = np.concatenate([[0], np.cumsum(sizes)])
+    a20, a21, a22 = int(off_l[20]), int(off_l[21]), int(off_l[22])
+    keys[a20:a21] = rng.integers(0x40000000, 0x40000400, a21 - a20, dtype=np.uint64)       # narrow key range: mostly runs of two or three equal keys
+    keys[a21:a22] = np.uint64(0x3f800000) + rng.integers(0, 2 ** 20, a22 - a21, dtype=np.uint64)   # depth-like keys: few ties, runs of exactly two
+    keys[a22:] = rng.integers(0x40000000, 0x40800000, n - a22, dtype=np.uint64)            # an oversize segment of depth-like keys
     ids = rng.permutation(n).astype(np.uint64)
     pairs = (keys << np.uint64(32)) | ids
     ctx = hg.higs_create(0, 1000, 1920, 1080, max_pairs=n + 10)
+    hg.higs_set_flags(ctx, flags)
     d_pairs = torch.from_numpy(pairs.view(np.int64)).cuda()
     d_off = torch.from_numpy(off.view(np.int32)).cuda()
     hg.higs_sort_segments(ctx, d_pairs, d_off)
@@ -232,7 +240,8 @@ def test_sort_segments_alone_against_numpy(hg):
     hg.higs_destroy(ctx)
 
 
-def test_sort_huge_segment_takes_bucket_fallback(hg):
+@pytest.mark.parametrize("flags", [0, 8])
+def test_sort_huge_segment_takes_bucket_fallback(hg, flags):
     """A 5 M-item segment: more than 512 buckets x 8192, so buckets exceed one block and take the merge-level path."""
     import torch
     rng = np.random.default_rng(10)
@@ -242,6 +251,7 @@ def test_sort_huge_segment_takes_bucket_fallback(hg):
     keys = rng.integers(0x3f000000, 0x41000000, n, dtype=np.uint64)
     pairs = (keys << np.uint64(32)) | rng.permutation(n).astype(np.uint64)
     ctx = hg.higs_create(0, 1000, 640, 480, max_pairs=n + 10)
+    hg.higs_set_flags(ctx, flags)
     d_pairs = torch.from_numpy(pairs.view(np.int64)).cuda()
     d_off = torch.from_numpy(off.view(np.int32)).cuda()
     hg.higs_sort_segments(ctx, d_pairs, d_off)
