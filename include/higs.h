@@ -79,7 +79,7 @@ typedef struct {
     int32_t batch_cap;       /* B_r in effect                                                     */
     int32_t overflow;        /* 1 if the frame hit HIGS_E_CAPACITY                                */
     int32_t n_launches;      /* kernels the library enqueued for the last frame (memsets excluded) */
-    int32_t reserved0;
+    int32_t tile;            /* render-tile edge in effect (8 or 16)                               */
     int64_t n_evals;         /* pixel-gaussian evaluations executed by the rasterizer; only
                                 counted when HIGS_FLAG_COUNT_EVALS is set, else 0                 */
     int64_t n_tile_pairs;    /* (gaussian, render tile) pairs that passed the inline visibility
@@ -113,6 +113,11 @@ typedef struct {
 #define HIGS_FLAG_COUNT_EVALS   2u   /* rasterizer counts evaluations (slower; for the roofline)  */
 #define HIGS_FLAG_NO_XBATCH_CUT 4u   /* disable the cross-batch saturation cut-off:
                                         every unit then rasterizes every tile it touches          */
+#define HIGS_FLAG_FP16          16u  /* fp16 data path: Cholesky conics prescaled for exp2, positions in
+                                        tile units relative to the macro-tile centre, half2 blending, fp16 RGBT partials (16 KB per
+                                        unit).  Culling, macro-tile lists and the depth sort are the same pinned fp32 code, so the
+                                        integer lists stay bit-exact; the image is accepted by PSNR against the fp32 oracle.  In
+                                        this mode higs_get_records returns valid_bits only (rec rows are not written).        */
 #define HIGS_FLAG_RADIX_SORT    8u   /* tier kernels run the block radix sort (8-bit passes) instead of
                                         the block merge sort; same result, measured slower on B200 (profiles/)   */
 
@@ -126,6 +131,10 @@ void higs_destroy(higs_ctx* ctx);
  * (tests use small B_r to force many batches per macro-tile; the paper's value is 1024). */
 int higs_set_flags(higs_ctx* ctx, uint32_t flags);
 int higs_set_batch_cap(higs_ctx* ctx, int batch_cap);
+/* Render-tile edge in pixels: 8 (default) or 16 (the variant of Table 2).  The macro-tile
+ * stays 8 x 4 render tiles, i.e. 64 x 32 or 128 x 64 px, and m = my*ceil(W/(8 tile)) + mx.  Reallocates the per-unit
+ * buffers (synchronises the device). */
+int higs_set_tile(higs_ctx* ctx, int tile);
 
 /* Render one frame.  All array arguments are DEVICE pointers:
  *   means [N][3], scales [N][3], quats [N][4], opacities [N], sh [N][(degree+1)^2][3],

@@ -71,6 +71,14 @@ def lib():
             fn.restype = C.c_int64
             fn.argtypes = [C.c_int64, u8p, u32p, f32p, f32p, f32p, f64p, C.c_int, C.c_int, C.c_int, C.c_int,
                            C.c_int, C.c_int, f64p, f64p]
+        L.orc_bin_tile.restype = C.c_int64
+        L.orc_bin_tile.argtypes = [C.c_int64, u8p, u32p, f32p, C.c_int, C.c_int, C.c_int, C.c_int, u32p, u32p, u32p, u32p, u32p, C.c_int64]
+        L.orc_render_batched_tile.restype = None
+        L.orc_render_batched_tile.argtypes = [u32p, u32p, f32p, f32p, f32p, f64p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, f64p]
+        L.orc_cholesky.restype = None
+        L.orc_cholesky.argtypes = [C.c_double, C.c_double, C.c_double, f64p]
+        L.orc_q_cholesky.restype = C.c_double
+        L.orc_q_cholesky.argtypes = [C.c_double, C.c_double, f64p]
         L.orc_render_batched.restype = None
         L.orc_render_batched.argtypes = [u32p, u32p, f32p, f32p, f32p, f64p, C.c_int, C.c_int, C.c_int, C.c_int, f64p]
         _lib = L
@@ -177,15 +185,16 @@ def scan(geo_row: np.ndarray, W: int, H: int, cw: int = MT_W, ch: int = MT_H) ->
     return out[:n].copy()
 
 
-def bin_lists(pr: Projected, B_r: int = B_R) -> Lists:
-    nmx, nmy = grid_dims(pr.W, pr.H)
+def bin_lists(pr: Projected, B_r: int = B_R, tile: int = TILE) -> Lists:
+    """O-LIST.  tile = render-tile edge (8, or 16 for the variant of PAPER.md:286-299); macro-tile = 8 x 4 tiles."""
+    nmx, nmy = (pr.W + 8 * tile - 1) // (8 * tile), (pr.H + 4 * tile - 1) // (4 * tile)
     NM = nmx * nmy
     mt_count = np.zeros(NM, np.uint32); mt_offset = np.zeros(NM + 1, np.uint32); batch_offset = np.zeros(NM + 1, np.uint32)
-    args = (pr.N, _p(pr.valid, C.c_uint8), _p(pr.key, C.c_uint32), _p(pr.geo, C.c_float), pr.W, pr.H, B_r,
+    args = (pr.N, _p(pr.valid, C.c_uint8), _p(pr.key, C.c_uint32), _p(pr.geo, C.c_float), pr.W, pr.H, B_r, tile,
             _p(mt_count, C.c_uint32), _p(mt_offset, C.c_uint32), _p(batch_offset, C.c_uint32))
-    npairs = int(lib().orc_bin(*args, None, None, 0))
+    npairs = int(lib().orc_bin_tile(*args, None, None, 0))
     keys = np.zeros(max(npairs, 1), np.uint32); ids = np.zeros(max(npairs, 1), np.uint32)
-    lib().orc_bin(*args, _p(keys, C.c_uint32), _p(ids, C.c_uint32), npairs)
+    lib().orc_bin_tile(*args, _p(keys, C.c_uint32), _p(ids, C.c_uint32), npairs)
     return Lists(npairs, int(batch_offset[NM]), mt_count, mt_offset, batch_offset, keys[:npairs], ids[:npairs])
 
 
@@ -210,14 +219,26 @@ def brute(pr: Projected, window=None, terminate: bool = True, threads: Optional[
     return _render(lib().orc_brute, pr, window, terminate, threads, want_T)
 
 
-def render_batched(pr: Projected, ls: Lists, B_r: int = B_R, terminate: bool = True) -> np.ndarray:
+def render_batched(pr: Projected, ls: Lists, B_r: int = B_R, terminate: bool = True, tile: int = TILE) -> np.ndarray:
     """The method step by step: per-macro-tile lists, batches of B_r, Eq. (1) merge."""
     out = np.zeros((pr.H, pr.W, 3), np.float64)
     ids = ls.ids if ls.ids.size else np.zeros(1, np.uint32)
-    lib().orc_render_batched(_p(ls.mt_offset, C.c_uint32), _p(ids, C.c_uint32), _p(pr.geo, C.c_float),
-                             _p(pr.conic, C.c_float), _p(pr.opac, C.c_float), _p(pr.rgb, C.c_double),
-                             pr.W, pr.H, B_r, int(terminate), _p(out, C.c_double))
+    lib().orc_render_batched_tile(_p(ls.mt_offset, C.c_uint32), _p(ids, C.c_uint32), _p(pr.geo, C.c_float),
+                                  _p(pr.conic, C.c_float), _p(pr.opac, C.c_float), _p(pr.rgb, C.c_double),
+                                  pr.W, pr.H, B_r, tile, int(terminate), _p(out, C.c_double))
     return out
+
+
+def cholesky(a: float, b: float, c: float) -> np.ndarray:
+    """(l0, l1, l2) with Sigma^-1 = L L^T, L = [[l0, 0], [l1, l2]], from the 2D covariance, fp64."""
+    l = np.zeros(3, np.float64)
+    lib().orc_cholesky(float(a), float(b), float(c), _p(l, C.c_double))
+    return l
+
+
+def q_cholesky(dx: float, dy: float, l: np.ndarray) -> float:
+    """q = (l0 dx + l1 dy)^2 + (l2 dy)^2, fp64."""
+    return float(lib().orc_q_cholesky(float(dx), float(dy), _p(np.ascontiguousarray(l, np.float64), C.c_double)))
 
 
 def render_scene(scene, cam, window=None, threads: Optional[int] = None) -> np.ndarray:

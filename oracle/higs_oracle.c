@@ -44,8 +44,7 @@
 #include <string.h>
 #include <pthread.h>
 
-#define MT_W 64   /* macro-tile = 8x4 render tiles of 8x8 px = 64x32 px */
-#define MT_H 32
+/* macro-tile = 8x4 render tiles of 8x8 px = 64x32 px, PAPER.md:73 (128x64 px in the 16x16-tile variant, Table 2) */
 #define ORC_EPS_T 1e-4   /* transmittance threshold epsilon, reading Q1 */
 #define ORC_ALPHA_MAX 0.99
 
@@ -352,11 +351,14 @@ static int cmp_u64(const void* pa, const void* pb)
     return a < b ? -1 : (a > b ? 1 : 0);
 }
 
-int64_t orc_bin(int64_t N, const uint8_t* valid, const uint32_t* key, const float* geo,
-                int W, int H, int B_r,
-                uint32_t* mt_count, uint32_t* mt_offset, uint32_t* batch_offset,
-                uint32_t* keys, uint32_t* ids, int64_t cap)
+/* tile = render-tile edge in px: 8 or 16 (the variant of Table 2); the macro-tile is
+ * always 8 x 4 render tiles, i.e. (8 tile) x (4 tile) px. */
+int64_t orc_bin_tile(int64_t N, const uint8_t* valid, const uint32_t* key, const float* geo,
+                     int W, int H, int B_r, int tile,
+                     uint32_t* mt_count, uint32_t* mt_offset, uint32_t* batch_offset,
+                     uint32_t* keys, uint32_t* ids, int64_t cap)
 {
+    const int MT_W = 8 * tile, MT_H = 4 * tile;
     const int nmx = (W + MT_W - 1) / MT_W, nmy = (H + MT_H - 1) / MT_H, NM = nmx * nmy;
     int32_t* cells = (int32_t*)malloc(sizeof(int32_t) * (size_t)NM);
     memset(mt_count, 0, sizeof(uint32_t) * (size_t)NM);
@@ -389,6 +391,14 @@ int64_t orc_bin(int64_t N, const uint8_t* valid, const uint32_t* key, const floa
     }
     free(cells);
     return npairs;
+}
+
+int64_t orc_bin(int64_t N, const uint8_t* valid, const uint32_t* key, const float* geo,
+                int W, int H, int B_r,
+                uint32_t* mt_count, uint32_t* mt_offset, uint32_t* batch_offset,
+                uint32_t* keys, uint32_t* ids, int64_t cap)
+{
+    return orc_bin_tile(N, valid, key, geo, W, H, B_r, 8, mt_count, mt_offset, batch_offset, keys, ids, cap);
 }
 
 /* ---------------------------------------------------------------------------------------
@@ -553,10 +563,11 @@ int64_t orc_brute(int64_t N, const uint8_t* valid, const uint32_t* key, const fl
  * terminate=1 stops a pixel once the running product of transmittances drops below 1e-4.
  * Full image only; pixel-major, slow: small scenes only.  out: H*W*3 fp64.
  * ------------------------------------------------------------------------------------- */
-void orc_render_batched(const uint32_t* mt_offset, const uint32_t* ids, const float* geo,
-                        const float* conic, const float* opac, const double* rgb,
-                        int W, int H, int B_r, int terminate, double* out)
+void orc_render_batched_tile(const uint32_t* mt_offset, const uint32_t* ids, const float* geo,
+                             const float* conic, const float* opac, const double* rgb,
+                             int W, int H, int B_r, int tile, int terminate, double* out)
 {
+    const int MT_W = 8 * tile, MT_H = 4 * tile;
     const int nmx = (W + MT_W - 1) / MT_W, nmy = (H + MT_H - 1) / MT_H;
     for (int my = 0; my < nmy; ++my) for (int mx = 0; mx < nmx; ++mx) {
         const int m = my * nmx + mx;
@@ -584,6 +595,34 @@ void orc_render_batched(const uint32_t* mt_offset, const uint32_t* ids, const fl
             out[3 * pix] = C[0]; out[3 * pix + 1] = C[1]; out[3 * pix + 2] = C[2];
         }
     }
+}
+
+void orc_render_batched(const uint32_t* mt_offset, const uint32_t* ids, const float* geo,
+                        const float* conic, const float* opac, const double* rgb,
+                        int W, int H, int B_r, int terminate, double* out)
+{
+    orc_render_batched_tile(mt_offset, ids, geo, conic, opac, rgb, W, H, B_r, 8, terminate, out);
+}
+
+/* ---------------------------------------------------------------------------------------
+ * Cholesky form of the inverse covariance (section 3.5):
+ *     Sigma^-1 = L L^T,  L = [[l0, 0], [l1, l2]],   q = (l0 dx + l1 dy)^2 + (l2 dy)^2.
+ * From the covariance (a, b, c), det = a c - b^2:  l0 = sqrt(c / det), l1 = -b / (det l0),
+ * l2 = 1 / sqrt(c)  (so that l0^2 = A, l0 l1 = B2 / 2, l1^2 + l2^2 = C).  fp64.
+ * Used by the tests of the fp16 data path (SURVEY.md 8(c) "Cholesky identity"); O-IMG does not use it.
+ * ------------------------------------------------------------------------------------- */
+void orc_cholesky(double a, double b, double c, double* l)
+{
+    const double det = a * c - b * b;
+    l[0] = sqrt(c / det);
+    l[1] = -b / (det * l[0]);
+    l[2] = 1.0 / sqrt(c);
+}
+
+double orc_q_cholesky(double dx, double dy, const double* l)
+{
+    const double t1 = l[0] * dx + l[1] * dy, t2 = l[2] * dy;
+    return t1 * t1 + t2 * t2;
 }
 
 int orc_abi_version(void) { return 1; }

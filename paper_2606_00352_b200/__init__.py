@@ -19,11 +19,11 @@ import numpy as np
 from . import build as _build
 
 HIGS_OK, HIGS_E_ARG, HIGS_E_CUDA, HIGS_E_CAPACITY, HIGS_E_NOMEM = 0, -1, -2, -3, -4
-HIGS_FLAG_STAGE_TIMERS, HIGS_FLAG_COUNT_EVALS, HIGS_FLAG_NO_XBATCH_CUT, HIGS_FLAG_RADIX_SORT = 1, 2, 4, 8
+HIGS_FLAG_STAGE_TIMERS, HIGS_FLAG_COUNT_EVALS, HIGS_FLAG_NO_XBATCH_CUT, HIGS_FLAG_RADIX_SORT, HIGS_FLAG_FP16 = 1, 2, 4, 8, 16
 HIGS_TILE, HIGS_MT_W, HIGS_MT_H, HIGS_MT_TILES, HIGS_BATCH_CAP = 8, 64, 32, 32, 1024
 
 EXPORTS = ["higs_abi_version", "higs_strerror", "higs_last_error", "higs_create", "higs_destroy", "higs_set_flags",
-           "higs_set_batch_cap", "higs_render", "higs_render_host", "higs_scene_upload", "higs_render_view_host",
+           "higs_set_batch_cap", "higs_set_tile", "higs_render", "higs_render_host", "higs_scene_upload", "higs_render_view_host",
            "higs_render_view", "higs_get_stats", "higs_get_lists", "higs_get_records", "higs_sort_segments", "higs_download"]
 
 
@@ -35,7 +35,7 @@ class higs_camera(C.Structure):
 class higs_stats(C.Structure):
     _fields_ = [("n_gaussians", C.c_int64), ("n_visible", C.c_int64), ("n_pairs", C.c_int64), ("n_units", C.c_int64),
                 ("max_segment", C.c_int64), ("n_oversize", C.c_int64), ("n_mt_x", C.c_int32), ("n_mt_y", C.c_int32),
-                ("batch_cap", C.c_int32), ("overflow", C.c_int32), ("n_launches", C.c_int32), ("reserved0", C.c_int32), ("n_evals", C.c_int64), ("n_tile_pairs", C.c_int64),
+                ("batch_cap", C.c_int32), ("overflow", C.c_int32), ("n_launches", C.c_int32), ("tile", C.c_int32), ("n_evals", C.c_int64), ("n_tile_pairs", C.c_int64),
                 ("ms_project", C.c_float), ("ms_count", C.c_float), ("ms_scan", C.c_float), ("ms_fill", C.c_float),
                 ("ms_sort", C.c_float), ("ms_raster", C.c_float), ("ms_merge", C.c_float), ("ms_total", C.c_float)]
 
@@ -80,6 +80,7 @@ def load() -> C.CDLL:
         L.higs_destroy.restype = None; L.higs_destroy.argtypes = [vp]
         L.higs_set_flags.restype = C.c_int; L.higs_set_flags.argtypes = [vp, C.c_uint32]
         L.higs_set_batch_cap.restype = C.c_int; L.higs_set_batch_cap.argtypes = [vp, C.c_int]
+        L.higs_set_tile.restype = C.c_int; L.higs_set_tile.argtypes = [vp, C.c_int]
         L.higs_render.restype = C.c_int
         L.higs_render.argtypes = [vp, f32p, f32p, f32p, f32p, f32p, C.c_int, C.c_int64, C.POINTER(higs_camera),
                                   C.c_int, C.c_int, f32p, vp]
@@ -155,6 +156,10 @@ def higs_set_flags(ctx, flags: int) -> None:
 
 def higs_set_batch_cap(ctx, batch_cap: int) -> None:
     _check(load().higs_set_batch_cap(ctx, batch_cap), "higs_set_batch_cap", ctx)
+
+
+def higs_set_tile(ctx, tile: int) -> None:
+    _check(load().higs_set_tile(ctx, tile), "higs_set_tile", ctx)
 
 
 def higs_render(ctx, means, scales, quats, opacities, sh, degree: int, cam: higs_camera, W: int, H: int, out_rgb,
@@ -247,9 +252,11 @@ class Renderer:
     """Owns a higs_ctx.  render(scene tensors on the device, camera) -> (H, W, 3) fp32 device tensor."""
 
     def __init__(self, max_gaussians: int, max_W: int, max_H: int, max_pairs: int = 0, device: int = 0,
-                 flags: int = 0, batch_cap: int = HIGS_BATCH_CAP):
+                 flags: int = 0, batch_cap: int = HIGS_BATCH_CAP, tile: int = HIGS_TILE):
         self.ctx = higs_create(device, max_gaussians, max_W, max_H, max_pairs)
         self.device = device
+        if tile != HIGS_TILE:
+            higs_set_tile(self.ctx, tile)
         if flags:
             higs_set_flags(self.ctx, flags)
         if batch_cap != HIGS_BATCH_CAP:

@@ -42,7 +42,7 @@ int alloc_unit_buffers(higs_ctx* ctx)
     if ((rc = dev_alloc(ctx, &ctx->unit_order, (size_t)ctx->max_units))) return rc;
     if ((rc = dev_alloc(ctx, &ctx->level_hist, (size_t)ctx->max_units + 2))) return rc;
     if ((rc = dev_alloc(ctx, &ctx->level_cur, (size_t)ctx->max_units + 2))) return rc;
-    if ((rc = dev_alloc(ctx, &ctx->partial, (size_t)ctx->max_units * HIGS_MT_TILES * 64))) return rc;
+    if ((rc = dev_alloc(ctx, &ctx->partial, (size_t)ctx->max_units * HIGS_MT_TILES * ctx->tile * ctx->tile))) return rc;   // float4 per pixel
     if ((rc = dev_alloc(ctx, &ctx->cut_term, (size_t)ctx->max_units * HIGS_MT_TILES))) return rc;
     return HIGS_OK;
 }
@@ -53,7 +53,8 @@ int check_frame_args(higs_ctx* ctx, int degree, int64_t N, const higs_camera* ca
     if (degree < 0 || degree > 3) return HIGS_E_ARG;
     if (N < 0 || N > ctx->max_gaussians) return HIGS_E_ARG;
     if (W <= 0 || H <= 0 || W > ctx->max_W || H > ctx->max_H) return HIGS_E_ARG;
-    const int64_t nm = (int64_t)((W + HIGS_MT_W - 1) / HIGS_MT_W) * ((H + HIGS_MT_H - 1) / HIGS_MT_H);
+    const int mw = 8 * ctx->tile, mh = 4 * ctx->tile;
+    const int64_t nm = (int64_t)((W + mw - 1) / mw) * ((H + mh - 1) / mh);
     if (nm > ctx->max_nm) return HIGS_E_ARG;
     return HIGS_OK;
 }
@@ -68,7 +69,8 @@ int render_impl(higs_ctx* ctx, const float* means, const float* scales, const fl
     P.fx = cam->fx; P.fy = cam->fy; P.cx = cam->cx; P.cy = cam->cy; P.near_z = cam->near_z;
     memcpy(P.cam, cam->cam_pos, sizeof(P.cam));
     P.W = W; P.H = H;
-    P.n_mx = (W + HIGS_MT_W - 1) / HIGS_MT_W; P.n_my = (H + HIGS_MT_H - 1) / HIGS_MT_H; P.n_m = P.n_mx * P.n_my;
+    P.tile = ctx->tile;
+    P.n_mx = (W + 8 * P.tile - 1) / (8 * P.tile); P.n_my = (H + 4 * P.tile - 1) / (4 * P.tile); P.n_m = P.n_mx * P.n_my;
     P.degree = degree; P.batch_cap = ctx->batch_cap; P.flags = ctx->flags;
     P.max_pairs = (uint32_t)ctx->max_pairs; P.max_units = (uint32_t)ctx->max_units;
     const bool timers = (ctx->flags & HIGS_FLAG_STAGE_TIMERS) != 0;
@@ -164,7 +166,7 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     if (!ctx) return HIGS_E_NOMEM;
     memset(ctx, 0, sizeof(*ctx));
     ctx->device = device; ctx->max_gaussians = max_gaussians; ctx->max_W = max_W; ctx->max_H = max_H;
-    ctx->max_nm = (int)nm; ctx->max_pairs = max_pairs; ctx->batch_cap = HIGS_BATCH_CAP; ctx->flags = 0;
+    ctx->max_nm = (int)nm; ctx->max_pairs = max_pairs; ctx->batch_cap = HIGS_BATCH_CAP; ctx->flags = 0; ctx->tile = HIGS_TILE;
     int rc = HIGS_OK;
     auto fail = [&](int code) { higs_destroy(ctx); return code; };
     if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return fail(HIGS_E_CUDA); }
@@ -177,6 +179,7 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     if ((rc = dev_alloc(ctx, &ctx->valid_bits, (size_t)(n + 31) / 32 + 1))) return fail(rc);
     const size_t n_slots = (size_t)ctx->n_chunks_max * HIGS_CHUNK;
     if ((rc = dev_alloc(ctx, &ctx->rec, n_slots * 4))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->rec16, n_slots * 2))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->bin, n_slots))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->chunk_count, (size_t)ctx->n_chunks_max))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->part_list, (size_t)ctx->n_chunks_max))) return fail(rc);
@@ -226,7 +229,7 @@ void higs_destroy(higs_ctx* ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaDeviceSynchronize();
-    dev_free(ctx->valid_bits); dev_free(ctx->rec); dev_free(ctx->bin); dev_free(ctx->chunk_count); dev_free(ctx->part_list); dev_free(ctx->part_desc); dev_free(ctx->rec_export); dev_free(ctx->hist); dev_free(ctx->hdr_block);
+    dev_free(ctx->valid_bits); dev_free(ctx->rec); dev_free(ctx->rec16); dev_free(ctx->bin); dev_free(ctx->chunk_count); dev_free(ctx->part_list); dev_free(ctx->part_desc); dev_free(ctx->rec_export); dev_free(ctx->hist); dev_free(ctx->hdr_block);
     dev_free(ctx->mt_offset); dev_free(ctx->batch_offset); dev_free(ctx->unit_mt);
     dev_free(ctx->unit_active); dev_free(ctx->pairs); dev_free(ctx->pairs_alt); dev_free(ctx->sort_jobs);
     dev_free(ctx->over_segs); dev_free(ctx->split_segs); dev_free(ctx->splitters); dev_free(ctx->bucket_count);
@@ -261,6 +264,16 @@ int higs_set_batch_cap(higs_ctx* ctx, int batch_cap)
     HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
     HIGS_CUDA(ctx, cudaDeviceSynchronize());
     ctx->batch_cap = batch_cap;
+    return alloc_unit_buffers(ctx);
+}
+
+int higs_set_tile(higs_ctx* ctx, int tile)
+{
+    if (!ctx || (tile != 8 && tile != 16)) return HIGS_E_ARG;
+    if (tile == ctx->tile) return HIGS_OK;
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    HIGS_CUDA(ctx, cudaDeviceSynchronize());
+    ctx->tile = tile;
     return alloc_unit_buffers(ctx);
 }
 
@@ -340,7 +353,7 @@ int higs_get_stats(higs_ctx* ctx, higs_stats* out)
     out->n_gaussians = ctx->last_n; out->n_visible = h.n_visible; out->n_pairs = h.n_pairs; out->n_units = h.n_units;
     out->max_segment = h.max_segment; out->n_oversize = h.n_oversize;
     out->n_mt_x = ctx->last_mx; out->n_mt_y = ctx->last_my; out->batch_cap = ctx->batch_cap; out->overflow = (int32_t)h.overflow;
-    out->n_launches = ctx->n_launches;
+    out->n_launches = ctx->n_launches; out->tile = ctx->tile;
     out->n_evals = (int64_t)h.n_evals; out->n_tile_pairs = (int64_t)h.n_tile_pairs;
     if (ctx->timers_valid) {
         float* dst[7] = { &out->ms_project, &out->ms_count, &out->ms_scan, &out->ms_fill, &out->ms_sort, &out->ms_raster, &out->ms_merge };

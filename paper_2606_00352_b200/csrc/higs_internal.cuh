@@ -55,6 +55,7 @@ struct FrameParams {
     int   n_mx, n_my, n_m;
     int   degree;
     int   batch_cap;
+    int   tile;                // render-tile edge, 8 or 16; macro-tile = 8 x 4 tiles
     uint32_t flags;
     uint32_t max_pairs, max_units;
 };
@@ -69,11 +70,14 @@ struct higs_ctx {
     int n_sm;
     uint32_t flags;
     int batch_cap;
+    int tile;                  // render-tile edge in effect (8 or 16)
     // scratch (device)
     uint32_t* valid_bits;      // [ceil(maxN/32)]
     float4*   rec;             // [slots][4]  mux,muy,A,B2 | C,tau,log2o,r | g,b,a,b | c,bits(key),id,-   (64 B; the rasterizer gathers the
                                //             first 48 B).  A slot is the dense position of a surviving gaussian: survivor k of the
                                //             HIGS_CHUNK-id chunk c sits at c*HIGS_CHUNK + k (monotone in the id)
+    uint4*    rec16;           // [slots][2]  fp16 data path (HIGS_FLAG_FP16): mux, muy (fp32) | half2 (l0', l1') | half2 (l2', o) ;
+                               //             half2 (r, g) | half2 (b, 0) | - | -   (32 B = one sector)
     uint4*    bin;             // [slots]     bits(key), span descriptor lo, hi, id   (16 B, read by fill)
     uint32_t* chunk_count;     // [chunks]    survivors of the chunk
     uint32_t* part_list;       // [chunks]    chunk ids grouped by the partition CTA that claimed them
@@ -121,7 +125,7 @@ struct higs_ctx {
     bool timers_valid;
     int n_launches;            // kernels enqueued by the current / last frame
     // resident CTAs per SM of the persistent kernels (occupancy queried at create time, per device)
-    int raster_ctas_per_sm, merge_ctas_per_sm, over_ctas_per_sm, tier_ctas_per_sm[2][HIGS_N_TIERS];   // tiers: [0] radix, [1] merge sort
+    int raster_ctas_per_sm[2][2], merge_ctas_per_sm, over_ctas_per_sm, tier_ctas_per_sm[2][HIGS_N_TIERS];   // tiers: [0] radix, [1] merge sort
     char err[512];
 };
 

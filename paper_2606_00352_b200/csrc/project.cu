@@ -14,6 +14,7 @@
 // the pinned fp32 sequence N-PROJ of DESIGN.md section 3, one correctly rounded op per written op:
 // the __f*_rn intrinsics are never contracted into FMAs by nvcc.
 #include <stdio.h>
+#include <cuda_fp16.h>
 #include "higs_internal.cuh"
 
 // inputs go through the read-only L1 path: consecutive loads of a warp share sectors (12-byte strides, halves of a
@@ -210,22 +211,22 @@ __device__ __forceinline__ bool project_cull(const RawIn& in, const FrameParams&
 
 // Phase B for one survivor: a2 macro-tile row scan (N-SCAN, pinned) -> private histogram + span descriptor,
 // SH colour, and the two records at dense slot `slot`.
-template <int DEG>
+template <int DEG, bool HALF>
 __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size_t slot, const float* __restrict__ sh,
                                               const FrameParams& P, uint32_t* s_hist, float4* __restrict__ rec,
-                                              uint4* __restrict__ bin)
+                                              uint4* __restrict__ rec16, uint4* __restrict__ bin)
 {
     unsigned long long desc = 0;
     {
         RowScan rs;
-        rs.init(s.mux, s.muy, s.a, s.b, s.c, tau_scan(s.a, s.b, s.c, s.tau), (float)HIGS_MT_H, P.n_my);
+        rs.init(s.mux, s.muy, s.a, s.b, s.c, tau_scan(s.a, s.b, s.c, s.tau), (float)(4 * P.tile), P.n_my);
         const float fW = (float)P.W, fH = (float)P.H;
         bool fits = (rs.r1 - rs.r0) <= 3 && P.n_mx <= 511 && rs.r0 <= 511;
         desc = (unsigned long long)(uint32_t)rs.r0 | ((unsigned long long)(uint32_t)((rs.r1 - rs.r0) & 3) << 9);
         for (int r = rs.r0; r <= rs.r1; ++r) {
             int m0, m1;
             uint32_t field = 511u;
-            if (rs.row(r, (float)HIGS_MT_W, (float)HIGS_MT_H, fW, fH, P.n_mx, m0, m1)) {
+            if (rs.row(r, (float)(8 * P.tile), (float)(4 * P.tile), fW, fH, P.n_mx, m0, m1)) {
                 for (int m = m0; m <= m1; ++m) atomicAdd(&s_hist[r * P.n_mx + m], 1u);
                 fits = fits && (m1 - m0) <= 15;
                 field = (uint32_t)m0 | ((uint32_t)((m1 - m0) & 15) << 9);
@@ -241,11 +242,26 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
     float r, g, bl;
     sh_accumulate<DEG>(sh + i * (int64_t)((DEG + 1) * (DEG + 1) * 3), dx * rl, dy * rl, dz * rl, r, g, bl);
     const uint32_t key = __float_as_uint(s.zc);
-    float4* rp = rec + 4 * slot;
-    rp[0] = make_float4(s.mux, s.muy, s.A, s.B2);
-    rp[1] = make_float4(s.C, s.tau, log2f(s.o), r);
-    rp[2] = make_float4(g, bl, s.a, s.b);
-    rp[3] = make_float4(s.c, __uint_as_float(key), __uint_as_float((uint32_t)i), 0.0f);
+    if constexpr (HALF) {
+        // fp16 data path: inverse covariance as Cholesky factors L = [[l0, 0], [l1, l2]], L L^T = conic,
+        // from the covariance without cancellation: l0 = sqrt(c / det), l1 = -b / (det l0), l2 = 1 / sqrt(c); prescaled by
+        // sqrt(log2 e / 2) * tile so that alpha = o * exp2(-q') with q' = (l0' dx + l1' dy)^2 + (l2' dy)^2 in tile units
+        const float det = __fmaf_rn(s.a, s.c, -__fmul_rn(s.b, s.b));
+        const float l0 = sqrtf(s.c / det), l2 = rsqrtf(s.c);
+        const float l1 = -s.b / (det * l0);
+        const float ks = 0.84932180f * (float)P.tile;                // sqrt(log2(e) / 2) * tile_size
+        const __half2 h01 = __floats2half2_rn(l0 * ks, l1 * ks), h2o = __floats2half2_rn(l2 * ks, s.o);
+        const __half2 hrg = __floats2half2_rn(r, g), hb = __floats2half2_rn(bl, 0.0f);
+        rec16[2 * slot] = make_uint4(__float_as_uint(s.mux), __float_as_uint(s.muy), *reinterpret_cast<const uint32_t*>(&h01), *reinterpret_cast<const uint32_t*>(&h2o));
+        rec16[2 * slot + 1] = make_uint4(*reinterpret_cast<const uint32_t*>(&hrg), *reinterpret_cast<const uint32_t*>(&hb), 0u, 0u);
+    }
+    if (!HALF || desc == HIGS_DESC_FALLBACK) {                       // fp16 path: the fill pass reads rec only to redo the row scan of wide gaussians
+        float4* rp = rec + 4 * slot;
+        rp[0] = make_float4(s.mux, s.muy, s.A, s.B2);
+        rp[1] = make_float4(s.C, s.tau, log2f(s.o), r);
+        rp[2] = make_float4(g, bl, s.a, s.b);
+        rp[3] = make_float4(s.c, __uint_as_float(key), __uint_as_float((uint32_t)i), 0.0f);
+    }
     bin[slot] = make_uint4(key, (uint32_t)desc, (uint32_t)(desc >> 32), (uint32_t)i);
 }
 
@@ -256,11 +272,11 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
 // and queues the survivors (about 4 in 10 at paper scale) in shared memory; whenever 32 are queued it runs phase B
 // on them with every lane busy.  Survivor k of chunk c gets dense slot c*HIGS_CHUNK + k: slots are monotone in the
 // gaussian id, so (key, slot) order = (key, id) order (Q7).
-template <int DEG>
+template <int DEG, bool HALF>
 __global__ void __launch_bounds__(PROJ_THREADS, 2)
 k_project(const float* __restrict__ means, const float* __restrict__ scales, const float* __restrict__ quats,
           const float* __restrict__ opac, const float* __restrict__ sh, int64_t N, const FrameParams P,
-          uint32_t* __restrict__ valid_bits, float4* __restrict__ rec, uint4* __restrict__ bin,
+          uint32_t* __restrict__ valid_bits, float4* __restrict__ rec, uint4* __restrict__ rec16, uint4* __restrict__ bin,
           uint32_t* __restrict__ chunk_count, uint32_t* __restrict__ hist, uint32_t* __restrict__ mt_count, uint32_t* __restrict__ part_list,
           uint2* __restrict__ part_desc, int lcap, FrameHeader* __restrict__ hdr)
 {
@@ -302,7 +318,7 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
                 s.tau = q[8 * PROJ_QCAP + e]; s.zc = q[9 * PROJ_QCAP + e]; s.o = q[10 * PROJ_QCAP + e];
                 s.mx = q[11 * PROJ_QCAP + e]; s.my = q[12 * PROJ_QCAP + e]; s.mz = q[13 * PROJ_QCAP + e];
                 s.local = __float_as_uint(q[14 * PROJ_QCAP + e]);
-                emit_survivor<DEG>(s, c0 + s.local, slot0 + head + lane, sh, P, s_hist, rec, bin);
+                emit_survivor<DEG, HALF>(s, c0 + s.local, slot0 + head + lane, sh, P, s_hist, rec, rec16, bin);
             }
             head += n_live;
             __syncwarp();
@@ -392,8 +408,9 @@ int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, cons
     const unsigned grid = (unsigned)higs_part_grid(ctx, N);
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, (int)grid);
     const size_t smem = project_smem_bytes(P.n_m, lcap);
-#define HIGS_PROJ(D) k_project<D><<<grid, PROJ_THREADS, smem, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
-                                                                   ctx->bin, ctx->chunk_count, ctx->hist, ctx->mt_count, ctx->part_list, ctx->part_desc, lcap, ctx->hdr)
+#define HIGS_PROJ_(D, H) k_project<D, H><<<grid, PROJ_THREADS, smem, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
+                                                                   ctx->rec16, ctx->bin, ctx->chunk_count, ctx->hist, ctx->mt_count, ctx->part_list, ctx->part_desc, lcap, ctx->hdr)
+#define HIGS_PROJ(D) do { if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(D, true); else HIGS_PROJ_(D, false); } while (0)
     switch (P.degree) {
         case 0: HIGS_PROJ(0); break;
         case 1: HIGS_PROJ(1); break;
@@ -401,6 +418,7 @@ int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, cons
         default: HIGS_PROJ(3); break;
     }
 #undef HIGS_PROJ
+#undef HIGS_PROJ_
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }
@@ -410,12 +428,16 @@ int higs_project_smem_setup(higs_ctx* ctx)
     // worst case for the list: the full grid on max_gaussians (a smaller grid has at most 16 chunks per CTA)
     const int lcap_max = higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) > 6 * PROJ_WARPS ? higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) : 6 * PROJ_WARPS;
     const int bytes = (int)project_smem_bytes(ctx->max_nm, lcap_max);
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     int occ = 0;
-    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3>, PROJ_THREADS, (size_t)bytes));
+    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3, false>, PROJ_THREADS, (size_t)bytes));
     ctx->n_part_max = ctx->n_sm * (occ < 1 ? 1 : occ);
     return HIGS_OK;
 }

@@ -213,3 +213,26 @@ def test_odd_sizes_empty_and_all_culled():
     ls = oracle.bin_lists(pr)
     assert ls.n_pairs == 0 and ls.n_units == 0
     assert not oracle.render(pr).any()
+
+
+def test_lists_and_batched_render_with_16x16_tiles():
+    """The 16x16-tile variant (Table 2): macro-tiles of 8x4 tiles = 128x64 px.  Counts and sorted
+    segments against numpy on the scan at 128x64 cells, and the batched renderer on those lists equals O-IMG."""
+    s = hs.scene_cfg1(N=4000, W=320, H=240)
+    cam = s.cameras[0]
+    pr = oracle.project(s, cam)
+    ls = oracle.bin_lists(pr, B_r=64, tile=16)
+    nmx, nmy = (cam.W + 127) // 128, (cam.H + 63) // 64
+    assert ls.mt_count.size == nmx * nmy
+    cells = [oracle.scan(pr.geo[i], cam.W, cam.H, 128, 64) for i in np.nonzero(pr.valid)[0]]
+    flat = np.concatenate(cells)
+    assert np.array_equal(ls.mt_count, np.bincount(flat, minlength=nmx * nmy).astype(np.uint32))
+    assert np.array_equal(ls.batch_offset[1:], np.cumsum((ls.mt_count + 63) // 64))
+    owner = np.concatenate([np.full(len(c), i, np.uint32) for c, i in zip(cells, np.nonzero(pr.valid)[0])])
+    for m in (0, nmx * nmy // 2, nmx * nmy - 1):
+        ids = owner[flat == m]
+        order = np.lexsort((ids, pr.key[ids]))
+        a, b = int(ls.mt_offset[m]), int(ls.mt_offset[m + 1])
+        assert np.array_equal(ls.ids[a:b], ids[order])
+    img = oracle.render(pr)
+    assert np.abs(oracle.render_batched(pr, ls, B_r=64, tile=16) - img).max() <= 1e-6

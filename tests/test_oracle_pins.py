@@ -404,3 +404,25 @@ def test_sh_degree3_colour_uses_view_direction_and_clamps_at_zero():
         ref = np.maximum(0.0, 0.5 + Y @ s.sh[i].astype(np.float64))
         np.testing.assert_allclose(pr.rgb[i], ref, atol=1e-10)
     assert (pr.rgb >= 0).all()
+
+
+def test_cholesky_identity_and_factors():
+    """Sigma^-1 = L L^T gives q = (l0 dx + l1 dy)^2 + (l2 dy)^2, equal to the conic form
+    A dx^2 + B2 dx dy + C dy^2.  Checked against an independent fp64 evaluation written here from the covariance
+    (numpy inverse and numpy Cholesky), on ordinary gaussians of cfg1 and on ill-conditioned needles, where the
+    conic form cancels but the sum of squares does not; a swapped l1 / l2, a wrong sign of l1 or an upper-triangular
+    factor each fail."""
+    rng = np.random.default_rng(12)
+    for scene in (hs.scene_cfg1(N=400), hs.needle_scene(200, 1920, 1080, seed=3, sigma_lo_px=50, sigma_hi_px=1500)):
+        pr = oracle.project(scene, scene.cameras[0])
+        for i in np.nonzero(pr.valid)[0][:150]:
+            a, b, c = (float(v) for v in pr.geo[i, 2:5])
+            l = oracle.cholesky(a, b, c)
+            Sinv = np.linalg.inv(np.array([[a, b], [b, c]], np.float64))
+            Lnp = np.linalg.cholesky(Sinv)                      # lower triangular, positive diagonal: unique
+            assert np.allclose([l[0], l[1], l[2]], [Lnp[0, 0], Lnp[1, 0], Lnp[1, 1]], rtol=1e-9, atol=0)
+            for _ in range(4):
+                dx, dy = rng.normal(0, 3 * math.sqrt(a)), rng.normal(0, 3 * math.sqrt(c))
+                d = np.array([dx, dy])
+                q_ref = float(d @ Sinv @ d)
+                assert abs(oracle.q_cholesky(dx, dy, l) - q_ref) <= 1e-6 * max(q_ref, 1e-12)
