@@ -118,6 +118,8 @@ typedef struct {
                                         unit).  Culling, macro-tile lists and the depth sort are the same pinned fp32 code, so the
                                         integer lists stay bit-exact; the image is accepted by PSNR against the fp32 oracle.  In
                                         this mode higs_get_records returns valid_bits only (rec rows are not written).        */
+#define HIGS_FLAG_SH32          32u  /* resident-scene renders (higs_render_view*) read the 32-byte SH codes made by
+                                        higs_scene_compress_sh instead of the 192-byte fp32 rows              */
 #define HIGS_FLAG_RADIX_SORT    8u   /* tier kernels run the block radix sort (8-bit passes) instead of
                                         the block merge sort; same result, measured slower on B200 (profiles/)   */
 
@@ -157,6 +159,14 @@ int higs_render_host(higs_ctx* ctx, const float* means, const float* scales, con
 int higs_scene_upload(higs_ctx* ctx, const float* means, const float* scales, const float* quats,
                       const float* opacities, const float* sh, int degree, int64_t N);
 int higs_render_view_host(higs_ctx* ctx, const higs_camera* cam, int W, int H, float* out_rgb);
+/* 32-byte SH codec (section 4.2): encode the resident scene's degree-3 SH rows on the device - YCoCg-R,
+ * square-root gamma quantisation (6 bits luma, 4 bits chroma; 16 / 15 / 15 bits for the DC basis), per-(basis, channel)
+ * scales = the 99.9th percentile of |value| over the scene (the maximum for DC); bit layout in DESIGN.md (Q20).  With
+ * HIGS_FLAG_SH32 set, higs_render_view / higs_render_view_host then decode the codes inline in the projection kernel.
+ * Synchronises.  HIGS_E_ARG if no degree-3 scene is resident.  higs_scene_upload discards the codes. */
+int higs_scene_compress_sh(higs_ctx* ctx);
+/* Copies the codes ([N][32] bytes) and the scale table ([16][3] floats: Y, Co, Cg) to HOST memory (either may be NULL). */
+int higs_get_sh32(higs_ctx* ctx, uint8_t* host_codes, float* host_scales);
 /* Resident-scene path with a DEVICE image (no download, no synchronisation). */
 int higs_render_view(higs_ctx* ctx, const higs_camera* cam, int W, int H, float* out_rgb, void* cuda_stream);
 

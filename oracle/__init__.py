@@ -75,6 +75,9 @@ def lib():
         L.orc_bin_tile.argtypes = [C.c_int64, u8p, u32p, f32p, C.c_int, C.c_int, C.c_int, C.c_int, u32p, u32p, u32p, u32p, u32p, C.c_int64]
         L.orc_render_batched_tile.restype = None
         L.orc_render_batched_tile.argtypes = [u32p, u32p, f32p, f32p, f32p, f64p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, f64p]
+        L.orc_sh32_scales.restype = None; L.orc_sh32_scales.argtypes = [C.c_int64, f32p, f32p]
+        L.orc_sh32_encode.restype = None; L.orc_sh32_encode.argtypes = [C.c_int64, f32p, f32p, u8p]
+        L.orc_sh32_decode.restype = None; L.orc_sh32_decode.argtypes = [C.c_int64, u8p, f32p, f32p]
         L.orc_cholesky.restype = None
         L.orc_cholesky.argtypes = [C.c_double, C.c_double, C.c_double, f64p]
         L.orc_q_cholesky.restype = C.c_double
@@ -244,3 +247,27 @@ def q_cholesky(dx: float, dy: float, l: np.ndarray) -> float:
 def render_scene(scene, cam, window=None, threads: Optional[int] = None) -> np.ndarray:
     """project -> O-IMG; what bench.py's cpu_baseline leg times."""
     return render(project(scene, cam), window=window, threads=threads)
+
+
+# ---- 32-byte SH codec (PAPER.md:245; layout: DESIGN.md reading Q20) -------------------------------
+def sh32_scales(sh: np.ndarray) -> np.ndarray:
+    """Per-(basis, channel) scale table [16][3] (Y, Co, Cg): |v| at sorted index floor(0.999 N), the maximum for the DC basis."""
+    sh = np.ascontiguousarray(sh, np.float32)
+    assert sh.shape[1:] == (16, 3)
+    out = np.zeros((16, 3), np.float32)
+    lib().orc_sh32_scales(sh.shape[0], _p(sh, C.c_float), _p(out, C.c_float))
+    return out
+
+
+def sh32_encode(sh: np.ndarray, scales: np.ndarray) -> np.ndarray:
+    sh = np.ascontiguousarray(sh, np.float32); scales = np.ascontiguousarray(scales, np.float32)
+    out = np.zeros((sh.shape[0], 32), np.uint8)
+    lib().orc_sh32_encode(sh.shape[0], _p(sh, C.c_float), _p(scales, C.c_float), _p(out, C.c_uint8))
+    return out
+
+
+def sh32_decode(codes: np.ndarray, scales: np.ndarray) -> np.ndarray:
+    codes = np.ascontiguousarray(codes, np.uint8); scales = np.ascontiguousarray(scales, np.float32)
+    out = np.zeros((codes.shape[0], 16, 3), np.float32)
+    lib().orc_sh32_decode(codes.shape[0], _p(codes, C.c_uint8), _p(scales, C.c_float), _p(out, C.c_float))
+    return out

@@ -625,4 +625,129 @@ double orc_q_cholesky(double dx, double dy, const double* l)
     return t1 * t1 + t2 * t2;
 }
 
+
+/* ---------------------------------------------------------------------------------------
+ * 32-byte SH codec (section 4.2): "YCoCg-R color-space conversion to decorrelate channels,
+ * square-root gamma quantization (6 bits luma, 4 bits chroma), and per-basis percentile scaling ... 192 bytes
+ * (fp32) to 32 bytes".  The paper gives no bit layout; this is the reading of DESIGN.md section 2 (Q20):
+ *   per basis k = 0..15 the coefficient triple (r, g, b) goes to (Y, Co, Cg) by the lifting steps of YCoCg-R
+ *       Co = r - b;  t = b + Co/2;  Cg = g - t;  Y = t + Cg/2        (inverse: t = Y - Cg/2; g = Cg + t; b = t - Co/2; r = b + Co)
+ *   each value v is scaled by s = the per-(basis, channel) percentile of |v| over the scene (p = 0.999; p = 1 for the DC
+ *   basis), clamped to [-1, 1] and quantised on a square-root curve:  code = bias + sign(u) * rint(sqrt(|u|) * L),
+ *   u = v / s, with (L, bias) = (31, 32) for 6-bit luma and (7, 8) for 4-bit chroma; decode: w = (code - bias) / L,
+ *   v = s * w * |w|.  16 x (6 + 4 + 4) = 224 bits; the remaining 32 bits extend the DC basis, which carries the
+ *   base colour, to 16-bit luma (L = 32767) and 15-bit chroma (L = 16383): the 6 / 4-bit fields of k = 0 are the
+ *   top bits of those codes.
+ *   Layout: bytes 0-11 luma, 6 bits per basis, little-endian bit stream; byte 12 + k = Cg_k << 4 | Co_k;
+ *   bytes 28-31 (little-endian word) = DC Y low 10 bits | DC Co low 11 bits << 10 | DC Cg low 11 bits << 21.
+ * The encoder's arithmetic is fp32, one rounding per written op (the CUDA encoder produces the same bytes); decoding is fp64.
+ * ------------------------------------------------------------------------------------- */
+static inline void ycocg_fwd(float r, float g, float b, float* y, float* co, float* cg)
+{
+    float Co = r - b;
+    float t = b + 0.5f * Co;
+    float Cg = g - t;
+    *y = t + 0.5f * Cg; *co = Co; *cg = Cg;
+}
+
+static int cmp_f32(const void* pa, const void* pb)
+{
+    float a = *(const float*)pa, b = *(const float*)pb;
+    return a < b ? -1 : (a > b ? 1 : 0);
+}
+
+/* scales[k*3 + c], c = 0 Y, 1 Co, 2 Cg: |v| at sorted index min(N-1, floor(p N)), p = 1 for k = 0 else 0.999; 1 if that is 0 */
+void orc_sh32_scales(int64_t N, const float* sh, float* scales)
+{
+    float* col = (float*)malloc(sizeof(float) * (size_t)(N > 0 ? N : 1));
+    for (int k = 0; k < 16; ++k) for (int c = 0; c < 3; ++c) {
+        for (int64_t i = 0; i < N; ++i) {
+            const float* q = sh + (i * 16 + k) * 3;
+            float v[3];
+            ycocg_fwd(q[0], q[1], q[2], &v[0], &v[1], &v[2]);
+            col[i] = fabsf(v[c]);
+        }
+        qsort(col, (size_t)N, sizeof(float), cmp_f32);
+        int64_t idx = k == 0 ? N - 1 : (int64_t)((double)N * 0.999);
+        if (idx > N - 1) idx = N - 1;
+        float sc = N > 0 ? col[idx] : 1.0f;
+        scales[k * 3 + c] = (sc > 0.0f && sc <= FLT_MAX) ? sc : 1.0f;
+    }
+    free(col);
+}
+
+static inline uint32_t sh32_quant(float v, float s, int L)
+{
+    float u = v / s;
+    float a = fminf(fabsf(u), 1.0f);
+    float w = sqrtf(a);
+    int c = (int)rintf(w * (float)L);
+    return (uint32_t)((L + 1) + (u < 0.0f ? -c : c));
+}
+
+void orc_sh32_encode(int64_t N, const float* sh, const float* scales, uint8_t* out)
+{
+    for (int64_t i = 0; i < N; ++i) {
+        uint8_t* o = out + 32 * i;
+        memset(o, 0, 32);
+        uint64_t luma_lo = 0; uint32_t luma_hi = 0;          /* 96-bit little-endian bit stream */
+        for (int k = 0; k < 16; ++k) {
+            const float* q = sh + (i * 16 + k) * 3;
+            float y, co, cg;
+            ycocg_fwd(q[0], q[1], q[2], &y, &co, &cg);
+            uint32_t cy, cco, ccg;
+            if (k == 0) {
+                uint32_t y16 = sh32_quant(y, scales[0], 32767), co15 = sh32_quant(co, scales[1], 16383), cg15 = sh32_quant(cg, scales[2], 16383);
+                uint32_t ext = (y16 & 0x3ffu) | ((co15 & 0x7ffu) << 10) | ((cg15 & 0x7ffu) << 21);
+                o[28] = (uint8_t)ext; o[29] = (uint8_t)(ext >> 8); o[30] = (uint8_t)(ext >> 16); o[31] = (uint8_t)(ext >> 24);
+                cy = y16 >> 10; cco = co15 >> 11; ccg = cg15 >> 11;
+            } else {
+                cy = sh32_quant(y, scales[k * 3], 31); cco = sh32_quant(co, scales[k * 3 + 1], 7); ccg = sh32_quant(cg, scales[k * 3 + 2], 7);
+            }
+            int bit = 6 * k;
+            if (bit < 64) { luma_lo |= (uint64_t)cy << bit; if (bit > 58) luma_hi |= cy >> (64 - bit); }
+            else luma_hi |= cy << (bit - 64);
+            o[12 + k] = (uint8_t)((ccg << 4) | cco);
+        }
+        for (int b = 0; b < 8; ++b) o[b] = (uint8_t)(luma_lo >> (8 * b));
+        for (int b = 0; b < 4; ++b) o[8 + b] = (uint8_t)(luma_hi >> (8 * b));
+    }
+}
+
+static inline double sh32_dequant(uint32_t code, double s, int L)
+{
+    double w = ((double)code - (double)(L + 1)) / (double)L;
+    return s * w * fabs(w);
+}
+
+/* decoded coefficients, [N][16][3] fp32 (rounded once from the fp64 decode) */
+void orc_sh32_decode(int64_t N, const uint8_t* in, const float* scales, float* sh)
+{
+    for (int64_t i = 0; i < N; ++i) {
+        const uint8_t* o = in + 32 * i;
+        uint64_t luma_lo = 0; uint32_t luma_hi = 0;
+        for (int b = 0; b < 8; ++b) luma_lo |= (uint64_t)o[b] << (8 * b);
+        for (int b = 0; b < 4; ++b) luma_hi |= (uint32_t)o[8 + b] << (8 * b);
+        uint32_t ext = (uint32_t)o[28] | ((uint32_t)o[29] << 8) | ((uint32_t)o[30] << 16) | ((uint32_t)o[31] << 24);
+        for (int k = 0; k < 16; ++k) {
+            int bit = 6 * k;
+            uint32_t cy = bit < 64 ? (uint32_t)(luma_lo >> bit) : (luma_hi >> (bit - 64));
+            if (bit < 64 && bit > 58) cy |= luma_hi << (64 - bit);
+            cy &= 63u;
+            uint32_t cco = o[12 + k] & 15u, ccg = o[12 + k] >> 4;
+            double y, co, cg;
+            if (k == 0) {
+                y = sh32_dequant((cy << 10) | (ext & 0x3ffu), scales[0], 32767);
+                co = sh32_dequant((cco << 11) | ((ext >> 10) & 0x7ffu), scales[1], 16383);
+                cg = sh32_dequant((ccg << 11) | (ext >> 21), scales[2], 16383);
+            } else {
+                y = sh32_dequant(cy, scales[k * 3], 31); co = sh32_dequant(cco, scales[k * 3 + 1], 7); cg = sh32_dequant(ccg, scales[k * 3 + 2], 7);
+            }
+            double t = y - 0.5 * cg, g = cg + t, b = t - 0.5 * co, r = b + co;
+            float* q = sh + (i * 16 + k) * 3;
+            q[0] = (float)r; q[1] = (float)g; q[2] = (float)b;
+        }
+    }
+}
+
 int orc_abi_version(void) { return 1; }

@@ -19,12 +19,12 @@ import numpy as np
 from . import build as _build
 
 HIGS_OK, HIGS_E_ARG, HIGS_E_CUDA, HIGS_E_CAPACITY, HIGS_E_NOMEM = 0, -1, -2, -3, -4
-HIGS_FLAG_STAGE_TIMERS, HIGS_FLAG_COUNT_EVALS, HIGS_FLAG_NO_XBATCH_CUT, HIGS_FLAG_RADIX_SORT, HIGS_FLAG_FP16 = 1, 2, 4, 8, 16
+HIGS_FLAG_STAGE_TIMERS, HIGS_FLAG_COUNT_EVALS, HIGS_FLAG_NO_XBATCH_CUT, HIGS_FLAG_RADIX_SORT, HIGS_FLAG_FP16, HIGS_FLAG_SH32 = 1, 2, 4, 8, 16, 32
 HIGS_TILE, HIGS_MT_W, HIGS_MT_H, HIGS_MT_TILES, HIGS_BATCH_CAP = 8, 64, 32, 32, 1024
 
 EXPORTS = ["higs_abi_version", "higs_strerror", "higs_last_error", "higs_create", "higs_destroy", "higs_set_flags",
            "higs_set_batch_cap", "higs_set_tile", "higs_render", "higs_render_host", "higs_scene_upload", "higs_render_view_host",
-           "higs_render_view", "higs_get_stats", "higs_get_lists", "higs_get_records", "higs_sort_segments", "higs_download"]
+           "higs_render_view", "higs_scene_compress_sh", "higs_get_sh32", "higs_get_stats", "higs_get_lists", "higs_get_records", "higs_sort_segments", "higs_download"]
 
 
 class higs_camera(C.Structure):
@@ -93,6 +93,8 @@ def load() -> C.CDLL:
         L.higs_render_view_host.argtypes = [vp, C.POINTER(higs_camera), C.c_int, C.c_int, f32p]
         L.higs_render_view.restype = C.c_int
         L.higs_render_view.argtypes = [vp, C.POINTER(higs_camera), C.c_int, C.c_int, f32p, vp]
+        L.higs_scene_compress_sh.restype = C.c_int; L.higs_scene_compress_sh.argtypes = [vp]
+        L.higs_get_sh32.restype = C.c_int; L.higs_get_sh32.argtypes = [vp, vp, vp]
         L.higs_get_stats.restype = C.c_int; L.higs_get_stats.argtypes = [vp, C.POINTER(higs_stats)]
         L.higs_get_lists.restype = C.c_int; L.higs_get_lists.argtypes = [vp, C.POINTER(higs_lists)]
         L.higs_get_records.restype = C.c_int; L.higs_get_records.argtypes = [vp, C.POINTER(higs_records)]
@@ -184,6 +186,17 @@ def higs_scene_upload(ctx, means, scales, quats, opacities, sh, degree: int) -> 
     N = int(opacities.shape[0])
     _check(load().higs_scene_upload(ctx, _ptr(means), _ptr(scales), _ptr(quats), _ptr(opacities), _ptr(sh), degree, N),
            "higs_scene_upload", ctx)
+
+
+def higs_scene_compress_sh(ctx) -> None:
+    _check(load().higs_scene_compress_sh(ctx), "higs_scene_compress_sh", ctx)
+
+
+def higs_get_sh32(ctx, n: int):
+    """(codes [n][32] uint8, scales [16][3] float32) of the resident scene's 32-byte SH codes."""
+    codes = np.zeros((n, 32), np.uint8); scales = np.zeros((16, 3), np.float32)
+    _check(load().higs_get_sh32(ctx, C.c_void_p(codes.ctypes.data), C.c_void_p(scales.ctypes.data)), "higs_get_sh32", ctx)
+    return codes, scales
 
 
 def higs_render_view_host(ctx, cam: higs_camera, W: int, H: int, out_rgb) -> None:

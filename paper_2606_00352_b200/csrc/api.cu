@@ -61,7 +61,7 @@ int check_frame_args(higs_ctx* ctx, int degree, int64_t N, const higs_camera* ca
 
 int render_impl(higs_ctx* ctx, const float* means, const float* scales, const float* quats, const float* opac,
                 const float* sh, int degree, int64_t N, const higs_camera* cam, int W, int H, float* out_rgb,
-                cudaStream_t st)
+                cudaStream_t st, bool sh32 = false)
 {
     HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
     FrameParams P;
@@ -81,7 +81,7 @@ int render_impl(higs_ctx* ctx, const float* means, const float* scales, const fl
     // one memset: frame header, per-macro-tile pair counts and fill cursors (one allocation)
     HIGS_CUDA(ctx, cudaMemsetAsync(ctx->hdr, 0, sizeof(uint32_t) * (HIGS_HDR_WORDS + 2 * ((size_t)ctx->max_nm + 1)), st));
     if (timers) cudaEventRecord(ev[0], st);
-    if ((rc = launch_project(ctx, P, means, scales, quats, opac, sh, N, st))) return rc;
+    if ((rc = launch_project(ctx, P, means, scales, quats, opac, sh, sh32, N, st))) return rc;
     if (timers) cudaEventRecord(ev[1], st);
     if ((rc = launch_binning(ctx, P, N, st, timers ? ev[2] : nullptr, timers ? ev[3] : nullptr))) return rc;
     if (timers) cudaEventRecord(ev[4], st);
@@ -236,7 +236,7 @@ void higs_destroy(higs_ctx* ctx)
     dev_free(ctx->bucket_cursor); dev_free(ctx->partial); dev_free(ctx->cut_word); dev_free(ctx->cut_term);
     dev_free(ctx->unit_order); dev_free(ctx->level_hist); dev_free(ctx->level_cur);
     dev_free(ctx->s_means); dev_free(ctx->s_scales); dev_free(ctx->s_quats); dev_free(ctx->s_opac); dev_free(ctx->s_sh);
-    dev_free(ctx->s_img);
+    dev_free(ctx->s_img); dev_free(ctx->s_sh32); dev_free(ctx->sh32_work);
     if (ctx->hdr_host) cudaFreeHost(ctx->hdr_host);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     for (int i = 0; i < 9; ++i) if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
@@ -305,7 +305,32 @@ int higs_scene_upload(higs_ctx* ctx, const float* means, const float* scales, co
         HIGS_CUDA(ctx, cudaMemcpyAsync(ctx->s_sh, sh, sizeof(float) * 3 * K * N, cudaMemcpyHostToDevice, st));
     }
     HIGS_CUDA(ctx, cudaStreamSynchronize(st));
-    ctx->s_n = N; ctx->s_degree = degree;
+    ctx->s_n = N; ctx->s_degree = degree; ctx->s_sh32_valid = false;
+    return HIGS_OK;
+}
+
+int higs_scene_compress_sh(higs_ctx* ctx)
+{
+    if (!ctx || ctx->s_degree != 3 || ctx->s_n < 0) return HIGS_E_ARG;
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (ctx->s_n > ctx->s_sh32_cap) {
+        dev_free(ctx->s_sh32); ctx->s_sh32_cap = 0;
+        int rc = dev_alloc(ctx, &ctx->s_sh32, (size_t)ctx->s_n * 2);
+        if (rc) return rc;
+        ctx->s_sh32_cap = ctx->s_n;
+    }
+    int rc = launch_sh32_encode(ctx, ctx->own_stream);
+    if (rc) return rc;
+    ctx->s_sh32_valid = true;
+    return HIGS_OK;
+}
+
+int higs_get_sh32(higs_ctx* ctx, uint8_t* host_codes, float* host_scales)
+{
+    if (!ctx || !ctx->s_sh32_valid) return HIGS_E_ARG;
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (host_codes && ctx->s_n > 0) HIGS_CUDA(ctx, cudaMemcpy(host_codes, ctx->s_sh32, (size_t)ctx->s_n * 32, cudaMemcpyDeviceToHost));
+    if (host_scales) memcpy(host_scales, ctx->sh32_scales_host, sizeof(float) * 48);
     return HIGS_OK;
 }
 
@@ -314,8 +339,9 @@ int higs_render_view(higs_ctx* ctx, const higs_camera* cam, int W, int H, float*
     if (!ctx) return HIGS_E_ARG;
     int rc = check_frame_args(ctx, ctx->s_degree, ctx->s_n, cam, W, H, out_rgb);
     if (rc) return rc;
-    return render_impl(ctx, ctx->s_means, ctx->s_scales, ctx->s_quats, ctx->s_opac, ctx->s_sh, ctx->s_degree, ctx->s_n,
-                       cam, W, H, out_rgb, (cudaStream_t)cuda_stream);
+    const bool sh32 = (ctx->flags & HIGS_FLAG_SH32) && ctx->s_sh32_valid;
+    return render_impl(ctx, ctx->s_means, ctx->s_scales, ctx->s_quats, ctx->s_opac, sh32 ? reinterpret_cast<const float*>(ctx->s_sh32) : ctx->s_sh,
+                       ctx->s_degree, ctx->s_n, cam, W, H, out_rgb, (cudaStream_t)cuda_stream, sh32);
 }
 
 int higs_render_view_host(higs_ctx* ctx, const higs_camera* cam, int W, int H, float* out_rgb)
@@ -326,8 +352,9 @@ int higs_render_view_host(higs_ctx* ctx, const higs_camera* cam, int W, int H, f
     HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
     if ((rc = ensure_image_capacity(ctx, W, H))) return rc;
     cudaStream_t st = ctx->own_stream;
-    rc = render_impl(ctx, ctx->s_means, ctx->s_scales, ctx->s_quats, ctx->s_opac, ctx->s_sh, ctx->s_degree, ctx->s_n,
-                     cam, W, H, ctx->s_img, st);
+    const bool sh32 = (ctx->flags & HIGS_FLAG_SH32) && ctx->s_sh32_valid;
+    rc = render_impl(ctx, ctx->s_means, ctx->s_scales, ctx->s_quats, ctx->s_opac, sh32 ? reinterpret_cast<const float*>(ctx->s_sh32) : ctx->s_sh,
+                     ctx->s_degree, ctx->s_n, cam, W, H, ctx->s_img, st, sh32);
     if (rc) return rc;
     HIGS_CUDA(ctx, cudaMemcpyAsync(out_rgb, ctx->s_img, sizeof(float) * 3 * (size_t)W * H, cudaMemcpyDeviceToHost, st));
     HIGS_CUDA(ctx, cudaStreamSynchronize(st));

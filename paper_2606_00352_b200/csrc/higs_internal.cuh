@@ -60,6 +60,8 @@ struct FrameParams {
     uint32_t max_pairs, max_units;
 };
 
+struct ShScales { float s[48]; };   // 32-byte SH code: scale of (basis k, channel Y / Co / Cg) at [k*3 + c], passed to kernels by value
+
 struct higs_ctx {
     int device;
     int64_t max_gaussians;
@@ -113,6 +115,11 @@ struct higs_ctx {
     FrameHeader* hdr_host;     // pinned
     // resident scene / host staging
     float *s_means, *s_scales, *s_quats, *s_opac, *s_sh, *s_img;
+    uint4* s_sh32;             // [s_n][2] 32-byte SH codes of the resident scene (higs_scene_compress_sh), or null
+    int64_t s_sh32_cap;
+    bool s_sh32_valid;
+    float sh32_scales_host[48];
+    uint32_t* sh32_work;       // device scratch of the encoder: hist [48][256] | prefix [48] | rank lo/hi [48][2] | scales [48]
     int64_t s_cap_n; int s_cap_k; int64_t s_img_cap;
     int64_t s_n; int s_degree;
     // last frame
@@ -156,7 +163,8 @@ inline cudaError_t launch_pdl(void (*kernel)(KP...), dim3 grid, dim3 block, size
 
 // ---- launch entry points, one per pipeline step (defined in the .cu files) ----------------------
 int launch_project(higs_ctx*, const FrameParams&, const float* means, const float* scales, const float* quats,
-                   const float* opac, const float* sh, int64_t N, cudaStream_t);
+                   const float* opac, const float* sh, bool sh32, int64_t N, cudaStream_t);
+int launch_sh32_encode(higs_ctx*, cudaStream_t);
 int higs_part_grid(const higs_ctx*, int64_t N);
 int higs_part_lcap(int64_t n_chunks, int grid);
 int launch_binning(higs_ctx*, const FrameParams&, int64_t N, cudaStream_t, cudaEvent_t ev_count, cudaEvent_t ev_scan);

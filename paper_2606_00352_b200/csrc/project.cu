@@ -14,6 +14,7 @@
 // the pinned fp32 sequence N-PROJ of DESIGN.md section 3, one correctly rounded op per written op:
 // the __f*_rn intrinsics are never contracted into FMAs by nvcc.
 #include <stdio.h>
+#include <string.h>
 #include <cuda_fp16.h>
 #include "higs_internal.cuh"
 
@@ -97,6 +98,54 @@ __device__ __forceinline__ void sh_accumulate(const float* __restrict__ shp, flo
         b = fmaf(Y[k], c[3 * k + 2], b);
     }
     r = fmaxf(r, 0.0f); g = fmaxf(g, 0.0f); b = fmaxf(b, 0.0f);
+}
+
+// Colour from the 32-byte SH code (layout and quantiser: DESIGN.md reading Q20, shcodec.cu).  The evaluation is
+// linear, so it runs in YCoCg space - sum_k Y_k(dir) * (y, co, cg)_k - and one inverse YCoCg-R lifting at the end gives
+// r, g, b.  lut: [16][64] luma then [16][2][16] chroma dequantised values s * w|w| (built per CTA from the scale table),
+// so a coefficient costs a bit-field extract, one shared load and one FMA.  The DC basis (16 / 15 / 15 bits) is
+// dequantised arithmetically.
+__device__ __forceinline__ void sh32_colour(const uint4* __restrict__ codes, int64_t i, const float* __restrict__ lut,
+                                            const ShScales& sc, float x, float y, float z, float& r, float& g, float& b)
+{
+    const uint4 c0 = HIGS_LD(codes + 2 * i), c1 = HIGS_LD(codes + 2 * i + 1);
+    const uint32_t lw[4] = { c0.x, c0.y, c0.z, 0u };               // luma bit stream
+    const uint32_t cw[4] = { c0.w, c1.x, c1.y, c1.z };             // chroma bytes: Cg << 4 | Co
+    float Y[16];
+    Y[0] = 0.28209479177387814f;
+    {
+        const float C1 = 0.4886025119029199f;
+        Y[1] = -C1 * y; Y[2] = C1 * z; Y[3] = -C1 * x;
+        const float xx = x * x, yy = y * y, zz = z * z;
+        const float C2a = 1.0925484305920792f, C2b = 0.31539156525252005f, C2c = 0.5462742152960396f;
+        Y[4] = C2a * x * y; Y[5] = -C2a * y * z; Y[6] = C2b * (2.0f * zz - xx - yy); Y[7] = -C2a * x * z; Y[8] = C2c * (xx - yy);
+        const float C3a = 0.5900435899266435f, C3b = 2.890611442640554f, C3c = 0.4570457994644658f,
+                    C3d = 0.3731763325901154f, C3e = 1.445305721320277f;
+        Y[9]  = -C3a * y * (3.0f * xx - yy); Y[10] = C3b * x * y * z; Y[11] = -C3c * y * (4.0f * zz - xx - yy);
+        Y[12] = C3d * z * (2.0f * zz - 3.0f * xx - 3.0f * yy); Y[13] = -C3c * x * (4.0f * zz - xx - yy);
+        Y[14] = C3e * z * (xx - yy); Y[15] = -C3a * x * (xx - 3.0f * yy);
+    }
+    // DC: 16-bit luma, 15-bit chroma codes = (field of k = 0) << 10 / 11 | extension bits
+    const uint32_t ext = c1.w;
+    const uint32_t y16 = ((c0.x & 63u) << 10) | (ext & 0x3ffu);
+    const uint32_t co15 = ((c0.w & 15u) << 11) | ((ext >> 10) & 0x7ffu), cg15 = (((c0.w >> 4) & 15u) << 11) | (ext >> 21);
+    const float wy = ((float)(int)y16 - 32768.0f) * (1.0f / 32767.0f), wco = ((float)(int)co15 - 16384.0f) * (1.0f / 16383.0f),
+                wcg = ((float)(int)cg15 - 16384.0f) * (1.0f / 16383.0f);
+    float ay = Y[0] * (sc.s[0] * wy * fabsf(wy)), aco = Y[0] * (sc.s[1] * wco * fabsf(wco)), acg = Y[0] * (sc.s[2] * wcg * fabsf(wcg));
+#pragma unroll
+    for (int k = 1; k < 16; ++k) {
+        const int bit = 6 * k, wd = bit >> 5, sh_ = bit & 31;
+        const uint32_t cy = __funnelshift_r(lw[wd], lw[wd + 1 < 4 ? wd + 1 : 3], sh_) & 63u;
+        const uint32_t cb = cw[k >> 2] >> (8 * (k & 3));
+        ay = fmaf(Y[k], lut[k * 64 + cy], ay);
+        aco = fmaf(Y[k], lut[1024 + k * 32 + (cb & 15u)], aco);
+        acg = fmaf(Y[k], lut[1024 + k * 32 + 16 + ((cb >> 4) & 15u)], acg);
+    }
+    const float t = ay - 0.5f * acg;
+    g = acg + t;
+    b = t - 0.5f * aco;
+    r = b + aco;
+    r = fmaxf(r + 0.5f, 0.0f); g = fmaxf(g + 0.5f, 0.0f); b = fmaxf(b + 0.5f, 0.0f);
 }
 
 constexpr int PROJ_THREADS = 512;
@@ -211,8 +260,8 @@ __device__ __forceinline__ bool project_cull(const RawIn& in, const FrameParams&
 
 // Phase B for one survivor: a2 macro-tile row scan (N-SCAN, pinned) -> private histogram + span descriptor,
 // SH colour, and the two records at dense slot `slot`.
-template <int DEG, bool HALF>
-__device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size_t slot, const float* __restrict__ sh,
+template <int DEG, bool HALF, bool SHC>
+__device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size_t slot, const float* __restrict__ sh, const float* __restrict__ lut, const ShScales& sc,
                                               const FrameParams& P, uint32_t* s_hist, float4* __restrict__ rec,
                                               uint4* __restrict__ rec16, uint4* __restrict__ bin)
 {
@@ -240,7 +289,8 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
     const float len2 = dx * dx + dy * dy + dz * dz;
     const float rl = len2 > 0.0f ? rsqrtf(len2) : 0.0f;
     float r, g, bl;
-    sh_accumulate<DEG>(sh + i * (int64_t)((DEG + 1) * (DEG + 1) * 3), dx * rl, dy * rl, dz * rl, r, g, bl);
+    if constexpr (SHC) sh32_colour(reinterpret_cast<const uint4*>(sh), i, lut, sc, dx * rl, dy * rl, dz * rl, r, g, bl);
+    else sh_accumulate<DEG>(sh + i * (int64_t)((DEG + 1) * (DEG + 1) * 3), dx * rl, dy * rl, dz * rl, r, g, bl);
     const uint32_t key = __float_as_uint(s.zc);
     if constexpr (HALF) {
         // fp16 data path: inverse covariance as Cholesky factors L = [[l0, 0], [l1, l2]], L L^T = conic,
@@ -272,13 +322,13 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
 // and queues the survivors (about 4 in 10 at paper scale) in shared memory; whenever 32 are queued it runs phase B
 // on them with every lane busy.  Survivor k of chunk c gets dense slot c*HIGS_CHUNK + k: slots are monotone in the
 // gaussian id, so (key, slot) order = (key, id) order (Q7).
-template <int DEG, bool HALF>
+template <int DEG, bool HALF, bool SHC>
 __global__ void __launch_bounds__(PROJ_THREADS, 2)
 k_project(const float* __restrict__ means, const float* __restrict__ scales, const float* __restrict__ quats,
           const float* __restrict__ opac, const float* __restrict__ sh, int64_t N, const FrameParams P,
           uint32_t* __restrict__ valid_bits, float4* __restrict__ rec, uint4* __restrict__ rec16, uint4* __restrict__ bin,
           uint32_t* __restrict__ chunk_count, uint32_t* __restrict__ hist, uint32_t* __restrict__ mt_count, uint32_t* __restrict__ part_list,
-          uint2* __restrict__ part_desc, int lcap, FrameHeader* __restrict__ hdr)
+          uint2* __restrict__ part_desc, int lcap, FrameHeader* __restrict__ hdr, const ShScales sc)
 {
     extern __shared__ uint32_t s_dyn[];
     __shared__ uint32_t s_nvis, s_nlist, s_lbase;
@@ -287,6 +337,15 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
     pdl_trigger();                                                   // k_plan may be scheduled as this grid drains
     float* q = reinterpret_cast<float*>(s_dyn + ((P.n_m + 3) & ~3)) + w * (PROJ_QF * PROJ_QCAP);
     uint32_t* s_list = s_dyn + ((P.n_m + 3) & ~3) + PROJ_WARPS * PROJ_QF * PROJ_QCAP;   // [lcap] chunks this CTA claimed
+    float* s_lut = reinterpret_cast<float*>(s_list + lcap);         // [1536] dequantisation tables of the 32-byte SH code (SHC only)
+    if constexpr (SHC) {
+        for (int e = threadIdx.x; e < 1536; e += PROJ_THREADS) {
+            const bool luma = e < 1024;
+            const int k = luma ? e >> 6 : (e - 1024) >> 5, c = luma ? 0 : 1 + (((e - 1024) >> 4) & 1), code = luma ? e & 63 : e & 15;
+            const float wq = luma ? (float)(code - 32) * (1.0f / 31.0f) : (float)(code - 8) * (1.0f / 7.0f);
+            s_lut[e] = sc.s[k * 3 + c] * wq * fabsf(wq);
+        }
+    }
     for (int m = threadIdx.x; m < P.n_m; m += PROJ_THREADS) s_hist[m] = 0;
     if (threadIdx.x == 0) { s_nvis = 0; s_nlist = 0; }
     __syncthreads();
@@ -318,7 +377,7 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
                 s.tau = q[8 * PROJ_QCAP + e]; s.zc = q[9 * PROJ_QCAP + e]; s.o = q[10 * PROJ_QCAP + e];
                 s.mx = q[11 * PROJ_QCAP + e]; s.my = q[12 * PROJ_QCAP + e]; s.mz = q[13 * PROJ_QCAP + e];
                 s.local = __float_as_uint(q[14 * PROJ_QCAP + e]);
-                emit_survivor<DEG, HALF>(s, c0 + s.local, slot0 + head + lane, sh, P, s_hist, rec, rec16, bin);
+                emit_survivor<DEG, HALF, SHC>(s, c0 + s.local, slot0 + head + lane, sh, s_lut, sc, P, s_hist, rec, rec16, bin);
             }
             head += n_live;
             __syncwarp();
@@ -384,7 +443,8 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
 
 static size_t project_smem_bytes(int n_m, int lcap)
 {
-    return sizeof(uint32_t) * (size_t)((n_m + 3) & ~3) + sizeof(float) * (size_t)PROJ_WARPS * PROJ_QF * PROJ_QCAP + sizeof(uint32_t) * (size_t)lcap;
+    return sizeof(uint32_t) * (size_t)((n_m + 3) & ~3) + sizeof(float) * (size_t)PROJ_WARPS * PROJ_QF * PROJ_QCAP + sizeof(uint32_t) * (size_t)lcap
+           + sizeof(float) * 1536;
 }
 
 // list capacity of one partition CTA: four times its fair share of the chunks, so a CTA that fills its list and
@@ -402,16 +462,21 @@ int higs_part_grid(const higs_ctx* ctx, int64_t N)
 }
 
 int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, const float* scales, const float* quats,
-                   const float* opac, const float* sh, int64_t N, cudaStream_t st)
+                   const float* opac, const float* sh, bool sh32, int64_t N, cudaStream_t st)
 {
     if (N <= 0) return HIGS_OK;
     const unsigned grid = (unsigned)higs_part_grid(ctx, N);
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, (int)grid);
     const size_t smem = project_smem_bytes(P.n_m, lcap);
-#define HIGS_PROJ_(D, H) k_project<D, H><<<grid, PROJ_THREADS, smem, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
-                                                                   ctx->rec16, ctx->bin, ctx->chunk_count, ctx->hist, ctx->mt_count, ctx->part_list, ctx->part_desc, lcap, ctx->hdr)
-#define HIGS_PROJ(D) do { if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(D, true); else HIGS_PROJ_(D, false); } while (0)
-    switch (P.degree) {
+#define HIGS_PROJ_(D, H, C) k_project<D, H, C><<<grid, PROJ_THREADS, smem, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
+                                                                   ctx->rec16, ctx->bin, ctx->chunk_count, ctx->hist, ctx->mt_count, ctx->part_list, ctx->part_desc, lcap, ctx->hdr, sc)
+#define HIGS_PROJ(D) do { if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(D, true, false); else HIGS_PROJ_(D, false, false); } while (0)
+    ShScales sc;
+    memset(&sc, 0, sizeof(sc));
+    if (sh32) {                                                      // sh = the 32-byte codes of the resident scene (degree 3)
+        memcpy(sc.s, ctx->sh32_scales_host, sizeof(sc.s));
+        if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(3, true, true); else HIGS_PROJ_(3, false, true);
+    } else switch (P.degree) {
         case 0: HIGS_PROJ(0); break;
         case 1: HIGS_PROJ(1); break;
         case 2: HIGS_PROJ(2); break;
@@ -428,16 +493,13 @@ int higs_project_smem_setup(higs_ctx* ctx)
     // worst case for the list: the full grid on max_gaussians (a smaller grid has at most 16 chunks per CTA)
     const int lcap_max = higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) > 6 * PROJ_WARPS ? higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) : 6 * PROJ_WARPS;
     const int bytes = (int)project_smem_bytes(ctx->max_nm, lcap_max);
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+#define HIGS_ATTR(D, H, C) HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<D, H, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))
+    HIGS_ATTR(0, false, false); HIGS_ATTR(1, false, false); HIGS_ATTR(2, false, false); HIGS_ATTR(3, false, false);
+    HIGS_ATTR(0, true, false); HIGS_ATTR(1, true, false); HIGS_ATTR(2, true, false); HIGS_ATTR(3, true, false);
+    HIGS_ATTR(3, false, true); HIGS_ATTR(3, true, true);
+#undef HIGS_ATTR
     int occ = 0;
-    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3, false>, PROJ_THREADS, (size_t)bytes));
+    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3, false, false>, PROJ_THREADS, (size_t)bytes));
     ctx->n_part_max = ctx->n_sm * (occ < 1 ? 1 : occ);
     return HIGS_OK;
 }
