@@ -48,6 +48,29 @@ FP32_LANES_PER_SM = 128          # ALU peak = SMs x 128 lan
 RASTER_FP32_INST_PER_EVAL = 13.0  # FP32-pipe instructions per pixel-gaussian evaluation (SASS count)
 
 
+def source_sha() -> str:
+    """sha256 over the library's sources: ties the committed ncu traffic figures to the code they were captured on."""
+    import hashlib
+    h = hashlib.sha256()
+    for p in sorted((ROOT / "paper_2606_00352_b200" / "csrc").glob("*.cu*")) + [ROOT / "include" / "higs.h"]:
+        h.update(p.name.encode()); h.update(p.read_bytes())
+    return h.hexdigest()[:16]
+
+
+def committed_traffic() -> dict:
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the stage kernels from the committed
+    `ncu --set full` capture (profiles/r02_traffic.json, written from profiles/r02_final.md's capture).  ncu cannot run
+    inside a timed bench, so the figures are tied to the source hash they were captured on and dropped (null) when the
+    library's sources have changed since."""
+    p = ROOT / "profiles" / "r02_traffic.json"
+    if not p.exists():
+        return {"note": "no committed capture"}
+    d = json.loads(p.read_text())
+    if d.get("src_sha") != source_sha():
+        return {"note": f"stale: captured on sources {d.get('src_sha')}, now {source_sha()}"}
+    return dict(d["traffic"], note=f"ncu --set full capture on sources {d['src_sha']}")
+
+
 def measured_peaks() -> dict:
     p = ROOT / "MEASURED_PEAKS.json"
     if p.exists():
@@ -186,7 +209,7 @@ def workload_config(scene, args, world) -> dict:
     return {"workload": "configs[3]: large scene, paper scale (heavy-tailed planes/shells + 20% background + 10% hot region)",
             "n_gaussians": scene.N, "sh_degree": scene.degree, "image": "1920x1080", "fov_x_deg": 60,
             "views": f"orbit of {len(scene.cameras)} poses, step i -> view (i*{world}+rank) % {len(scene.cameras)}; view 0 = configs[3]'s pose",
-            "tiles": f"8x8 px render tiles, 8x4 macro-tiles (64x32 px), B_r={args.batch_cap}, partition batches = 2 persistent CTAs per SM over 512-id chunks",
+            "tiles": f"8x8 px render tiles, 8x4 macro-tiles (64x32 px), B_r={args.batch_cap}, partition batches = 2 persistent CTAs per SM over 256-id chunks",
             "l2": "inputs (1.37 GB) and per-frame records (0.46 GB) exceed the 126 MB L2; no flush between frames",
             "parallelism": f"replicas x{world} (views sharded, no collective)"}
 
@@ -235,15 +258,16 @@ def run_higs(args) -> int:
     for i in range(args.warmup):
         frame(i)
     barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     t_mark0 = sampler.mark()
-    e0.record(stream)
+    evs[0].record(stream)
     for i in range(args.steps):
         frame(args.warmup + i)
-    e1.record(stream)
+        evs[i + 1].record(stream)              # between frames only: the kernel chains inside a frame are untouched
     barrier()
     t_mark1 = sampler.mark()
-    secs = e0.elapsed_time(e1) / 1000.0
+    secs = evs[0].elapsed_time(evs[-1]) / 1000.0
+    frame_ms = np.array([evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)])
     st_last = hg.higs_get_stats(ctx)
     launches_per_frame = int(st_last["n_launches"])
     if world > 1:
@@ -287,22 +311,22 @@ def run_higs(args) -> int:
         "fill": 16.0 * n_vis + 12.0 * n_b * n_m + 8.0 * n_pairs,                    # 16-B bin record per survivor, bases, pairs written
         "sort": 16.0 * n_pairs,
     }
-    # DRAM bytes per launch (read + write) from the committed ncu --set full capture of this workload
-    # (profiles/r01_final.md); measured once per round under the profiler, not in this run
-    NCU_TRAFFIC = {"project": 1.357e9, "fill": 1.19e8, "sort": 1.30e8, "raster": 3.10e8}
+    NCU_TRAFFIC = committed_traffic()
     def hbm_roof(stage, nbytes):
         ms = stage_ms[stage]
         ach = nbytes / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
         return {"bound": "hbm", "achieved": ach, "peak": hbm, "unit": "GB/s", "frac": ach / hbm, "traffic": NCU_TRAFFIC.get(stage),
-                "peak_source": peaks["which"], "algorithmic_bytes": nbytes, "ms": ms}
+                "traffic_source": NCU_TRAFFIC.get("note"), "peak_source": peaks["which"], "algorithmic_bytes": nbytes, "ms": ms}
     sm_hz = peaks["sm_max_mhz"] * 1e6
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     alu_peak = n_sm * FP32_LANES_PER_SM * sm_hz / 1e9                      # G FP32-pipe thread-instructions / s
     ras_ms = stage_ms["raster"]
     ras_ach = n_evals * RASTER_FP32_INST_PER_EVAL / (ras_ms * 1e-3) / 1e9 if ras_ms > 0 else 0.0
     roof = {k: hbm_roof(k, v) for k, v in alg_bytes.items()}
+    survey_bytes = 44.0 * N + (12.0 * K + 56.0) * n_vis                      # SURVEY.md 8(d)'s own per-unit figure (56 B written per survivor)
+    roof["project"]["frac_survey_formula"] = survey_bytes / (stage_ms["project"] * 1e-3) / 1e9 / hbm if stage_ms["project"] > 0 else 0.0
     roof["raster"] = {"bound": "alu", "achieved": ras_ach, "peak": alu_peak, "unit": "G FP32 thread-inst/s",
-                      "frac": ras_ach / alu_peak, "traffic": NCU_TRAFFIC["raster"], "peak_source": f"{n_sm} SMs x {FP32_LANES_PER_SM} lanes x {peaks['sm_max_mhz']:.0f} MHz",
+                      "frac": ras_ach / alu_peak, "traffic": NCU_TRAFFIC.get("raster"), "peak_source": f"{n_sm} SMs x {FP32_LANES_PER_SM} lanes x {peaks['sm_max_mhz']:.0f} MHz",
                       "evals_per_frame": n_evals, "tile_pairs_per_frame": n_tile_pairs,
                       "gevals_per_s": n_evals / (ras_ms * 1e-3) / 1e9 if ras_ms > 0 else 0.0,
                       "fp32_inst_per_eval": RASTER_FP32_INST_PER_EVAL, "ms": ras_ms}
@@ -344,32 +368,105 @@ def run_higs(args) -> int:
            "resident_scene": {"value": aggregate_fps(args.steps, world, res_secs), "unit": UNIT, "h2d_bytes_per_step": 80,
                               "d2h_bytes_per_step": d2h, "api": "higs_scene_upload once, then higs_render_view_host per frame"}}
 
-    # -- 4K sweep (configs[4]): every orbit view, 1 warm + 3 timed frames each --
+    # -- load map (Fig. 1): per render tile, gaussians that pass the per-tile test / units of its macro-tile --
+    def load_map(cams, W, H, out, view):
+        hg.higs_set_flags(ctx, args.flags | hg.HIGS_FLAG_COUNT_EVALS | hg.HIGS_FLAG_NO_XBATCH_CUT)
+        hg.higs_render(ctx, *dev, scene.degree, cams[view], W, H, out, stream.cuda_stream)
+        ls = hg.higs_get_lists(ctx)
+        hg.higs_set_flags(ctx, args.flags)
+        nb = np.diff(ls["batch_offset"]).astype(np.float64)
+        tl = ls["tile_load"].astype(np.float64)
+        has = nb > 0
+        per_unit = tl[has] / nb[has, None]                    # what one (macro-tile, batch) unit brings to the tile on average
+        touched = tl[has] > 0
+        seg = ls["mt_count"].astype(np.int64)
+        unit_len = np.concatenate([np.minimum(args.batch_cap, np.maximum(0, n - args.batch_cap * np.arange((n + args.batch_cap - 1) // args.batch_cap)))
+                                   for n in seg[seg > 0]]) if (seg > 0).any() else np.zeros(1)
+        return {"view": view, "per_tile_gaussians_max": float(tl.max()), "per_tile_gaussians_mean": float(tl[has][touched].mean()) if touched.any() else 0.0,
+                "per_tile_load_per_unit_max": float(per_unit.max()) if has.any() else 0.0,
+                "per_tile_load_per_unit_mean": float(per_unit[touched].mean()) if touched.any() else 0.0,
+                "unit_len_max": int(unit_len.max()), "unit_len_mean": float(unit_len.mean()), "n_units": int(ls["n_units"]),
+                "what": "per render tile: gaussians overlapping the tile (inline visibility test, no cross-batch cut) summed over the macro-tile's "
+                        "units = the per-tile list length of a per-tile renderer; divided by the units of the macro-tile = the per-unit load"}
+    load_1080 = load_map(ccams_1080, 1920, 1080, img, 0)
+
+    # -- 4K sweep (configs[4]): every orbit view, timed like the 1080p number (no stage events inside the timed frames) --
     fps_4k = None
     if not args.no_4k:
         img4 = torch.empty((2160, 3840, 3), dtype=torch.float32, device=f"cuda:{local}")
-        hg.higs_set_flags(ctx, args.flags | hg.HIGS_FLAG_STAGE_TIMERS)
         per_view, st4 = [], []
         my_views = [v for v in range(n_views) if v % world == rank]
+        reps = max(3, args.reps_4k)
         for v in my_views:
-            ms = []
-            for rep in range(4):
+            hg.higs_set_flags(ctx, args.flags)
+            for _ in range(2):
                 hg.higs_render(ctx, *dev, scene.degree, ccams_4k[v], 3840, 2160, img4, stream.cuda_stream)
-                s = hg.higs_get_stats(ctx)
-                if rep:
-                    ms.append(s["ms_total"])
-            per_view.append(1000.0 / float(np.median(ms)))
-            st4.append(s)
+            ev4 = [torch.cuda.Event(enable_timing=True) for _ in range(reps + 1)]
+            ev4[0].record(stream)
+            for r_ in range(reps):
+                hg.higs_render(ctx, *dev, scene.degree, ccams_4k[v], 3840, 2160, img4, stream.cuda_stream)
+                ev4[r_ + 1].record(stream)
+            torch.cuda.synchronize()
+            per_view.append(1000.0 / float(np.median([ev4[r_].elapsed_time(ev4[r_ + 1]) for r_ in range(reps)])))
+            hg.higs_set_flags(ctx, args.flags | hg.HIGS_FLAG_STAGE_TIMERS)     # one more frame for the stage breakdown
+            hg.higs_render(ctx, *dev, scene.degree, ccams_4k[v], 3840, 2160, img4, stream.cuda_stream)
+            st4.append(hg.higs_get_stats(ctx))
         hg.higs_set_flags(ctx, args.flags)
         pv = np.array(per_view)
-        fps_4k = {"workload": "configs[4]: same scene at 3840x2160, 32 orbit views", "views": len(my_views),
+        fps_4k = {"workload": "configs[4]: same scene at 3840x2160, 32 orbit views", "views": len(my_views), "frames_per_view": reps,
+                  "timing": "median over the frames of a view, CUDA events between frames, no stage events",
                   "median": float(np.median(pv)), "min": float(pv.min()), "max": float(pv.max()),
                   "per_view": [round(float(x), 1) for x in pv],
-                  "stages_ms_mean": {k: float(np.mean([s["ms_" + k] for s in st4])) for k in stage_names},
-                  "n_pairs_mean": float(np.mean([s["n_pairs"] for s in st4])), "n_units_mean": float(np.mean([s["n_units"] for s in st4])),
-                  "unit_load_mean": float(np.mean([s["n_pairs"] / max(1, s["n_units"]) for s in st4])), "unit_load_max": 1024,
-                  "max_segment": int(max(s["max_segment"] for s in st4))}
+                  "stages_ms_mean": {k: float(np.mean([s_["ms_" + k] for s_ in st4])) for k in stage_names},
+                  "n_pairs_mean": float(np.mean([s_["n_pairs"] for s_ in st4])), "n_units_mean": float(np.mean([s_["n_units"] for s_ in st4])),
+                  "unit_load_mean": float(np.mean([s_["n_pairs"] / max(1, s_["n_units"]) for s_ in st4])),
+                  "max_segment": int(max(s_["max_segment"] for s_ in st4)),
+                  "load_map": [load_map(ccams_4k, 3840, 2160, img4, v) for v in (0, 8, 16, 24) if v in my_views]}
         del img4
+
+    # -- variants: fp16 data path, 16x16 render tiles, 32-byte SH codes; same views, same timing --
+    variants = None
+    if not args.no_variants:
+        def timed(render, n):
+            for i in range(3):
+                render(i)
+            evv = [torch.cuda.Event(enable_timing=True) for _ in range(n + 1)]
+            evv[0].record(stream)
+            for i in range(n):
+                render(args.warmup + i)
+                evv[i + 1].record(stream)
+            torch.cuda.synchronize()
+            return evv[0].elapsed_time(evv[-1]) / n
+
+        def stage_means(render, n):
+            rows_ = []
+            for i in range(n):
+                render(args.warmup + i)
+                s_ = hg.higs_get_stats(ctx)
+                rows_.append([s_["ms_" + k] for k in stage_names])
+            return dict(zip(stage_names, np.mean(np.array(rows_), axis=0).tolist()))
+
+        nv = min(args.steps, 32)
+        variants = {}
+        def run_variant(name, flags, render, note):
+            hg.higs_set_flags(ctx, args.flags | flags)
+            ms = timed(render, nv)
+            hg.higs_set_flags(ctx, args.flags | flags | hg.HIGS_FLAG_STAGE_TIMERS)
+            variants[name] = {"fps": 1000.0 / ms, "ms_per_frame": ms, "stages_ms_mean": stage_means(render, min(nv, 8)), "note": note}
+            hg.higs_set_flags(ctx, args.flags)
+        run_variant("fp32_8x8", 0, frame, "the headline configuration, re-timed here over the same frames as the variants")
+        run_variant("fp16_8x8", hg.HIGS_FLAG_FP16, frame,
+                    "PAPER.md:180-226, 280: Cholesky conics, tile-unit coordinates, half2 blending, 16 KB fp16 partials per unit (fp32: 32 KB)")
+        hg.higs_set_tile(ctx, 16)
+        run_variant("fp32_16x16", 0, frame, "PAPER.md:286-299 (Table 2): 16x16 render tiles, macro-tiles of 128x64 px")
+        run_variant("fp16_16x16", hg.HIGS_FLAG_FP16, frame, "both")
+        hg.higs_set_tile(ctx, 8)
+        hg.higs_scene_upload(ctx, *[np.ascontiguousarray(a, dtype=np.float32) for a in (scene.means, scene.scales, scene.quats, scene.opacities, scene.sh)], scene.degree)
+        hg.higs_scene_compress_sh(ctx)
+        view = lambda i: hg.higs_render_view(ctx, ccams_1080[views_for_rank(i, rank, world, n_views)], 1920, 1080, img, stream.cuda_stream)
+        run_variant("resident_fp32sh", 0, view, "resident scene (higs_scene_upload + higs_render_view), 192-byte fp32 SH rows")
+        run_variant("resident_sh32", hg.HIGS_FLAG_SH32, view, "PAPER.md:245: 32-byte SH codes decoded inline in the projection kernel")
+        run_variant("resident_sh32_fp16", hg.HIGS_FLAG_SH32 | hg.HIGS_FLAG_FP16, view, "the paper's default configuration: fp16 data path + 32-byte SH")
 
     hg.higs_destroy(ctx)
     if rank == 0:
@@ -391,13 +488,14 @@ def run_higs(args) -> int:
     if rank != 0:
         return 0
     line = {"metric": METRIC, "value": fps, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": 1000.0 * secs / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": 1000.0 * secs / args.steps, "ms_per_step_median": float(np.median(frame_ms)),
+            "fps_from_median_frame": 1000.0 / float(np.median(frame_ms)), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic", "config": workload_config(scene, args, world),
             "clocks": clocks, "gpu_launches": launches_per_frame * args.steps, "gpu_launches_per_frame": launches_per_frame,
             "roofline": dict(roof[dominant], kernel=dominant), "stages": {"ms_mean": stage_ms, "ms_median": stage_med, "roofline": roof},
             "frame": {"n_visible": n_vis, "n_pairs": n_pairs, "n_units": n_units, "max_segment": mean_of("max_segment"),
-                      "n_oversize": mean_of("n_oversize"), "unit_load_mean": n_pairs / max(1.0, n_units), "unit_load_max": 1024},
-            "e2e": e2e, "fps_4k": fps_4k, "cpu_baseline": cpu_baseline,
+                      "n_oversize": mean_of("n_oversize"), "unit_load_mean": n_pairs / max(1.0, n_units), "load_map": load_1080},
+            "e2e": e2e, "fps_4k": fps_4k, "variants": variants, "cpu_baseline": cpu_baseline,
             "paper_context": "1,124 FPS at 1080p on a 5.8 M-gaussian scene, RTX PRO 6000 Blackwell, fp16 + 32-byte SH (PAPER.md:9): other hardware, other scene, not a target"}
     print(json.dumps(line), flush=True)
     return 0
@@ -414,6 +512,8 @@ def main() -> int:
     ap.add_argument("--flags", type=int, default=0, help="extra HIGS_FLAG_* bits for every frame (4 = no cross-batch cut, 8 = merge-sort tiers)")
     ap.add_argument("--no-4k", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-variants", action="store_true", help="skip the fp16 / 16x16 / SH32 variant timings")
+    ap.add_argument("--reps-4k", type=int, default=5, help="timed frames per 4K view (median)")
     ap.add_argument("--e2e-steps", type=int, default=16)
     ap.add_argument("--cpu-stride", type=int, default=1, help="cpu_baseline renders every k-th gaussian (1 = the whole frame)")
     ap.add_argument("--ref-stride", type=int, default=1, help="--impl reference renders every k-th gaussian per step")

@@ -98,6 +98,9 @@ typedef struct {
     const uint32_t* batch_offset;    /* [N_M+1]   exclusive prefix sum of ceil(n_m/B_r)           */
     const uint64_t* pairs;           /* [n_pairs] (key << 32 | id), each segment ascending        */
     const uint32_t* unit_active;     /* [n_units] 32-bit active-tile mask per unit  */
+    const uint32_t* tile_load;       /* [N_M][32] per render tile: gaussians that passed the inline visibility test, summed over
+                                        the macro-tile's units - the load map of PAPER.md:9 (Fig. 1); only filled with
+                                        HIGS_FLAG_COUNT_EVALS (use HIGS_FLAG_NO_XBATCH_CUT as well for the uncut load)     */
 } higs_lists;
 
 /* Per-gaussian records of the last frame.  DEVICE pointers owned by the context. */

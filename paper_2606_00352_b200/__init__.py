@@ -45,7 +45,7 @@ class higs_stats(C.Structure):
 
 class higs_lists(C.Structure):
     _fields_ = [("n_pairs", C.c_int64), ("n_units", C.c_int64), ("n_mt", C.c_int32), ("mt_count", C.c_void_p),
-                ("mt_offset", C.c_void_p), ("batch_offset", C.c_void_p), ("pairs", C.c_void_p), ("unit_active", C.c_void_p)]
+                ("mt_offset", C.c_void_p), ("batch_offset", C.c_void_p), ("pairs", C.c_void_p), ("unit_active", C.c_void_p), ("tile_load", C.c_void_p)]
 
 
 class higs_records(C.Structure):
@@ -237,7 +237,8 @@ def higs_get_lists(ctx) -> dict:
             "mt_offset": _dev_to_numpy(ctx, ls.mt_offset, nm + 1, np.uint32),
             "batch_offset": _dev_to_numpy(ctx, ls.batch_offset, nm + 1, np.uint32),
             "keys": (pairs >> np.uint64(32)).astype(np.uint32), "ids": (pairs & np.uint64(0xffffffff)).astype(np.uint32),
-            "unit_active": _dev_to_numpy(ctx, ls.unit_active, nun, np.uint32)}
+            "unit_active": _dev_to_numpy(ctx, ls.unit_active, nun, np.uint32),
+            "tile_load": _dev_to_numpy(ctx, ls.tile_load, nm * HIGS_MT_TILES, np.uint32).reshape(nm, HIGS_MT_TILES)}
 
 
 def higs_get_records(ctx) -> dict:

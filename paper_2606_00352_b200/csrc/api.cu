@@ -186,6 +186,7 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     if ((rc = dev_alloc(ctx, &ctx->part_desc, (size_t)ctx->n_part_max))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->hist, (size_t)ctx->n_part_max * nm))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->cut_word, (size_t)nm * HIGS_MT_TILES))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->tile_load, (size_t)nm * HIGS_MT_TILES))) return fail(rc);
     static_assert(sizeof(FrameHeader) <= sizeof(uint32_t) * HIGS_HDR_WORDS, "frame header outgrew its block");
     if ((rc = dev_alloc(ctx, &ctx->hdr_block, HIGS_HDR_WORDS + 2 * ((size_t)nm + 1)))) return fail(rc);
     ctx->hdr = reinterpret_cast<FrameHeader*>(ctx->hdr_block);
@@ -233,7 +234,7 @@ void higs_destroy(higs_ctx* ctx)
     dev_free(ctx->mt_offset); dev_free(ctx->batch_offset); dev_free(ctx->unit_mt);
     dev_free(ctx->unit_active); dev_free(ctx->pairs); dev_free(ctx->pairs_alt); dev_free(ctx->sort_jobs);
     dev_free(ctx->over_segs); dev_free(ctx->split_segs); dev_free(ctx->splitters); dev_free(ctx->bucket_count);
-    dev_free(ctx->bucket_cursor); dev_free(ctx->partial); dev_free(ctx->cut_word); dev_free(ctx->cut_term);
+    dev_free(ctx->bucket_cursor); dev_free(ctx->partial); dev_free(ctx->cut_word); dev_free(ctx->cut_term); dev_free(ctx->tile_load);
     dev_free(ctx->unit_order); dev_free(ctx->level_hist); dev_free(ctx->level_cur);
     dev_free(ctx->s_means); dev_free(ctx->s_scales); dev_free(ctx->s_quats); dev_free(ctx->s_opac); dev_free(ctx->s_sh);
     dev_free(ctx->s_img); dev_free(ctx->s_sh32); dev_free(ctx->sh32_work);
@@ -402,7 +403,7 @@ int higs_get_lists(higs_ctx* ctx, higs_lists* out)
         HIGS_CUDA(ctx, cudaStreamSynchronize(ctx->last_stream));
     }
     out->n_pairs = h.n_pairs; out->n_units = h.n_units; out->n_mt = ctx->last_nm;
-    out->mt_count = ctx->mt_count; out->mt_offset = ctx->mt_offset; out->batch_offset = ctx->batch_offset;
+    out->mt_count = ctx->mt_count; out->mt_offset = ctx->mt_offset; out->batch_offset = ctx->batch_offset; out->tile_load = ctx->tile_load;
     out->pairs = reinterpret_cast<const uint64_t*>(ctx->pairs_alt); out->unit_active = ctx->unit_active;
     return h.overflow ? HIGS_E_CAPACITY : HIGS_OK;
 }

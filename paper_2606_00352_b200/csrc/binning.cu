@@ -126,7 +126,7 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
        const uint4* __restrict__ bin, const float4* __restrict__ rec,
        const FrameParams P, const uint32_t* __restrict__ hist, uint32_t* __restrict__ mt_fill, const uint32_t* __restrict__ mt_offset,
        unsigned long long* __restrict__ pairs, const FrameHeader* __restrict__ hdr,
-       unsigned long long* __restrict__ cut_word, int* __restrict__ cut_term)
+       unsigned long long* __restrict__ cut_word, int* __restrict__ cut_term, uint32_t* __restrict__ tile_load)
 {
     extern __shared__ uint32_t s_cursor[];
     uint32_t* s_chunk = s_cursor + P.n_m;           // [lcap]
@@ -144,6 +144,8 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
         for (size_t i = (size_t)blockIdx.x * BIN_THREADS + threadIdx.x; i < n_word; i += stride) cut_word[i] = 0ull;
         for (size_t i = (size_t)blockIdx.x * BIN_THREADS + threadIdx.x; i < n_term; i += stride) cut_term[i] = 0;
     }
+    if (P.flags & HIGS_FLAG_COUNT_EVALS)
+        for (size_t i = (size_t)blockIdx.x * BIN_THREADS + threadIdx.x; i < (size_t)P.n_m * HIGS_MT_TILES; i += (size_t)gridDim.x * BIN_THREADS) tile_load[i] = 0u;
     const uint32_t b = blockIdx.x;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const uint2 pd = part_desc[b];
@@ -270,7 +272,7 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
     HIGS_CUDA(ctx, launch_pdl(k_fill, dim3(n_b), dim3(BIN_THREADS), smem, st, ctx->chunk_count, ctx->part_list, ctx->part_desc, lcap, ctx->bin,
-                              ctx->rec, P, ctx->hist, ctx->mt_fill, ctx->mt_offset, ctx->pairs, ctx->hdr, ctx->cut_word, ctx->cut_term));
+                              ctx->rec, P, ctx->hist, ctx->mt_fill, ctx->mt_offset, ctx->pairs, ctx->hdr, ctx->cut_word, ctx->cut_term, ctx->tile_load));
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }

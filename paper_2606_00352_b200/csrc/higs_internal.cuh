@@ -111,6 +111,8 @@ struct higs_ctx {
     unsigned long long* cut_word;  // [max_nm][32] cross-batch cut: (k << 32 | sum of the terms of batches 0 .. k-1), a cached prefix (raster.cu)
     int*      cut_term;        // [max_units][32] log2(largest transmittance the unit left in the tile) x 1024, rounded towards zero, minus 1;
                                //             0 = not published.  Both are zeroed every frame by k_fill
+    uint32_t* tile_load;       // [max_nm][32] gaussians that passed the per-tile visibility test, summed over the macro-tile's units;
+                               //             only with HIGS_FLAG_COUNT_EVALS (zeroed by k_fill)
     FrameHeader* hdr;          // device
     FrameHeader* hdr_host;     // pinned
     // resident scene / host staging

@@ -177,7 +177,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
          const uint32_t* __restrict__ unit_order,
          const FrameParams P, FrameHeader* __restrict__ hdr,
          float4* __restrict__ partial, uint32_t* __restrict__ unit_active,
-         unsigned long long* __restrict__ cut_word, int* __restrict__ cut_term)
+         unsigned long long* __restrict__ cut_word, int* __restrict__ cut_term, uint32_t* __restrict__ tile_load)
 {
     typedef TileGeo<TILE> G;
     constexpr int NP = G::NP;
@@ -331,6 +331,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             uint32_t rank = 0;
 #pragma unroll
             for (int o = 0; o < 32; ++o) rank += __shfl_sync(0xffffffffu, key, o) > key ? 1u : 0u;
+            if (COUNT && cnt) atomicAdd(tile_load + (size_t)m * HIGS_MT_TILES + lane, cnt);   // Fig. 1 load map
             if (cnt) S.order[rank] = (uint8_t)lane;
             else if (use_cut && !((cut >> lane) & 1u)) cut_term[(size_t)u * HIGS_MT_TILES + lane] = -1;
             const uint32_t nt = __popc(__ballot_sync(0xffffffffu, cnt != 0u));
@@ -594,7 +595,7 @@ void launch_one(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
     const int grid = ctx->n_sm * ctx->raster_ctas_per_sm[TILE == 16][HALF];
     k_raster<COUNT, TILE, HALF><<<grid, RAS_THREADS, ras_smem_bytes<HALF>(), st>>>(
         ctx->pairs, ctx->rec, ctx->rec16, ctx->mt_offset, ctx->mt_count, ctx->batch_offset, ctx->unit_mt, ctx->unit_order, P, ctx->hdr,
-        ctx->partial, ctx->unit_active, ctx->cut_word, ctx->cut_term);
+        ctx->partial, ctx->unit_active, ctx->cut_word, ctx->cut_term, ctx->tile_load);
 }
 
 } // namespace

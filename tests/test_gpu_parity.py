@@ -437,6 +437,33 @@ def test_sh32_codec_bytes_and_render(hg):
     hg.higs_destroy(ctx)
 
 
+def test_tile_load_map_counts_cover_the_exact_per_tile_lists(hg):
+    """The Fig.-1 load map: with HIGS_FLAG_COUNT_EVALS | HIGS_FLAG_NO_XBATCH_CUT tile_load[m][t] counts the
+    gaussians whose inline visibility test touches render tile t of macro-tile m.  The test is conservative, so every count
+    is at least the exact number of gaussians whose threshold ellipse meets the tile (the oracle's row scan at 8-px cells)
+    and, summed over the frame, within a few percent of it."""
+    s = hs.scene_cfg1(N=20_000, W=320, H=240)
+    cam = s.cameras[0]
+    r, _ = _render(hg, s, cam, flags=hg.HIGS_FLAG_COUNT_EVALS | hg.HIGS_FLAG_NO_XBATCH_CUT, batch_cap=256)
+    tl = r.lists()["tile_load"]
+    pr = oracle.project(s, cam)
+    ntx, nty = (cam.W + 7) // 8, (cam.H + 7) // 8
+    exact = np.zeros(ntx * nty, np.int64)
+    for i in np.nonzero(pr.valid)[0]:
+        np.add.at(exact, oracle.scan(pr.geo[i], cam.W, cam.H, 8, 8), 1)
+    exact = exact.reshape(nty, ntx)
+    nmx = (cam.W + 63) // 64
+    got = np.zeros_like(exact)
+    for m in range(tl.shape[0]):
+        for t in range(32):
+            ty, tx = (m // nmx) * 4 + (t >> 3), (m % nmx) * 8 + (t & 7)
+            if ty < nty and tx < ntx:
+                got[ty, tx] = tl[m, t]
+    assert (got >= exact).all()
+    assert got.sum() <= 1.05 * exact.sum() + 64
+    r.close()
+
+
 def test_frame_captures_into_a_cuda_graph(hg):
     """higs_render only enqueues (no host synchronisation): a whole frame - memsets, 18 kernels on the
     render stream and the forked sort streams, the cooperative merge kernel, the PDL edges - captures into a CUDA graph,
