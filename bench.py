@@ -332,41 +332,43 @@ def run_higs(args) -> int:
                       "fp32_inst_per_eval": RASTER_FP32_INST_PER_EVAL, "ms": ras_ms}
     dominant = max(("project", "fill", "sort", "raster"), key=lambda k: stage_ms[k])
 
-    # -- e2e: the same frames through higs_render_host (pinned host arrays in, host image out) --
-    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
-    host = [pin(scene.means), pin(scene.scales), pin(scene.quats), pin(scene.opacities), pin(scene.sh)]
-    host_img = torch.empty((1080, 1920, 3), dtype=torch.float32).pin_memory()
-    h2d = sum(int(t.numel()) * 4 for t in host) + 80
-    d2h = int(host_img.numel()) * 4
-    def e2e_frame(i):
-        hg.higs_render_host(ctx, *host, scene.degree, ccams_1080[views_for_rank(i, rank, world, n_views)], 1920, 1080, host_img)
-    e2e_steps = max(1, min(args.steps, args.e2e_steps))
-    for i in range(min(args.warmup, 3)):
-        e2e_frame(i)
-    barrier()
-    t0 = time.perf_counter()
-    for i in range(e2e_steps):
-        e2e_frame(args.warmup + i)
-    barrier()
-    e2e_secs = time.perf_counter() - t0
-    # resident-scene variant: per frame only the camera goes in and the image comes out
-    hg.higs_scene_upload(ctx, *host, scene.degree)
-    for i in range(3):
-        hg.higs_render_view_host(ctx, ccams_1080[i % n_views], 1920, 1080, host_img)
-    barrier()
-    t0 = time.perf_counter()
-    for i in range(args.steps):
-        hg.higs_render_view_host(ctx, ccams_1080[views_for_rank(args.warmup + i, rank, world, n_views)], 1920, 1080, host_img)
-    barrier()
-    res_secs = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_secs, res_secs], dtype=torch.float64, device=f"cuda:{local}")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_secs, res_secs = (float(x) for x in t.tolist())
-    e2e = {"value": aggregate_fps(e2e_steps, world, e2e_secs), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-           "steps": e2e_steps, "api": "higs_render_host (all five arrays uploaded from pinned host memory every frame)",
-           "resident_scene": {"value": aggregate_fps(args.steps, world, res_secs), "unit": UNIT, "h2d_bytes_per_step": 80,
-                              "d2h_bytes_per_step": d2h, "api": "higs_scene_upload once, then higs_render_view_host per frame"}}
+    e2e = None
+    if not args.no_e2e:
+        # -- e2e: the same frames through higs_render_host (pinned host arrays in, host image out) --
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
+        host = [pin(scene.means), pin(scene.scales), pin(scene.quats), pin(scene.opacities), pin(scene.sh)]
+        host_img = torch.empty((1080, 1920, 3), dtype=torch.float32).pin_memory()
+        h2d = sum(int(t.numel()) * 4 for t in host) + 80
+        d2h = int(host_img.numel()) * 4
+        def e2e_frame(i):
+            hg.higs_render_host(ctx, *host, scene.degree, ccams_1080[views_for_rank(i, rank, world, n_views)], 1920, 1080, host_img)
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        for i in range(min(args.warmup, 3)):
+            e2e_frame(i)
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(e2e_steps):
+            e2e_frame(args.warmup + i)
+        barrier()
+        e2e_secs = time.perf_counter() - t0
+        # resident-scene variant: per frame only the camera goes in and the image comes out
+        hg.higs_scene_upload(ctx, *host, scene.degree)
+        for i in range(3):
+            hg.higs_render_view_host(ctx, ccams_1080[i % n_views], 1920, 1080, host_img)
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(args.steps):
+            hg.higs_render_view_host(ctx, ccams_1080[views_for_rank(args.warmup + i, rank, world, n_views)], 1920, 1080, host_img)
+        barrier()
+        res_secs = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([e2e_secs, res_secs], dtype=torch.float64, device=f"cuda:{local}")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_secs, res_secs = (float(x) for x in t.tolist())
+        e2e = {"value": aggregate_fps(e2e_steps, world, e2e_secs), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "steps": e2e_steps, "api": "higs_render_host (all five arrays uploaded from pinned host memory every frame)",
+               "resident_scene": {"value": aggregate_fps(args.steps, world, res_secs), "unit": UNIT, "h2d_bytes_per_step": 80,
+                                  "d2h_bytes_per_step": d2h, "api": "higs_scene_upload once, then higs_render_view_host per frame"}}
 
     # -- load map (Fig. 1): per render tile, gaussians that pass the per-tile test / units of its macro-tile --
     def load_map(cams, W, H, out, view):
@@ -512,6 +514,7 @@ def main() -> int:
     ap.add_argument("--flags", type=int, default=0, help="extra HIGS_FLAG_* bits for every frame (4 = no cross-batch cut, 8 = merge-sort tiers)")
     ap.add_argument("--no-4k", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end legs (gaussian-count sweeps beyond host memory for pinned copies)")
     ap.add_argument("--no-variants", action="store_true", help="skip the fp16 / 16x16 / SH32 variant timings")
     ap.add_argument("--reps-4k", type=int, default=5, help="timed frames per 4K view (median)")
     ap.add_argument("--e2e-steps", type=int, default=16)

@@ -30,11 +30,12 @@ def stale() -> bool:
     return any(p.stat().st_mtime > t for p in _deps())
 
 
-def build(force: bool = False, verbose: bool = False) -> Path:
-    if not force and not stale():
+def build(force: bool = False, verbose: bool = False, debug_bounds: bool = False) -> Path:
+    """debug_bounds: compile with -DHIGS_DEBUG_BOUNDS (device asserts on the frame's indexed writes, higs_internal.cuh)."""
+    if not force and not stale() and not debug_bounds:
         return LIB
     LIB.parent.mkdir(parents=True, exist_ok=True)
-    cmd = ["nvcc", *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", str(LIB), *[str(CSRC / s) for s in SOURCES]]
+    cmd = ["nvcc", *NVCC_FLAGS, *(["-DHIGS_DEBUG_BOUNDS"] if debug_bounds else []), *(["-Xptxas", "-v"] if verbose else []), "-o", str(LIB), *[str(CSRC / s) for s in SOURCES]]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
@@ -44,4 +45,4 @@ def build(force: bool = False, verbose: bool = False) -> Path:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, debug_bounds="--debug-bounds" in sys.argv))

@@ -205,6 +205,7 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     if ((rc = dev_alloc(ctx, &ctx->splitters, (size_t)ctx->max_buckets))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->bucket_count, (size_t)ctx->max_buckets))) return fail(rc);
     if ((rc = dev_alloc(ctx, &ctx->bucket_cursor, (size_t)ctx->max_buckets))) return fail(rc);
+    if ((rc = dev_alloc(ctx, &ctx->bucket_id, (size_t)max_pairs))) return fail(rc);
     if ((rc = alloc_unit_buffers(ctx))) return fail(rc);
     if (cudaMallocHost((void**)&ctx->hdr_host, sizeof(FrameHeader)) != cudaSuccess) return fail(HIGS_E_NOMEM);
     if (cudaMemset(ctx->hdr_block, 0, sizeof(uint32_t) * (HIGS_HDR_WORDS + 2 * ((size_t)nm + 1))) != cudaSuccess) return fail(HIGS_E_CUDA);
@@ -234,7 +235,7 @@ void higs_destroy(higs_ctx* ctx)
     dev_free(ctx->mt_offset); dev_free(ctx->batch_offset); dev_free(ctx->unit_mt);
     dev_free(ctx->unit_active); dev_free(ctx->pairs); dev_free(ctx->pairs_alt); dev_free(ctx->sort_jobs);
     dev_free(ctx->over_segs); dev_free(ctx->split_segs); dev_free(ctx->splitters); dev_free(ctx->bucket_count);
-    dev_free(ctx->bucket_cursor); dev_free(ctx->partial); dev_free(ctx->cut_word); dev_free(ctx->cut_term); dev_free(ctx->tile_load);
+    dev_free(ctx->bucket_cursor); dev_free(ctx->bucket_id); dev_free(ctx->partial); dev_free(ctx->cut_word); dev_free(ctx->cut_term); dev_free(ctx->tile_load);
     dev_free(ctx->unit_order); dev_free(ctx->level_hist); dev_free(ctx->level_cur);
     dev_free(ctx->s_means); dev_free(ctx->s_scales); dev_free(ctx->s_quats); dev_free(ctx->s_opac); dev_free(ctx->s_sh);
     dev_free(ctx->s_img); dev_free(ctx->s_sh32); dev_free(ctx->sh32_work);

@@ -111,7 +111,9 @@ k_plan(const FrameParams P,
         while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_bo[mid] <= u) lo = mid; else hi = mid - 1; }
         unit_mt[u] = (uint32_t)lo;
         const uint32_t lvl = u - s_bo[lo];
-        unit_order[atomicAdd(&level_cur[lvl], 1u)] = u;
+        const uint32_t at = atomicAdd(&level_cur[lvl], 1u);
+        HIGS_ASSERT(at < n_units && lvl < max_nb);
+        unit_order[at] = u;
     }
 }
 
@@ -191,7 +193,11 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
         for (int r = rs.r0; r <= rs.r1; ++r) {
             int m0, m1;
             if (!rs.row(r, (float)(8 * P.tile), (float)(4 * P.tile), fW, fH, P.n_mx, m0, m1)) continue;
-            for (int m = m0; m <= m1; ++m) pairs[atomicAdd(&s_cursor[r * P.n_mx + m], 1u)] = item;
+            for (int m = m0; m <= m1; ++m) {
+                const uint32_t at = atomicAdd(&s_cursor[r * P.n_mx + m], 1u);
+                HIGS_ASSERT(at >= mt_offset[r * P.n_mx + m] && at < mt_offset[r * P.n_mx + m + 1]);
+                pairs[at] = item;
+            }
         }
     };
     auto emit = [&](size_t slot, const uint4 bn) {  // bn = key, desc lo, desc hi, id
@@ -204,7 +210,11 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
                 const int m0 = (int)(f & 511u);
                 if (m0 == 511) continue;
                 const int cell0 = (r0 + rr) * P.n_mx + m0, wd = (int)(f >> 9);
-                for (int m = 0; m <= wd; ++m) pairs[atomicAdd(&s_cursor[cell0 + m], 1u)] = item;
+                for (int m = 0; m <= wd; ++m) {
+                    const uint32_t at = atomicAdd(&s_cursor[cell0 + m], 1u);
+                    HIGS_ASSERT(cell0 + m < P.n_m && at >= mt_offset[cell0 + m] && at < mt_offset[cell0 + m + 1]);
+                    pairs[at] = item;
+                }
             }
         } else {                                    // span too large for the descriptor: queue it (or, queue full, do it here)
             const uint32_t qpos = atomicAdd(&s_nq, 1u);

@@ -106,6 +106,7 @@ struct higs_ctx {
     unsigned long long* splitters;   // [max_buckets]  bucket b of a segment holds items in [splitter[b-1], splitter[b])
     uint32_t* bucket_count;    // [max_buckets]
     uint32_t* bucket_cursor;   // [max_buckets]  write position of the scatter pass
+    uint8_t*  bucket_id;       // [max_pairs]  bucket of every item of an oversize segment (phase 1 of k_oversize writes, phase 2 reads)
     int64_t   max_buckets;
     float4*   partial;         // [max_units][32 tiles][64 px] (r,g,b,T)
     unsigned long long* cut_word;  // [max_nm][32] cross-batch cut: (k << 32 | sum of the terms of batches 0 .. k-1), a cached prefix (raster.cu)
@@ -174,6 +175,16 @@ int launch_sort(higs_ctx*, const FrameParams&, cudaStream_t);
 int launch_sort_only(higs_ctx*, unsigned long long* pairs, const uint32_t* seg_offset, int n_seg, cudaStream_t);
 int launch_raster(higs_ctx*, const FrameParams&, cudaStream_t);
 int launch_merge(higs_ctx*, const FrameParams&, float* out_rgb, cudaStream_t);
+
+// ---- bounds checks of a debug build (python -m paper_2606_00352_b200.build --debug-bounds): compute-sanitizer is not
+// available on the GPU pool, so the indexed writes of the frame carry device asserts that the test suite runs through once
+// per round (profiles/r02_sanitizer.md).  A failed assert traps: the next CUDA call of the test fails loudly.
+#ifdef HIGS_DEBUG_BOUNDS
+#include <assert.h>
+#define HIGS_ASSERT(c) assert(c)
+#else
+#define HIGS_ASSERT(c) ((void)0)
+#endif
 
 // ---- device helpers ----------------------------------------------------------------------------
 __device__ __forceinline__ float clampf_(float v, float lo, float hi) { return fminf(fmaxf(v, lo), hi); }

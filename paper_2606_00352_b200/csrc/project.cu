@@ -23,6 +23,17 @@
 #define HIGS_LD __ldg
 namespace {
 
+// SH rows of the survivors are scattered 192-byte reads: ask L2 for 64-byte fills only (a row is three of them)
+__device__ __forceinline__ float4 ld_sh64(const float4* p)
+{
+    float4 v;
+    asm volatile("ld.global.nc.L2::64B.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+#ifndef HIGS_LD_SH
+#define HIGS_LD_SH HIGS_LD   /* ld_sh64 measured: no change (0.273 against 0.268 ms), DRAM over-fetch of the scattered rows stays */
+#endif
+
 // ln_spec (DESIGN.md N-LN): frexp + atanh series, separate mul and add, x in (1, 255].
 __device__ __forceinline__ float ln_spec(float x)
 {
@@ -57,7 +68,7 @@ __device__ __forceinline__ void sh_accumulate(const float* __restrict__ shp, flo
         const float4* p4 = reinterpret_cast<const float4*>(shp);
 #pragma unroll
         for (int k = 0; k < K * 3 / 4; ++k) {
-            float4 v = HIGS_LD(p4 + k);
+            float4 v = HIGS_LD_SH(p4 + k);
             c[4 * k] = v.x; c[4 * k + 1] = v.y; c[4 * k + 2] = v.z; c[4 * k + 3] = v.w;
         }
     } else {
@@ -276,6 +287,7 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
             int m0, m1;
             uint32_t field = 511u;
             if (rs.row(r, (float)(8 * P.tile), (float)(4 * P.tile), fW, fH, P.n_mx, m0, m1)) {
+                HIGS_ASSERT(r >= 0 && r < P.n_my && m0 >= 0 && m1 < P.n_mx);
                 for (int m = m0; m <= m1; ++m) atomicAdd(&s_hist[r * P.n_mx + m], 1u);
                 fits = fits && (m1 - m0) <= 15;
                 field = (uint32_t)m0 | ((uint32_t)((m1 - m0) & 15) << 9);

@@ -259,6 +259,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
         const int len = (int)min((uint32_t)P.batch_cap, seg_n - j * (uint32_t)P.batch_cap);
         const int mtx = (int)(m % (uint32_t)P.n_mx), mty = (int)(m / (uint32_t)P.n_mx);
         const float X0 = (float)(mtx * G::MT_W), Y0 = (float)(mty * G::MT_H);
+        HIGS_ASSERT(u < P.max_units && m < (uint32_t)P.n_m && len > 0 && len <= RAS_SUB && start + (uint32_t)len <= hdr->n_pairs);
 
         if constexpr (!HALF) {
             // ---- Phase 1a: gather of this unit's records (Alg. 1 line 4), first 48 B of each, by sorted id ----
@@ -380,6 +381,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
                     uint32_t pos = incl - __popc(bits);
                     const uint32_t base = rec_s + (uint32_t)(lane * 32) * RasLayout<HALF>::stride;
                     while (bits) {
+                        HIGS_ASSERT(pos < (uint32_t)RING);
                         ring[pos++] = base + (uint32_t)(__ffs(bits) - 1) * RasLayout<HALF>::stride;
                         bits &= bits - 1;
                     }

@@ -97,14 +97,21 @@ __device__ __forceinline__ void block_sort_smem(u64* buf, int n, int n_pad)
                 const int mid = (lo + hi) >> 1;
                 if (buf[sidx(A + mid)] < buf[sidx(B + diag - 1 - mid)]) lo = mid + 1; else hi = mid;
             }
+            // serial two-pointer merge of this thread's 16 outputs, branch-free: an exhausted run reads as ~0, which no item
+            // equals (a depth key is the bit pattern of a finite positive float), so one 64-bit compare decides; one predicated
+            // shared load per output refills the side that was consumed
             int ia = lo, ib = diag - lo;
             u64 ka = ia < na ? buf[sidx(A + ia)] : ~0ull, kb = ib < nb ? buf[sidx(B + ib)] : ~0ull;
 #pragma unroll
             for (int k = 0; k < IPT; ++k) {
-                const bool take_a = ib >= nb || (ia < na && ka < kb);
+                const bool take_a = ka < kb;
                 v[k] = take_a ? ka : kb;
-                if (take_a) { ++ia; ka = ia < na ? buf[sidx(A + ia)] : ~0ull; }
-                else        { ++ib; kb = ib < nb ? buf[sidx(B + ib)] : ~0ull; }
+                ia += take_a ? 1 : 0; ib += take_a ? 0 : 1;
+                const int nxt = take_a ? A + ia : B + ib;
+                const bool have = take_a ? ia < na : ib < nb;
+                u64 val = buf[sidx(nxt)];                        // at most one past the data: the buffer has a spare slot
+                val = have ? val : ~0ull;
+                ka = take_a ? val : ka; kb = take_a ? kb : val;
             }
         }
     }
@@ -136,6 +143,7 @@ k_block_sort(const SortJob* __restrict__ jobs, FrameHeader* __restrict__ hdr, in
         if (jb >= hdr->n_sort_jobs[list][tier]) return;
         const SortJob job = jobs[jb];
         const int n = (int)job.len;
+        HIGS_ASSERT(n >= 1 && n <= CAP);
         const u64* gsrc = ((job.flags & 2u) ? pairs_alt : pairs) + job.start;
         const int n_pad = min(CAP, ((n + IPT - 1) / IPT) * IPT);  // whole threads
         for (int i = t; i < n_pad; i += THREADS) buf[sidx(i)] = i < n ? gsrc[i] : ~0ull;
@@ -344,8 +352,8 @@ __device__ __forceinline__ uint32_t bucket_of(const u64* s_split, uint32_t n_spl
 
 constexpr int OVER_THREADS = 256;
 constexpr int SCAT_ITEMS = HIGS_SPLIT_TILE / OVER_THREADS;
-static_assert(HIGS_MAX_SPLIT <= OVER_THREADS, "one thread per bucket in the bucket scan");
-constexpr size_t OVER_BUF = sizeof(u64) * (OVER_THREADS * IPT + OVER_THREADS);    // sidx(4096) items of the sample sort
+static_assert(HIGS_MAX_SPLIT <= OVER_THREADS && HIGS_MAX_SPLIT <= 256, "one thread per bucket in the bucket scan; bucket ids are bytes");
+constexpr size_t OVER_BUF = sizeof(u64) * (OVER_THREADS * IPT + OVER_THREADS + 2);    // sidx(4096) items of the sample sort
 constexpr size_t OVER_SMEM = OVER_BUF + sizeof(u64) * HIGS_MAX_SPLIT + sizeof(uint32_t) * (2 * HIGS_MAX_SPLIT + 64);
 
 // last segment with tile_base <= tile
@@ -364,7 +372,7 @@ __device__ __forceinline__ int seg_of_tile(const SplitSeg* __restrict__ split, u
 __global__ void __launch_bounds__(OVER_THREADS)
 k_oversize(const SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr, const u64* __restrict__ pairs, u64* __restrict__ pairs_alt,
            u64* __restrict__ splitters, uint32_t* __restrict__ bucket_count, uint32_t* __restrict__ bucket_cursor,
-           SortJob* __restrict__ jobs /* list 1 */, size_t max_jobs, OverSeg* __restrict__ over)
+           SortJob* __restrict__ jobs /* list 1 */, size_t max_jobs, OverSeg* __restrict__ over, uint8_t* __restrict__ bucket_id)
 {
     extern __shared__ __align__(16) unsigned char s_raw[];
     __shared__ uint32_t s_claim;
@@ -426,7 +434,7 @@ k_oversize(const SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr, co
             const SplitSeg sg = split[si];
             __syncthreads();                                          // previous tile's shared state is free
             for (uint32_t b = t; b < sg.nb; b += OVER_THREADS) {
-                if (b + 1 < sg.nb) s_split[b] = splitters[sg.bucket_base + b];
+                if (phase == 1 && b + 1 < sg.nb) s_split[b] = splitters[sg.bucket_base + b];
                 s_hist[b] = 0;
             }
             uint32_t my_count = 0, my_start = 0;
@@ -460,8 +468,9 @@ k_oversize(const SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr, co
             for (int k = 0; k < SCAT_ITEMS; ++k) {
                 const uint32_t i = o0 + k * OVER_THREADS + t;
                 bk[k] = 0; rk[k] = 0;
-                if (i < sg.len) {
-                    bk[k] = bucket_of(s_split, sg.nb - 1, x[k]);
+                if (i < sg.len) {                                    // the search runs once: phase 2 reads the bucket back (nb <= 256)
+                    if (phase == 1) { bk[k] = bucket_of(s_split, sg.nb - 1, x[k]); bucket_id[sg.start + i] = (uint8_t)bk[k]; }
+                    else bk[k] = bucket_id[sg.start + i];
                     rk[k] = atomicAdd(&s_hist[bk[k]], 1u);
                 }
             }
@@ -476,7 +485,10 @@ k_oversize(const SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr, co
 #pragma unroll
                 for (int k = 0; k < SCAT_ITEMS; ++k) {
                     const uint32_t i = o0 + k * OVER_THREADS + t;
-                    if (i < sg.len) pairs_alt[s_base[bk[k]] + rk[k]] = x[k];
+                    if (i < sg.len) {
+                        HIGS_ASSERT(s_base[bk[k]] + rk[k] >= sg.start && s_base[bk[k]] + rk[k] < sg.start + sg.len);
+                        pairs_alt[s_base[bk[k]] + rk[k]] = x[k];
+                    }
                 }
                 if (tile == sg.tile_base && (uint32_t)t < sg.nb && my_count) {   // this segment's buckets -> tier jobs
                     const uint32_t n = my_count;
@@ -594,7 +606,7 @@ k_merge_levels(const OverSeg* __restrict__ over, const FrameHeader* __restrict__
 }
 
 template <int THREADS>
-constexpr size_t sort_smem() { return (size_t)(THREADS * IPT + THREADS) * sizeof(u64); }
+constexpr size_t sort_smem() { return (size_t)(THREADS * IPT + THREADS + 2) * sizeof(u64); }   // sidx(CAP) items + a spare slot read past the last run
 
 // tier t: segments / buckets of up to 1024 << t items
 template <int TIER> struct TierCfg;
@@ -652,7 +664,7 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, b
         u64* splitters = ctx->splitters; uint32_t* bc = ctx->bucket_count; uint32_t* bcur = ctx->bucket_cursor;
         size_t mj = (size_t)ctx->max_jobs; OverSeg* over = ctx->over_segs;
         HIGS_CUDA(ctx, launch_pdl(k_oversize, dim3(ctx->n_sm * ctx->over_ctas_per_sm), dim3(OVER_THREADS), OVER_SMEM, st, split, hdr, src, alt, splitters, bc, bcur,
-                                  jobs1, mj, over));
+                                  jobs1, mj, over, ctx->bucket_id));
         HIGS_LAUNCHED(ctx);
     }
     if ((rc = launch_tier<3>(ctx, 0, pairs, ms, ctx->aux_stream[0]))) return rc;
