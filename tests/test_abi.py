@@ -38,7 +38,7 @@ def test_struct_layouts_match_the_header():
     import paper_2606_00352_b200 as hg
     assert C.sizeof(hg.higs_camera) == 80
     assert C.sizeof(hg.higs_stats) == 6 * 8 + 6 * 4 + 2 * 8 + 8 * 4
-    assert C.sizeof(hg.higs_lists) == 2 * 8 + 8 + 5 * 8            # int32 n_mt padded to 8
+    assert C.sizeof(hg.higs_lists) == 2 * 8 + 8 + 6 * 8            # int32 n_mt padded to 8
     assert C.sizeof(hg.higs_records) == 8 + 2 * 8
     for macro, val in (("HIGS_TILE", hg.HIGS_TILE), ("HIGS_MT_W", hg.HIGS_MT_W), ("HIGS_MT_H", hg.HIGS_MT_H),
                        ("HIGS_MT_TILES", hg.HIGS_MT_TILES), ("HIGS_BATCH_CAP", hg.HIGS_BATCH_CAP)):
