@@ -70,6 +70,7 @@ int render_impl(higs_ctx* ctx, const float* means, const float* scales, const fl
     memcpy(P.cam, cam->cam_pos, sizeof(P.cam));
     P.W = W; P.H = H;
     P.tile = ctx->tile;
+    { const float tx = 0.65f * (float)W, ty = 0.65f * (float)H; P.limx = tx / P.fx; P.limy = ty / P.fy; }   // one rounding per op, as N-PROJ writes it
     P.n_mx = (W + 8 * P.tile - 1) / (8 * P.tile); P.n_my = (H + 4 * P.tile - 1) / (4 * P.tile); P.n_m = P.n_mx * P.n_my;
     P.degree = degree; P.batch_cap = ctx->batch_cap; P.flags = ctx->flags;
     P.max_pairs = (uint32_t)ctx->max_pairs; P.max_units = (uint32_t)ctx->max_units;

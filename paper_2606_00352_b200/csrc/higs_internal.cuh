@@ -56,6 +56,7 @@ struct FrameParams {
     int   degree;
     int   batch_cap;
     int   tile;                // render-tile edge, 8 or 16; macro-tile = 8 x 4 tiles
+    float limx, limy;          // (0.65 W) / fx, (0.65 H) / fy: the clamp of the Jacobian (N-PROJ step 3), the same for every gaussian
     uint32_t flags;
     uint32_t max_pairs, max_units;
 };
@@ -209,24 +210,31 @@ __device__ __forceinline__ float tau_scan(float a, float b, float c, float tau)
 struct RowScan {
     float mux, muy, tau, hx, hy, boc, rc, sdet, yR, nyR, ytop, ybot;
     int r0, r1;
-    __device__ __forceinline__ void init(float mux_, float muy_, float a, float b, float c, float tau_,
-                                         float fch, int ncy)
+    // tau_ = tau_s.  LEAN: cell sizes are powers of two, so x * (1 / size) is the correctly rounded x / size of the pinned
+    // sequence at the price of one multiply, and rcp.rn(c) is the correctly rounded 1 / c: same bits, fewer instructions.
+    // The lean form is used where it was measured faster (the projection kernel reading SH codes, which is bound by issue);
+    // on the DRAM-bound fp32-SH kernel it was slower (0.286 against 0.268 ms), so that one keeps the divisions.
+    template <bool LEAN = false>
+    __device__ __forceinline__ void init(float mux_, float muy_, float a, float b, float c, float tau_, float fch, int ncy)
     {
         mux = mux_; muy = muy_; tau = tau_;
         hx = __fsqrt_rn(__fmul_rn(tau, a));
         hy = __fsqrt_rn(__fmul_rn(tau, c));
         ytop = __fsub_rn(muy, hy); ybot = __fadd_rn(muy, hy);
-        r0 = (int)clampf_(floorf(__fdiv_rn(ytop, fch)), 0.0f, (float)(ncy - 1));
-        r1 = (int)clampf_(floorf(__fdiv_rn(ybot, fch)), 0.0f, (float)(ncy - 1));
+        const float rfch = 1.0f / fch;
+        r0 = (int)clampf_(floorf(LEAN ? __fmul_rn(ytop, rfch) : __fdiv_rn(ytop, fch)), 0.0f, (float)(ncy - 1));
+        r1 = (int)clampf_(floorf(LEAN ? __fmul_rn(ybot, rfch) : __fdiv_rn(ybot, fch)), 0.0f, (float)(ncy - 1));
         boc = __fdiv_rn(b, c);
-        rc = __fdiv_rn(1.0f, c);
+        rc = LEAN ? __frcp_rn(c) : __fdiv_rn(1.0f, c);
         sdet = fmaxf(0.0f, __fmaf_rn(-b, boc, a));
         yR = __fmul_rn(b, __fsqrt_rn(__fdiv_rn(tau, a)));
         nyR = -yR;
     }
     // columns [m0, m1] of row r; returns false when the row is not touched
+    template <bool LEAN = false>
     __device__ __forceinline__ bool row(int r, float fcw, float fch, float fW, float fH, int ncx, int& m0, int& m1) const
     {
+        const float rfcw = 1.0f / fcw;
         float y0 = __fmul_rn((float)r, fch);
         float y1 = fminf(__fmul_rn((float)(r + 1), fch), fH);
         float ylo = __fsub_rn(fmaxf(y0, ytop), muy);
@@ -238,8 +246,8 @@ struct RowScan {
         float xmin = (ylo <= nyR && nyR <= yhi) ? -hx : fminf(__fmaf_rn(boc, ylo, -rlo), __fmaf_rn(boc, yhi, -rhi));
         xmin = __fadd_rn(xmin, mux); xmax = __fadd_rn(xmax, mux);
         if (!(xmax > 0.0f) || !(xmin < fW)) return false;
-        m0 = (int)clampf_(floorf(__fdiv_rn(xmin, fcw)), 0.0f, (float)(ncx - 1));
-        m1 = (int)clampf_(floorf(__fdiv_rn(xmax, fcw)), 0.0f, (float)(ncx - 1));
+        m0 = (int)clampf_(floorf(LEAN ? __fmul_rn(xmin, rfcw) : __fdiv_rn(xmin, fcw)), 0.0f, (float)(ncx - 1));
+        m1 = (int)clampf_(floorf(LEAN ? __fmul_rn(xmax, rfcw) : __fdiv_rn(xmax, fcw)), 0.0f, (float)(ncx - 1));
         return true;
     }
 };

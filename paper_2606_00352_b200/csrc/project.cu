@@ -189,6 +189,7 @@ __device__ __forceinline__ RawIn load_raw(const float* __restrict__ means, const
 }
 
 // Phase A: N-PROJ steps 1-10 for one gaussian; false = culled.
+template <bool LEAN>
 __device__ __forceinline__ bool project_cull(const RawIn& in, const FrameParams& P, Survivor& s)
 {
     const float mx = in.mx, my = in.my, mz = in.mz;
@@ -203,8 +204,8 @@ __device__ __forceinline__ bool project_cull(const RawIn& in, const FrameParams&
     const float xz = __fmul_rn(xc, rz), yz = __fmul_rn(yc, rz);
     const float mux = __fmaf_rn(P.fx, xz, P.cx), muy = __fmaf_rn(P.fy, yz, P.cy);
     // 3. clamp inside the Jacobian only
-    const float limx = __fdiv_rn(__fmul_rn(0.65f, (float)P.W), P.fx);
-    const float limy = __fdiv_rn(__fmul_rn(0.65f, (float)P.H), P.fy);
+    const float limx = LEAN ? P.limx : __fdiv_rn(__fmul_rn(0.65f, (float)P.W), P.fx);     // LEAN: see RowScan (higs_internal.cuh)
+    const float limy = LEAN ? P.limy : __fdiv_rn(__fmul_rn(0.65f, (float)P.H), P.fy);
     const float txz = fminf(limx, fmaxf(-limx, xz));
     const float tyz = fminf(limy, fmaxf(-limy, yz));
     // 4. rotation from the normalised quaternion
@@ -279,14 +280,14 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
     unsigned long long desc = 0;
     {
         RowScan rs;
-        rs.init(s.mux, s.muy, s.a, s.b, s.c, tau_scan(s.a, s.b, s.c, s.tau), (float)(4 * P.tile), P.n_my);
+        rs.template init<SHC>(s.mux, s.muy, s.a, s.b, s.c, tau_scan(s.a, s.b, s.c, s.tau), (float)(4 * P.tile), P.n_my);
         const float fW = (float)P.W, fH = (float)P.H;
         bool fits = (rs.r1 - rs.r0) <= 3 && P.n_mx <= 511 && rs.r0 <= 511;
         desc = (unsigned long long)(uint32_t)rs.r0 | ((unsigned long long)(uint32_t)((rs.r1 - rs.r0) & 3) << 9);
         for (int r = rs.r0; r <= rs.r1; ++r) {
             int m0, m1;
             uint32_t field = 511u;
-            if (rs.row(r, (float)(8 * P.tile), (float)(4 * P.tile), fW, fH, P.n_mx, m0, m1)) {
+            if (rs.template row<SHC>(r, (float)(8 * P.tile), (float)(4 * P.tile), fW, fH, P.n_mx, m0, m1)) {
                 HIGS_ASSERT(r >= 0 && r < P.n_my && m0 >= 0 && m1 < P.n_mx);
                 for (int m = m0; m <= m1; ++m) atomicAdd(&s_hist[r * P.n_mx + m], 1u);
                 fits = fits && (m1 - m0) <= 15;
@@ -308,9 +309,10 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
         // fp16 data path: inverse covariance as Cholesky factors L = [[l0, 0], [l1, l2]], L L^T = conic,
         // from the covariance without cancellation: l0 = sqrt(c / det), l1 = -b / (det l0), l2 = 1 / sqrt(c); prescaled by
         // sqrt(log2 e / 2) * tile so that alpha = o * exp2(-q') with q' = (l0' dx + l1' dy)^2 + (l2' dy)^2 in tile units
+        // (smooth values, stored as half: approximate rsqrt is ample)  sqrt(c det) = det l0, so l0 = c r, l1 = -b r with r = rsqrt(c det)
         const float det = __fmaf_rn(s.a, s.c, -__fmul_rn(s.b, s.b));
-        const float l0 = sqrtf(s.c / det), l2 = rsqrtf(s.c);
-        const float l1 = -s.b / (det * l0);
+        const float rr = rsqrtf(s.c * det);
+        const float l0 = s.c * rr, l1 = -s.b * rr, l2 = rsqrtf(s.c);
         const float ks = 0.84932180f * (float)P.tile;                // sqrt(log2(e) / 2) * tile_size
         const __half2 h01 = __floats2half2_rn(l0 * ks, l1 * ks), h2o = __floats2half2_rn(l2 * ks, s.o);
         const __half2 hrg = __floats2half2_rn(r, g), hb = __floats2half2_rn(bl, 0.0f);
@@ -320,7 +322,7 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
     if (!HALF || desc == HIGS_DESC_FALLBACK) {                       // fp16 path: the fill pass reads rec only to redo the row scan of wide gaussians
         float4* rp = rec + 4 * slot;
         rp[0] = make_float4(s.mux, s.muy, s.A, s.B2);
-        rp[1] = make_float4(s.C, s.tau, log2f(s.o), r);
+        rp[1] = make_float4(s.C, s.tau, SHC ? __log2f(s.o) : log2f(s.o), r);
         rp[2] = make_float4(g, bl, s.a, s.b);
         rp[3] = make_float4(s.c, __uint_as_float(key), __uint_as_float((uint32_t)i), 0.0f);
     }
@@ -403,7 +405,7 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
             const RawIn cur = nxt;
             if (it + 1 < HIGS_CHUNK / 32 && i + 32 < N) nxt = load_raw(means, scales, quats, opac, i + 32);
             Survivor s;
-            const bool ok = (i < N) && project_cull(cur, P, s);
+            const bool ok = (i < N) && project_cull<SHC>(cur, P, s);
             const uint32_t vmask = __ballot_sync(0xffffffffu, ok);
             if (lane == 0) valid_bits[i >> 5] = vmask;               // chunk bases are multiples of 32
             if (ok) {
