@@ -132,9 +132,9 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
 {
     extern __shared__ uint32_t s_cursor[];
     uint32_t* s_chunk = s_cursor + P.n_m;           // [lcap]
-    uint32_t* s_pref = s_chunk + lcap;              // [lcap + 1] exclusive prefix of the chunk counts
+    uint32_t* s_pref = s_chunk + lcap;              // [lcap + 1] survivors of each chunk of the list
     uint32_t* s_queue = s_pref + lcap + 1;          // [2 * FILL_QCAP] (slot, key) of the gaussians with wide spans
-    __shared__ uint32_t s_nq;
+    __shared__ uint32_t s_nq, s_next;
     if (threadIdx.x == 0) s_nq = 0;
     pdl_wait(); pdl_trigger();
     if (hdr->overflow) return;                      // capacity exceeded: write nothing (HIGS_E_CAPACITY)
@@ -161,11 +161,12 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
             uint32_t x = n;
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) { const uint32_t y = __shfl_up_sync(0xffffffffu, x, d); if (lane >= d) x += y; }
-            if (e < n_list) { s_chunk[e] = c; s_pref[e] = run + x - n; }
+            if (e < n_list) { s_chunk[e] = c; s_pref[e] = n; }
             run += __shfl_sync(0xffffffffu, x, 31);
         }
         if (lane == 0) s_pref[n_list] = run;
     }
+    if (threadIdx.x == 0) s_next = 0;
     // this batch's share of every macro-tile it touches: reserved with one atomic on the macro-tile's fill counter
     // (which batch lands where inside a segment is arbitrary; the depth sort orders the segment anyway)
     for (int m = threadIdx.x; m < P.n_m; m += BIN_THREADS) {
@@ -173,12 +174,6 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
         s_cursor[m] = h ? mt_offset[m] + atomicAdd(&mt_fill[m], h) : 0u;
     }
     __syncthreads();
-    const uint32_t total = s_pref[n_list];
-    auto slot_of = [&](uint32_t k) -> size_t {
-        uint32_t lo = 0, hi = n_list - 1;           // last entry with pref <= k
-        while (lo < hi) { const uint32_t mid = (lo + hi + 1) >> 1; if (s_pref[mid] <= k) lo = mid; else hi = mid - 1; }
-        return (size_t)s_chunk[lo] * HIGS_CHUNK + (k - s_pref[lo]);
-    };
     // A gaussian whose span did not fit the descriptor (more than 4 macro-tile rows: 0.8 % of the survivors at 1080p,
     // 4.5 % at 4K) redoes the row scan, some hundreds of instructions.  Done in place it would run with one lane of the
     // warp active in a quarter (1080p) to three quarters (4K) of all warp iterations, so such gaussians are queued and
@@ -187,7 +182,7 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
         const unsigned long long item = ((unsigned long long)key << 32) | (unsigned long long)(uint32_t)slot;
         const float4 s0 = __ldcs(rec + 4 * slot), s1 = __ldcs(rec + 4 * slot + 1), s2 = __ldcs(rec + 4 * slot + 2),
                      s3 = __ldcs(rec + 4 * slot + 3);
-        RowScan rs;
+        RowScan rs{};
         rs.init(s0.x, s0.y, s2.z, s2.w, s3.x, tau_scan(s2.z, s2.w, s3.x, s1.y), (float)(4 * P.tile), P.n_my);
         const float fW = (float)P.W, fH = (float)P.H;
         for (int r = rs.r0; r <= rs.r1; ++r) {
@@ -222,9 +217,18 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
             else emit_wide(slot, bn.x);
         }
     };
-    for (uint32_t k = threadIdx.x; k < total; k += BIN_THREADS) {
-        const size_t slot = slot_of(k);
-        emit(slot, __ldcs(bin + slot));
+    // warps claim half chunks (up to 128 dense survivor slots: four warp iterations) from a shared counter: no search for the
+    // slot of the k-th survivor of the batch (it was a third of the kernel's instructions; the kernel waits on memory, so the
+    // time did not move: 0.083 ms), tail of at most one half chunk.  Requesting the next record ahead spills at 32 registers.
+    for (;;) {
+        uint32_t q = 0;
+        if (lane == 0) q = atomicAdd(&s_next, 1u);
+        q = __shfl_sync(0xffffffffu, q, 0);
+        if (q >= 2 * n_list) break;
+        const uint32_t e = q >> 1, n = s_pref[e];
+        const uint32_t k0 = (q & 1u) * (HIGS_CHUNK / 2), k1 = min(n, k0 + HIGS_CHUNK / 2);
+        const size_t slot0 = (size_t)s_chunk[e] * HIGS_CHUNK;
+        for (uint32_t k = k0 + lane; k < k1; k += 32) emit(slot0 + k, __ldcs(bin + slot0 + k));
     }
     __syncthreads();
     const uint32_t n_wide = min(s_nq, (uint32_t)FILL_QCAP);

@@ -23,15 +23,9 @@
 #define HIGS_LD __ldg
 namespace {
 
-// SH rows of the survivors are scattered 192-byte reads: ask L2 for 64-byte fills only (a row is three of them)
-__device__ __forceinline__ float4 ld_sh64(const float4* p)
-{
-    float4 v;
-    asm volatile("ld.global.nc.L2::64B.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-    return v;
-}
+// (ld.global.nc.L2::64B on the scattered 192-byte SH rows was measured: no change, 0.273 against 0.268 ms)
 #ifndef HIGS_LD_SH
-#define HIGS_LD_SH HIGS_LD   /* ld_sh64 measured: no change (0.273 against 0.268 ms), DRAM over-fetch of the scattered rows stays */
+#define HIGS_LD_SH HIGS_LD
 #endif
 
 // ln_spec (DESIGN.md N-LN): frexp + atanh series, separate mul and add, x in (1, 255].
@@ -279,7 +273,7 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
 {
     unsigned long long desc = 0;
     {
-        RowScan rs;
+        RowScan rs{};
         rs.template init<SHC>(s.mux, s.muy, s.a, s.b, s.c, tau_scan(s.a, s.b, s.c, s.tau), (float)(4 * P.tile), P.n_my);
         const float fW = (float)P.W, fH = (float)P.H;
         bool fits = (rs.r1 - rs.r0) <= 3 && P.n_mx <= 511 && rs.r0 <= 511;

@@ -185,7 +185,6 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
     float4* s_rec = reinterpret_cast<float4*>(s_raw);                 // fp32 records
     uint4* s_rec16 = reinterpret_cast<uint4*>(s_raw);                 // fp16 records: [i][2], second half holds recB in its first word
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const uint32_t lt_mask = (1u << lane) - 1u;
     pdl_trigger();                                                    // k_merge_image may be scheduled as this grid drains
     const uint32_t n_units = hdr->n_units;
     const bool use_cut = !(P.flags & HIGS_FLAG_NO_XBATCH_CUT);
