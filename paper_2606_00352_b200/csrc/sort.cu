@@ -72,6 +72,7 @@ template <int THREADS>
 __device__ __forceinline__ void block_sort_smem(u64* buf, int n, int n_pad)
 {
     const int t = threadIdx.x;
+    int* s_split = reinterpret_cast<int*>(buf + (THREADS * IPT + THREADS + 2));      // [THREADS + 1] merge-path splits of the threads
     u64 v[IPT];
     const bool live = t * IPT < n;                               // threads past the data hold nothing
     if (live) {
@@ -97,22 +98,31 @@ __device__ __forceinline__ void block_sort_smem(u64* buf, int n, int n_pad)
                 const int mid = (lo + hi) >> 1;
                 if (buf[sidx(A + mid)] < buf[sidx(B + diag - 1 - mid)]) lo = mid + 1; else hi = mid;
             }
-            // serial two-pointer merge of this thread's 16 outputs, branch-free: an exhausted run reads as ~0, which no item
-            // equals (a depth key is the bit pattern of a finite positive float), so one 64-bit compare decides; one predicated
-            // shared load per output refills the side that was consumed
-            int ia = lo, ib = diag - lo;
-            u64 ka = ia < na ? buf[sidx(A + ia)] : ~0ull, kb = ib < nb ? buf[sidx(B + ib)] : ~0ull;
+            s_split[t] = lo;
+        }
+        __syncthreads();
+        if (live) {
+            // This thread's 16 outputs are the merge of A[ia .. ia+ca) and B[ib .. ib+cb), ca + cb = 16, where ia + ca is the
+            // next thread's split (or the end of A when the next thread starts another pair of runs).  Loaded as A ascending
+            // followed by B descending they form a bitonic sequence: a 32-exchange bitonic merge network with static register
+            // indices sorts them - no data-dependent loads, no pointer bookkeeping (a two-pointer merge was 25 instructions
+            // per output, most of them on the ALU pipe that bounds this kernel).
+            const int o0 = t * IPT;
+            const int pb = o0 & ~(2 * run - 1);
+            const int na = min(run, n_pad - pb), nb = max(0, min(run, n_pad - pb - run));
+            const int A = pb, B = pb + run, diag = o0 - pb;
+            const int ia = s_split[t], ib = diag - ia;
+            const bool last = diag + IPT >= na + nb;             // the next thread belongs to another pair (or there is none)
+            const int ca = (last ? na : s_split[t + 1]) - ia;
+            const int pa = A + ia, pbd = B + ib + (IPT - 1);
 #pragma unroll
-            for (int k = 0; k < IPT; ++k) {
-                const bool take_a = ka < kb;
-                v[k] = take_a ? ka : kb;
-                ia += take_a ? 1 : 0; ib += take_a ? 0 : 1;
-                const int nxt = take_a ? A + ia : B + ib;
-                const bool have = take_a ? ia < na : ib < nb;
-                u64 val = buf[sidx(nxt)];                        // at most one past the data: the buffer has a spare slot
-                val = have ? val : ~0ull;
-                ka = take_a ? val : ka; kb = take_a ? kb : val;
-            }
+            for (int k = 0; k < IPT; ++k) v[k] = buf[sidx(k < ca ? pa + k : pbd - k)];
+#define X(a, b) cex(v[a], v[b]);
+            X(0,8) X(1,9) X(2,10) X(3,11) X(4,12) X(5,13) X(6,14) X(7,15)
+            X(0,4) X(1,5) X(2,6) X(3,7) X(8,12) X(9,13) X(10,14) X(11,15)
+            X(0,2) X(1,3) X(4,6) X(5,7) X(8,10) X(9,11) X(12,14) X(13,15)
+            X(0,1) X(2,3) X(4,5) X(6,7) X(8,9) X(10,11) X(12,13) X(14,15)
+#undef X
         }
     }
     __syncthreads();
@@ -353,7 +363,7 @@ __device__ __forceinline__ uint32_t bucket_of(const u64* s_split, uint32_t n_spl
 constexpr int OVER_THREADS = 256;
 constexpr int SCAT_ITEMS = HIGS_SPLIT_TILE / OVER_THREADS;
 static_assert(HIGS_MAX_SPLIT <= OVER_THREADS && HIGS_MAX_SPLIT <= 256, "one thread per bucket in the bucket scan; bucket ids are bytes");
-constexpr size_t OVER_BUF = sizeof(u64) * (OVER_THREADS * IPT + OVER_THREADS + 2);    // sidx(4096) items of the sample sort
+constexpr size_t OVER_BUF = sizeof(u64) * (OVER_THREADS * IPT + OVER_THREADS + 2) + sizeof(int) * (OVER_THREADS + 2);    // sidx(4096) items of the sample sort
 constexpr size_t OVER_SMEM = OVER_BUF + sizeof(u64) * HIGS_MAX_SPLIT + sizeof(uint32_t) * (2 * HIGS_MAX_SPLIT + 64);
 
 // last segment with tile_base <= tile
@@ -606,7 +616,7 @@ k_merge_levels(const OverSeg* __restrict__ over, const FrameHeader* __restrict__
 }
 
 template <int THREADS>
-constexpr size_t sort_smem() { return (size_t)(THREADS * IPT + THREADS + 2) * sizeof(u64); }   // sidx(CAP) items + a spare slot read past the last run
+constexpr size_t sort_smem() { return (size_t)(THREADS * IPT + THREADS + 2) * sizeof(u64) + (THREADS + 2) * sizeof(int); }   // sidx(CAP) items + the threads' splits
 
 // tier t: segments / buckets of up to 1024 << t items
 template <int TIER> struct TierCfg;
