@@ -25,11 +25,8 @@ constexpr int BIN_THREADS = 1024;   // two CTAs per SM at 32 registers: the pass
 __global__ void __launch_bounds__(1024)
 k_plan(const FrameParams P,
        const uint32_t* __restrict__ mt_count, uint32_t* __restrict__ mt_offset, uint32_t* __restrict__ batch_offset,
-       uint32_t* __restrict__ unit_mt, uint32_t* __restrict__ unit_order, uint32_t* __restrict__ level_hist,
-       uint32_t* __restrict__ level_cur, SortJob* __restrict__ sort_jobs, size_t max_jobs, SplitSeg* __restrict__ split,
-       FrameHeader* __restrict__ hdr)
+       SortJob* __restrict__ sort_jobs, size_t max_jobs, SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr)
 {
-    extern __shared__ uint32_t s_bo[];                            // [n_m + 1] copy of batch_offset for the unit -> macro-tile search
     __shared__ uint32_t s_warp[33 * 8];
     __shared__ uint32_t s_max;
     __shared__ unsigned long long s_total;
@@ -50,7 +47,7 @@ k_plan(const FrameParams P,
         }
         uint32_t v[2] = { n, (n + br - 1) / br };
         plan_scan<2>(v, carry, s_warp);
-        if (m < P.n_m) { mt_offset[m] = v[0]; batch_offset[m] = v[1]; s_bo[m] = v[1]; }
+        if (m < P.n_m) { mt_offset[m] = v[0]; batch_offset[m] = v[1]; }
     }
     // the 32-bit scan wraps beyond 2^32 pairs: the capacity check is on a 64-bit total (one shared atomic per warp)
 #pragma unroll
@@ -60,7 +57,7 @@ k_plan(const FrameParams P,
     const uint32_t n_pairs = carry[0], n_units = carry[1];
     const bool overflow = s_total > (unsigned long long)P.max_pairs || n_units > P.max_units;
     if (threadIdx.x == 0) {
-        mt_offset[P.n_m] = n_pairs; batch_offset[P.n_m] = n_units; s_bo[P.n_m] = n_units;
+        mt_offset[P.n_m] = n_pairs; batch_offset[P.n_m] = n_units;
         hdr->n_pairs = overflow ? 0u : n_pairs;
         hdr->n_units = overflow ? 0u : n_units;
         hdr->overflow = overflow ? 1u : 0u;
@@ -68,11 +65,22 @@ k_plan(const FrameParams P,
     }
     __syncthreads();                                              // mt_offset is complete (and visible to this CTA)
     sort_plan_body(mt_offset, P.n_m, overflow, sort_jobs, max_jobs, split, hdr, s_warp);
-    if (overflow) return;
-    __syncthreads();
-    // pass 2: unit table, and the order the rasterizer claims (sub-)units in: batch index j major ("level" j =
-    // the j-th batch of every macro-tile that has one), so that by the time a deep batch starts the batches
-    // in front of it have published their transmittance bounds (cross-batch cut).
+}
+
+// a6, second part (off the critical path: it runs beside the sort and is needed by the rasterizer only): the unit table and
+// the order the rasterizer claims units in - batch index j major ("level" j = the j-th batch of every macro-tile that has one),
+// so that by the time a deep batch starts the batches in front of it have published their transmittance bounds (cross-batch
+// cut).
+__global__ void __launch_bounds__(1024)
+k_units(const FrameParams P, const uint32_t* __restrict__ mt_count, const uint32_t* __restrict__ batch_offset,
+        uint32_t* __restrict__ unit_mt, uint32_t* __restrict__ unit_order, uint32_t* __restrict__ level_hist,
+        uint32_t* __restrict__ level_cur, const FrameHeader* __restrict__ hdr)
+{
+    extern __shared__ uint32_t s_bo[];                            // [n_m + 1] copy of batch_offset for the unit -> macro-tile search
+    __shared__ uint32_t s_warp[33 * 8];
+    if (hdr->overflow) return;
+    const uint32_t br = (uint32_t)P.batch_cap, s_max = hdr->max_segment, n_units = hdr->n_units;
+    for (int m = threadIdx.x; m <= P.n_m; m += 1024) s_bo[m] = batch_offset[m];
     const uint32_t max_nb = (s_max + br - 1) / br;
     for (uint32_t v = threadIdx.x; v <= max_nb + 1; v += 1024) level_hist[v] = 0;
     __syncthreads();
@@ -280,13 +288,21 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, n_b);
     const size_t smem = sizeof(uint32_t) * ((size_t)P.n_m + 2 * (size_t)lcap + 1 + 2 * FILL_QCAP);
     if (ev_count) cudaEventRecord(ev_count, st);    // the count pass ran inside k_project: this stage is empty
-    HIGS_CUDA(ctx, launch_pdl(k_plan, dim3(1), dim3(1024), sizeof(uint32_t) * ((size_t)P.n_m + 1), st, P, ctx->mt_count, ctx->mt_offset,
-                              ctx->batch_offset, ctx->unit_mt, ctx->unit_order, ctx->level_hist, ctx->level_cur, ctx->sort_jobs,
+    HIGS_CUDA(ctx, launch_pdl(k_plan, dim3(1), dim3(1024), 0, st, P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->sort_jobs,
                               (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr));
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
     HIGS_CUDA(ctx, launch_pdl(k_fill, dim3(n_b), dim3(BIN_THREADS), smem, st, ctx->chunk_count, ctx->part_list, ctx->part_desc, lcap, ctx->bin,
                               ctx->rec, P, ctx->hist, ctx->mt_fill, ctx->mt_offset, ctx->pairs, ctx->hdr, ctx->cut_word, ctx->cut_term, ctx->tile_load));
+    HIGS_LAUNCHED(ctx);
+    return HIGS_OK;
+}
+
+// enqueued on a side stream of the sort (sort.cu), behind the event recorded after k_fill
+int launch_units(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
+{
+    k_units<<<1, 1024, sizeof(uint32_t) * ((size_t)P.n_m + 1), st>>>(P, ctx->mt_count, ctx->batch_offset, ctx->unit_mt, ctx->unit_order,
+                                                                     ctx->level_hist, ctx->level_cur, ctx->hdr);
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }
@@ -315,6 +331,6 @@ int higs_binning_smem_setup(higs_ctx* ctx)
         HIGS_CUDA(ctx, cudaFuncSetAttribute(k_fill, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
     }
     const int plan_bytes = (int)(sizeof(uint32_t) * ((size_t)ctx->max_nm + 1));
-    if (plan_bytes > 40 * 1024) HIGS_CUDA(ctx, cudaFuncSetAttribute(k_plan, cudaFuncAttributeMaxDynamicSharedMemorySize, plan_bytes));
+    if (plan_bytes > 40 * 1024) HIGS_CUDA(ctx, cudaFuncSetAttribute(k_units, cudaFuncAttributeMaxDynamicSharedMemorySize, plan_bytes));
     return HIGS_OK;
 }

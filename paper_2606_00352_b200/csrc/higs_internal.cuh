@@ -173,6 +173,7 @@ int higs_part_grid(const higs_ctx*, int64_t N);
 int higs_part_lcap(int64_t n_chunks, int grid);
 int launch_binning(higs_ctx*, const FrameParams&, int64_t N, cudaStream_t, cudaEvent_t ev_count, cudaEvent_t ev_scan);
 int launch_sort(higs_ctx*, const FrameParams&, cudaStream_t);
+int launch_units(higs_ctx*, const FrameParams&, cudaStream_t);
 int launch_sort_only(higs_ctx*, unsigned long long* pairs, const uint32_t* seg_offset, int n_seg, cudaStream_t);
 int launch_raster(higs_ctx*, const FrameParams&, cudaStream_t);
 int launch_merge(higs_ctx*, const FrameParams&, float* out_rgb, cudaStream_t);

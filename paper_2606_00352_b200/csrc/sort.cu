@@ -654,8 +654,9 @@ int setup_tier(higs_ctx* ctx)
     return HIGS_OK;
 }
 
-int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, bool plan_done, cudaStream_t st)
+int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, const FrameParams* frame, cudaStream_t st)
 {
+    const bool plan_done = frame != nullptr;
     SortJob* jobs0 = ctx->sort_jobs;
     SortJob* jobs1 = ctx->sort_jobs + (size_t)HIGS_N_TIERS * ctx->max_jobs;
     u64* alt = ctx->pairs_alt;
@@ -678,6 +679,7 @@ int run_sort(higs_ctx* ctx, u64* pairs, const uint32_t* seg_offset, int n_seg, b
         HIGS_LAUNCHED(ctx);
     }
     if ((rc = launch_tier<3>(ctx, 0, pairs, ms, ctx->aux_stream[0]))) return rc;
+    if (frame && (rc = launch_units(ctx, *frame, ctx->aux_stream[0]))) return rc;   // the unit table: needed by the rasterizer only
     if ((rc = launch_tier<2>(ctx, 0, pairs, ms, ctx->aux_stream[1]))) return rc;
     if ((rc = launch_tier<1>(ctx, 0, pairs, ms, ctx->aux_stream[2]))) return rc;
     if ((rc = launch_tier<0>(ctx, 0, pairs, ms, ctx->aux_stream[3]))) return rc;
@@ -720,10 +722,10 @@ int higs_sort_smem_setup(higs_ctx* ctx)
 
 int launch_sort(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
 {
-    return run_sort(ctx, ctx->pairs, ctx->mt_offset, P.n_m, true, st);
+    return run_sort(ctx, ctx->pairs, ctx->mt_offset, P.n_m, &P, st);
 }
 
 int launch_sort_only(higs_ctx* ctx, unsigned long long* pairs, const uint32_t* seg_offset, int n_seg, cudaStream_t st)
 {
-    return run_sort(ctx, pairs, seg_offset, n_seg, false, st);
+    return run_sort(ctx, pairs, seg_offset, n_seg, nullptr, st);
 }
