@@ -209,7 +209,7 @@ def workload_config(scene, args, world) -> dict:
     return {"workload": "configs[3]: large scene, paper scale (heavy-tailed planes/shells + 20% background + 10% hot region)",
             "n_gaussians": scene.N, "sh_degree": scene.degree, "image": "1920x1080", "fov_x_deg": 60,
             "views": f"orbit of {len(scene.cameras)} poses, step i -> view (i*{world}+rank) % {len(scene.cameras)}; view 0 = configs[3]'s pose",
-            "tiles": f"8x8 px render tiles, 8x4 macro-tiles (64x32 px), B_r={args.batch_cap}, partition batches = 2 persistent CTAs per SM over 256-id chunks",
+            "tiles": f"8x8 px render tiles, 8x4 macro-tiles (64x32 px), B_r={args.batch_cap}, partition batches = 2 persistent CTAs per SM over 128-id chunks",
             "l2": "inputs (1.37 GB) and per-frame records (0.46 GB) exceed the 126 MB L2; no flush between frames",
             "parallelism": f"replicas x{world} (views sharded, no collective)"}
 
@@ -469,6 +469,11 @@ def run_higs(args) -> int:
         run_variant("resident_fp32sh", 0, view, "resident scene (higs_scene_upload + higs_render_view), 192-byte fp32 SH rows")
         run_variant("resident_sh32", hg.HIGS_FLAG_SH32, view, "PAPER.md:245: 32-byte SH codes decoded inline in the projection kernel")
         run_variant("resident_sh32_fp16", hg.HIGS_FLAG_SH32 | hg.HIGS_FLAG_FP16, view, "the paper's default configuration: fp16 data path + 32-byte SH")
+        hg.higs_scene_sort_spatial(ctx, scene.N)
+        hg.higs_scene_compress_sh(ctx)
+        run_variant("sorted_fp32sh", 0, view, "resident scene stored along a Morton curve (higs_scene_sort_spatial): survivors of the cull are contiguous")
+        run_variant("sorted_sh32", hg.HIGS_FLAG_SH32, view, "Morton order + 32-byte SH codes")
+        run_variant("sorted_sh32_fp16", hg.HIGS_FLAG_SH32 | hg.HIGS_FLAG_FP16, view, "Morton order + 32-byte SH codes + fp16 data path")
 
     hg.higs_destroy(ctx)
     if rank == 0:

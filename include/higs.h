@@ -162,6 +162,14 @@ int higs_render_host(higs_ctx* ctx, const float* means, const float* scales, con
 int higs_scene_upload(higs_ctx* ctx, const float* means, const float* scales, const float* quats,
                       const float* opacities, const float* sh, int degree, int64_t N);
 int higs_render_view_host(higs_ctx* ctx, const higs_camera* cam, int W, int H, float* out_rgb);
+/* Store the resident scene in a spatially coherent order: its gaussians are sorted along a Morton curve of their means
+ * (10 bits per axis over the bounding box, ties by index).  The order of the gaussians is part of a scene - the ids in the
+ * lists and the (depth key, id) tie-break refer to the new order - so the permutation is returned: host_perm[i] (HOST, [N],
+ * may be NULL) = index in the uploaded arrays of the gaussian now at i.  Rendering the reordered scene is rendering the
+ * uploaded arrays permuted that way.  Why: survivors of the cull become contiguous, so the projection kernel's scattered
+ * 192-byte SH reads stop over-fetching.  Needs N <= max_pairs (it uses the frame's sort scratch).
+ * Synchronises; discards SH codes made before it. */
+int higs_scene_sort_spatial(higs_ctx* ctx, uint32_t* host_perm);
 /* 32-byte SH codec (section 4.2): encode the resident scene's degree-3 SH rows on the device - YCoCg-R,
  * square-root gamma quantisation (6 bits luma, 4 bits chroma; 16 / 15 / 15 bits for the DC basis), per-(basis, channel)
  * scales = the 99.9th percentile of |value| over the scene (the maximum for DC); bit layout in DESIGN.md (Q20).  With

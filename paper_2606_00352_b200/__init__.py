@@ -24,7 +24,7 @@ HIGS_TILE, HIGS_MT_W, HIGS_MT_H, HIGS_MT_TILES, HIGS_BATCH_CAP = 8, 64, 32, 32, 
 
 EXPORTS = ["higs_abi_version", "higs_strerror", "higs_last_error", "higs_create", "higs_destroy", "higs_set_flags",
            "higs_set_batch_cap", "higs_set_tile", "higs_render", "higs_render_host", "higs_scene_upload", "higs_render_view_host",
-           "higs_render_view", "higs_scene_compress_sh", "higs_get_sh32", "higs_get_stats", "higs_get_lists", "higs_get_records", "higs_sort_segments", "higs_download"]
+           "higs_render_view", "higs_scene_sort_spatial", "higs_scene_compress_sh", "higs_get_sh32", "higs_get_stats", "higs_get_lists", "higs_get_records", "higs_sort_segments", "higs_download"]
 
 
 class higs_camera(C.Structure):
@@ -93,6 +93,7 @@ def load() -> C.CDLL:
         L.higs_render_view_host.argtypes = [vp, C.POINTER(higs_camera), C.c_int, C.c_int, f32p]
         L.higs_render_view.restype = C.c_int
         L.higs_render_view.argtypes = [vp, C.POINTER(higs_camera), C.c_int, C.c_int, f32p, vp]
+        L.higs_scene_sort_spatial.restype = C.c_int; L.higs_scene_sort_spatial.argtypes = [vp, vp]
         L.higs_scene_compress_sh.restype = C.c_int; L.higs_scene_compress_sh.argtypes = [vp]
         L.higs_get_sh32.restype = C.c_int; L.higs_get_sh32.argtypes = [vp, vp, vp]
         L.higs_get_stats.restype = C.c_int; L.higs_get_stats.argtypes = [vp, C.POINTER(higs_stats)]
@@ -186,6 +187,13 @@ def higs_scene_upload(ctx, means, scales, quats, opacities, sh, degree: int) -> 
     N = int(opacities.shape[0])
     _check(load().higs_scene_upload(ctx, _ptr(means), _ptr(scales), _ptr(quats), _ptr(opacities), _ptr(sh), degree, N),
            "higs_scene_upload", ctx)
+
+
+def higs_scene_sort_spatial(ctx, n: int) -> np.ndarray:
+    """Reorders the resident scene along a Morton curve; returns perm (uint32 [n]): new index i holds uploaded gaussian perm[i]."""
+    perm = np.zeros(n, np.uint32)
+    _check(load().higs_scene_sort_spatial(ctx, C.c_void_p(perm.ctypes.data)), "higs_scene_sort_spatial", ctx)
+    return perm
 
 
 def higs_scene_compress_sh(ctx) -> None:

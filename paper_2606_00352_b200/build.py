@@ -14,7 +14,7 @@ from pathlib import Path
 PKG = Path(__file__).resolve().parent
 CSRC = PKG / "csrc"
 LIB = PKG / "lib" / "libhigs.so"
-SOURCES = ["api.cu", "project.cu", "binning.cu", "sort.cu", "raster.cu", "shcodec.cu"]
+SOURCES = ["api.cu", "project.cu", "binning.cu", "sort.cu", "raster.cu", "shcodec.cu", "scene.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--extended-lambda", "-Xcompiler", "-fPIC", "-shared"]
 

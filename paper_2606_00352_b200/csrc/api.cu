@@ -328,6 +328,26 @@ int higs_scene_compress_sh(higs_ctx* ctx)
     return HIGS_OK;
 }
 
+int higs_scene_sort_spatial(higs_ctx* ctx, uint32_t* host_perm)
+{
+    if (!ctx || ctx->s_n < 0 || ctx->s_n > ctx->max_pairs) return HIGS_E_ARG;
+    HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
+    HIGS_CUDA(ctx, cudaDeviceSynchronize());
+    uint32_t* d_perm = nullptr;
+    int rc;
+    if (host_perm && ctx->s_n > 0 && (rc = dev_alloc(ctx, &d_perm, (size_t)ctx->s_n))) return rc;
+    if (ctx->s_n == 1 && host_perm) host_perm[0] = 0u;
+    rc = launch_scene_sort(ctx, d_perm, ctx->own_stream);
+    if (!rc && host_perm && ctx->s_n > 1) {
+        cudaError_t e = cudaMemcpy(host_perm, d_perm, sizeof(uint32_t) * (size_t)ctx->s_n, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) { dev_free(d_perm); HIGS_CUDA(ctx, e); }
+    }
+    dev_free(d_perm);
+    ctx->s_sh32_valid = false;
+    ctx->last_stream = ctx->own_stream;
+    return rc;
+}
+
 int higs_get_sh32(higs_ctx* ctx, uint8_t* host_codes, float* host_scales)
 {
     if (!ctx || !ctx->s_sh32_valid) return HIGS_E_ARG;

@@ -225,18 +225,17 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
             else emit_wide(slot, bn.x);
         }
     };
-    // warps claim half chunks (up to 128 dense survivor slots: four warp iterations) from a shared counter: no search for the
+    // warps claim chunks (up to 128 dense survivor slots: four warp iterations) from a shared counter: no search for the
     // slot of the k-th survivor of the batch (it was a third of the kernel's instructions; the kernel waits on memory, so the
-    // time did not move: 0.083 ms), tail of at most one half chunk.  Requesting the next record ahead spills at 32 registers.
+    // time did not move: 0.083 ms), tail of at most one chunk.  Requesting the next record ahead spills at 32 registers.
     for (;;) {
         uint32_t q = 0;
         if (lane == 0) q = atomicAdd(&s_next, 1u);
         q = __shfl_sync(0xffffffffu, q, 0);
-        if (q >= 2 * n_list) break;
-        const uint32_t e = q >> 1, n = s_pref[e];
-        const uint32_t k0 = (q & 1u) * (HIGS_CHUNK / 2), k1 = min(n, k0 + HIGS_CHUNK / 2);
-        const size_t slot0 = (size_t)s_chunk[e] * HIGS_CHUNK;
-        for (uint32_t k = k0 + lane; k < k1; k += 32) emit(slot0 + k, __ldcs(bin + slot0 + k));
+        if (q >= n_list) break;
+        const uint32_t n = s_pref[q];
+        const size_t slot0 = (size_t)s_chunk[q] * HIGS_CHUNK;
+        for (uint32_t k = lane; k < n; k += 32) emit(slot0 + k, __ldcs(bin + slot0 + k));
     }
     __syncthreads();
     const uint32_t n_wide = min(s_nq, (uint32_t)FILL_QCAP);

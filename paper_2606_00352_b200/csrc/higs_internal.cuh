@@ -10,7 +10,7 @@
 #define HIGS_HDR_WORDS  64           // 32-bit words reserved for the FrameHeader at the head of its block
 #define HIGS_MAX_NM     32768        // macro-tiles per frame the shared-memory histograms are sized for
 #define HIGS_N_TIERS    4            // block-sort tiers, capacities 1024 / 2048 / 4096 / 8192
-#define HIGS_CHUNK      256          // consecutive ids projected by one warp; survivors are stored densely per chunk
+#define HIGS_CHUNK      128          // consecutive ids projected by one warp; survivors are stored densely per chunk
 #define HIGS_MERGE_TILE 4096         // output items per merge-path tile (overflow path)
 #define HIGS_SPLIT_TILE 2048         // items per CTA pass of the bucket count / scatter kernels
 #define HIGS_BUCKET_TARGET 1536      // mean items per depth bucket of an oversize segment
@@ -169,6 +169,7 @@ inline cudaError_t launch_pdl(void (*kernel)(KP...), dim3 grid, dim3 block, size
 int launch_project(higs_ctx*, const FrameParams&, const float* means, const float* scales, const float* quats,
                    const float* opac, const float* sh, bool sh32, int64_t N, cudaStream_t);
 int launch_sh32_encode(higs_ctx*, cudaStream_t);
+int launch_scene_sort(higs_ctx*, uint32_t* d_perm, cudaStream_t);
 int higs_part_grid(const higs_ctx*, int64_t N);
 int higs_part_lcap(int64_t n_chunks, int grid);
 int launch_binning(higs_ctx*, const FrameParams&, int64_t N, cudaStream_t, cudaEvent_t ev_count, cudaEvent_t ev_scan);

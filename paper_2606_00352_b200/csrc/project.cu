@@ -1,6 +1,6 @@
 // project.cu -- steps a1 + a2: fused EWA projection + cull + SH colour (section 4.2), with the
 // count pass of the partitioning folded in: every persistent CTA is one partition batch
-// (the chunks of HIGS_CHUNK = 256 consecutive ids its warps claim), keeps the private shared-memory histogram with one counter
+// (the chunks of HIGS_CHUNK = 128 consecutive ids its warps claim), keeps the private shared-memory histogram with one counter
 // per macro-tile and flushes it as one row of the N_B x N_M matrix (N_B = CTAs = a whole number per SM).  The kernel is HBM-latency-bound, so the row scan runs in issue
 // slots that were idle; the macro-tile span it finds is also packed into a 64-bit descriptor in the record, so
 // the fill pass replays it without redoing the arithmetic.  (Section 4.2:
@@ -323,7 +323,7 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
     bin[slot] = make_uint4(key, (uint32_t)desc, (uint32_t)(desc >> 32), (uint32_t)i);
 }
 
-// Persistent CTAs (a whole number per SM), one histogram row per CTA.  A warp claims chunks of HIGS_CHUNK = 256
+// Persistent CTAs (a whole number per SM), one histogram row per CTA.  A warp claims chunks of HIGS_CHUNK = 128
 // consecutive ids from a device counter, so the load balances itself and the grid never has a partial wave; the
 // paper's fixed partition batch of B_p consecutive ids becomes "the chunks one CTA happened to
 // claim", listed in part_list / part_desc for the fill pass.  A warp runs phase A on 32 gaussians at a time

@@ -464,6 +464,36 @@ def test_tile_load_map_counts_cover_the_exact_per_tile_lists(hg):
     r.close()
 
 
+def test_spatially_sorted_resident_scene(hg):
+    """higs_scene_sort_spatial: the permutation it returns is a permutation, neighbours in memory are neighbours in space,
+    and rendering the reordered resident scene matches the oracle on the uploaded arrays permuted that way - every output,
+    bit-exact lists included (ids refer to the new order).  Also with the SH codes made after the reordering."""
+    import torch
+    s = hs.scene_cfg1()
+    cam = s.cameras[0]
+    ctx = hg.higs_create(0, s.N, cam.W, cam.H)
+    f = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    hg.higs_scene_upload(ctx, f(s.means), f(s.scales), f(s.quats), f(s.opacities), f(s.sh), 3)
+    perm = hg.higs_scene_sort_spatial(ctx, s.N)
+    assert np.array_equal(np.sort(perm), np.arange(s.N, dtype=np.uint32))
+    m = s.means[perm]
+    step = np.linalg.norm(np.diff(m, axis=0), axis=1).mean()
+    rnd = np.linalg.norm(np.diff(s.means, axis=0), axis=1).mean()
+    assert step < 0.2 * rnd, (step, rnd)
+    s2 = hs.Scene(s.name + "_sorted", f(s.means[perm]), f(s.scales[perm]), f(s.quats[perm]), f(s.opacities[perm]), f(s.sh[perm]), 3, s.cameras)
+    img = torch.zeros((cam.H, cam.W, 3), dtype=torch.float32, device="cuda")
+    hg.higs_render_view(ctx, hg.make_camera(cam), cam.W, cam.H, img)
+    torch.cuda.synchronize()
+    pr = oracle.project(s2, cam)
+    _check_records(hg.higs_get_records(ctx), pr)
+    _check_lists(hg.higs_get_lists(ctx), oracle.bin_lists(pr))
+    assert np.abs(img.cpu().numpy().astype(np.float64) - oracle.render(pr)).max() <= PIX_TOL
+    hg.higs_scene_compress_sh(ctx)
+    codes, scales = hg.higs_get_sh32(ctx, s.N)
+    assert np.array_equal(codes, oracle.sh32_encode(s2.sh, oracle.sh32_scales(s2.sh)))
+    hg.higs_destroy(ctx)
+
+
 def test_frame_captures_into_a_cuda_graph(hg):
     """higs_render only enqueues (no host synchronisation): a whole frame - memsets, 18 kernels on the
     render stream and the forked sort streams, the cooperative merge kernel, the PDL edges - captures into a CUDA graph,
