@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define HIGS_ABI_VERSION 1
+#define HIGS_ABI_VERSION 2    /* 2: higs_lists.tile_load, higs_stats.tile, set_tile / scene_sort_spatial / scene_compress_sh / get_sh32 */
 
 #define HIGS_TILE        8      /* render tile edge, px  */
 #define HIGS_MT_W        64     /* macro-tile width,  px (8 tiles)  */
@@ -128,7 +128,8 @@ typedef struct {
 
 /* Create a context on CUDA device `device` and preallocate all scratch (PAPER.md:83, 284:
  * "preallocated up front").  max_pairs bounds N_pairs (<= 2^31-1; 0 selects 4*max_gaussians + 65536).
- * Device memory taken: ~64 B/gaussian + 16 B/pair + 32 KB per unit (units <= N_M + max_pairs/1024). */
+ * Device memory taken: ~120 B/gaussian (64-B and 32-B records, 16-B bin record) + 17 B/pair + 32 KB per unit
+ * (units <= N_M + max_pairs/1024; 128 KB per unit after higs_set_tile(ctx, 16)). */
 int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, int max_H, int64_t max_pairs);
 void higs_destroy(higs_ctx* ctx);
 
