@@ -152,8 +152,13 @@ int higs_render(higs_ctx* ctx, const float* means, const float* scales, const fl
                 const float* opacities, const float* sh, int degree, int64_t N,
                 const higs_camera* cam, int W, int H, float* out_rgb, void* cuda_stream);
 
-/* Same frame with HOST buffers: uploads the five arrays, renders, downloads the image into the
- * host buffer out_rgb and synchronises.  Staging device buffers are owned by the context. */
+/* Same frame with HOST buffers: uploads the arrays, renders, downloads the image into the host buffer out_rgb and
+ * synchronises.  Staging device buffers are owned by the context and shared with the resident scene, which this call
+ * invalidates (higs_render_view returns HIGS_E_ARG until the next higs_scene_upload).
+ * If sh is page-locked host memory the device can address (cudaHostAlloc, cudaHostRegister, torch pin_memory()), the SH
+ * array is NOT uploaded: the projection kernel (a1) reads the rows of the gaussians that survive the cull directly from
+ * host memory, whole warps copying 16 contiguous bytes per lane (the cull keeps fewer than half of the gaussians and the
+ * SH rows are 4/5 of a scene's bytes).  Results are identical bit for bit to the uploaded path. */
 int higs_render_host(higs_ctx* ctx, const float* means, const float* scales, const float* quats,
                      const float* opacities, const float* sh, int degree, int64_t N,
                      const higs_camera* cam, int W, int H, float* out_rgb);

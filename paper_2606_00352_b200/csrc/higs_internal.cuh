@@ -124,7 +124,7 @@ struct higs_ctx {
     bool s_sh32_valid;
     float sh32_scales_host[48];
     uint32_t* sh32_work;       // device scratch of the encoder: hist [48][256] | prefix [48] | rank lo/hi [48][2] | scales [48]
-    int64_t s_cap_n; int s_cap_k; int64_t s_img_cap;
+    int64_t s_cap_n, s_cap_sh, s_img_cap;
     int64_t s_n; int s_degree;
     // last frame
     int64_t last_n; int last_W, last_H, last_nm; int last_mx, last_my;
@@ -136,6 +136,7 @@ struct higs_ctx {
     bool timers_valid;
     int n_launches;            // kernels enqueued by the current / last frame
     // resident CTAs per SM of the persistent kernels (occupancy queried at create time, per device)
+    bool proj_staged_ok;                                   // the staged-row projection variants fit in shared memory
     int raster_ctas_per_sm[2][2], merge_ctas_per_sm, over_ctas_per_sm, tier_ctas_per_sm[2][HIGS_N_TIERS];   // tiers: [0] radix, [1] merge sort
     char err[512];
 };
@@ -166,8 +167,12 @@ inline cudaError_t launch_pdl(void (*kernel)(KP...), dim3 grid, dim3 block, size
 }
 
 // ---- launch entry points, one per pipeline step (defined in the .cu files) ----------------------
+// sh_mode of launch_project: where the SH coefficients come from
+#define HIGS_SH_ROWS   0        /* fp32 rows, device memory */
+#define HIGS_SH_CODES  1        /* 32-byte codes of the resident scene */
+#define HIGS_SH_STAGED 2        /* fp32 rows in mapped host memory, copied to shared memory by whole warps */
 int launch_project(higs_ctx*, const FrameParams&, const float* means, const float* scales, const float* quats,
-                   const float* opac, const float* sh, bool sh32, int64_t N, cudaStream_t);
+                   const float* opac, const float* sh, int sh_mode, int64_t N, cudaStream_t);
 int launch_sh32_encode(higs_ctx*, cudaStream_t);
 int launch_scene_sort(higs_ctx*, uint32_t* d_perm, cudaStream_t);
 int higs_part_grid(const higs_ctx*, int64_t N);

@@ -52,7 +52,8 @@ __device__ __forceinline__ float ln_spec(float x)
 __device__ __forceinline__ bool finite_pos(float v) { return (v > 0.0f) && (v <= 3.402823466e+38f); }
 
 // Real SH basis in the convention of the public 3DGS models (reading Q12), fp32 (smooth).
-template <int DEG>
+// STAGED: shp points at the row's copy in shared memory (k_project's SH_STAGED mode), else at the row in global memory.
+template <int DEG, bool STAGED>
 __device__ __forceinline__ void sh_accumulate(const float* __restrict__ shp, float x, float y, float z,
                                               float& r, float& g, float& b)
 {
@@ -62,12 +63,13 @@ __device__ __forceinline__ void sh_accumulate(const float* __restrict__ shp, flo
         const float4* p4 = reinterpret_cast<const float4*>(shp);
 #pragma unroll
         for (int k = 0; k < K * 3 / 4; ++k) {
-            float4 v = HIGS_LD_SH(p4 + k);
+            float4 v;
+            if constexpr (STAGED) v = p4[k]; else v = HIGS_LD_SH(p4 + k);
             c[4 * k] = v.x; c[4 * k + 1] = v.y; c[4 * k + 2] = v.z; c[4 * k + 3] = v.w;
         }
     } else {
 #pragma unroll
-        for (int k = 0; k < K * 3; ++k) c[k] = HIGS_LD(shp + k);
+        for (int k = 0; k < K * 3; ++k) { if constexpr (STAGED) c[k] = shp[k]; else c[k] = HIGS_LD(shp + k); }
     }
     float Y[K];
     Y[0] = 0.28209479177387814f;
@@ -157,6 +159,22 @@ constexpr int PROJ_THREADS = 512;
 constexpr int PROJ_WARPS = PROJ_THREADS / 32;
 constexpr int PROJ_QCAP = 64;                              // per-warp survivor queue (entries), >= 31 + 32
 constexpr int PROJ_QF = 15;                                // words per queued survivor
+
+// where phase B takes a survivor's SH coefficients from
+constexpr int SH_ROWS = 0;                                 // fp32 rows in device memory: every lane reads its own row
+constexpr int SH_CODES = 1;                                // 32-byte codes of the resident scene (shcodec.cu)
+constexpr int SH_STAGED = 2;                               // fp32 rows in mapped host memory: the warp copies the rows of its 32 survivors into
+                                                           // shared memory with contiguous 16-byte pieces first (one lane per row over PCIe: 12 GB/s;
+                                                           // contiguous pieces: 49 GB/s, the rate of a bulk copy, for the surviving rows only)
+// staged row: pieces of 16 bytes when the row is a whole number of them (degrees 1, 3), else of 4 bytes; one piece of padding
+// per row keeps the per-lane reads free of bank conflicts
+template <int DEG> struct ShStage {
+    static constexpr int ROW_W = 3 * (DEG + 1) * (DEG + 1);
+    static constexpr bool V4 = ROW_W % 4 == 0;
+    static constexpr int PIECES = V4 ? ROW_W / 4 : ROW_W;
+    static constexpr int STRIDE_W = V4 ? 4 * (PIECES + 1) : ROW_W + 1;     // words
+};
+constexpr int SH_STAGE_WORDS_MAX = 32 * ShStage<3>::STRIDE_W;               // per warp
 
 // 64-bit macro-tile span descriptor (internal): bit 63 = "not representable, rerun the row scan";
 // bits 0-8 first macro-tile row r0, bits 9-10 rows-1 (<= 4 rows), then 13 bits per row:
@@ -266,11 +284,12 @@ __device__ __forceinline__ bool project_cull(const RawIn& in, const FrameParams&
 
 // Phase B for one survivor: a2 macro-tile row scan (N-SCAN, pinned) -> private histogram + span descriptor,
 // SH colour, and the two records at dense slot `slot`.
-template <int DEG, bool HALF, bool SHC>
+template <int DEG, bool HALF, int SHM>
 __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size_t slot, const float* __restrict__ sh, const float* __restrict__ lut, const ShScales& sc,
                                               const FrameParams& P, uint32_t* s_hist, float4* __restrict__ rec,
                                               uint4* __restrict__ rec16, uint4* __restrict__ bin)
 {
+    constexpr bool SHC = SHM == SH_CODES;
     unsigned long long desc = 0;
     {
         RowScan rs{};
@@ -297,7 +316,8 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
     const float rl = len2 > 0.0f ? rsqrtf(len2) : 0.0f;
     float r, g, bl;
     if constexpr (SHC) sh32_colour(reinterpret_cast<const uint4*>(sh), i, lut, sc, dx * rl, dy * rl, dz * rl, r, g, bl);
-    else sh_accumulate<DEG>(sh + i * (int64_t)((DEG + 1) * (DEG + 1) * 3), dx * rl, dy * rl, dz * rl, r, g, bl);
+    else if constexpr (SHM == SH_STAGED) sh_accumulate<DEG, true>(sh, dx * rl, dy * rl, dz * rl, r, g, bl);       // sh = this lane's staged row
+    else sh_accumulate<DEG, false>(sh + i * (int64_t)((DEG + 1) * (DEG + 1) * 3), dx * rl, dy * rl, dz * rl, r, g, bl);
     const uint32_t key = __float_as_uint(s.zc);
     if constexpr (HALF) {
         // fp16 data path: inverse covariance as Cholesky factors L = [[l0, 0], [l1, l2]], L L^T = conic,
@@ -330,7 +350,7 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
 // and queues the survivors (about 4 in 10 at paper scale) in shared memory; whenever 32 are queued it runs phase B
 // on them with every lane busy.  Survivor k of chunk c gets dense slot c*HIGS_CHUNK + k: slots are monotone in the
 // gaussian id, so (key, slot) order = (key, id) order (Q7).
-template <int DEG, bool HALF, bool SHC>
+template <int DEG, bool HALF, int SHM>
 __global__ void __launch_bounds__(PROJ_THREADS, 2)
 k_project(const float* __restrict__ means, const float* __restrict__ scales, const float* __restrict__ quats,
           const float* __restrict__ opac, const float* __restrict__ sh, int64_t N, const FrameParams P,
@@ -346,6 +366,8 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
     float* q = reinterpret_cast<float*>(s_dyn + ((P.n_m + 3) & ~3)) + w * (PROJ_QF * PROJ_QCAP);
     uint32_t* s_list = s_dyn + ((P.n_m + 3) & ~3) + PROJ_WARPS * PROJ_QF * PROJ_QCAP;   // [lcap] chunks this CTA claimed
     float* s_lut = reinterpret_cast<float*>(s_list + lcap);         // [1536] dequantisation tables of the 32-byte SH code (SHC only)
+    constexpr bool SHC = SHM == SH_CODES;
+    uint32_t* s_stage = reinterpret_cast<uint32_t*>(s_lut + 1536) + w * SH_STAGE_WORDS_MAX;   // SH_STAGED only
     if constexpr (SHC) {
         for (int e = threadIdx.x; e < 1536; e += PROJ_THREADS) {
             const bool luma = e < 1024;
@@ -377,6 +399,21 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
         uint32_t head = 0, tail = 0;
 
         auto drain = [&](uint32_t n_live) {                          // phase B on queue entries head .. head+n_live-1
+            if constexpr (SHM == SH_STAGED) {
+                using SG = ShStage<DEG>;
+                const uint32_t my_local = (uint32_t)lane < n_live ? __float_as_uint(q[14 * PROJ_QCAP + (int)((head + lane) & (PROJ_QCAP - 1))]) : 0u;
+                const uint32_t n_pieces = n_live * SG::PIECES;
+                for (uint32_t p0 = 0; p0 < n_pieces; p0 += 32) {     // piece p = row p / PIECES, part p % PIECES: consecutive lanes, consecutive bytes
+                    const uint32_t p = p0 + lane;
+                    const uint32_t r = min(p / SG::PIECES, n_live - 1u), part = p - r * SG::PIECES;
+                    const int64_t id = c0 + __shfl_sync(0xffffffffu, my_local, (int)r);
+                    if (p < n_pieces) {
+                        if constexpr (SG::V4) *reinterpret_cast<uint4*>(s_stage + r * SG::STRIDE_W + 4 * part) = __ldg(reinterpret_cast<const uint4*>(sh + id * SG::ROW_W) + part);
+                        else s_stage[r * SG::STRIDE_W + part] = __ldg(reinterpret_cast<const uint32_t*>(sh + id * SG::ROW_W) + part);
+                    }
+                }
+                __syncwarp();
+            }
             if ((uint32_t)lane < n_live) {
                 const int e = (int)((head + lane) & (PROJ_QCAP - 1));
                 Survivor s;
@@ -385,7 +422,8 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
                 s.tau = q[8 * PROJ_QCAP + e]; s.zc = q[9 * PROJ_QCAP + e]; s.o = q[10 * PROJ_QCAP + e];
                 s.mx = q[11 * PROJ_QCAP + e]; s.my = q[12 * PROJ_QCAP + e]; s.mz = q[13 * PROJ_QCAP + e];
                 s.local = __float_as_uint(q[14 * PROJ_QCAP + e]);
-                emit_survivor<DEG, HALF, SHC>(s, c0 + s.local, slot0 + head + lane, sh, s_lut, sc, P, s_hist, rec, rec16, bin);
+                const float* shp = SHM == SH_STAGED ? reinterpret_cast<const float*>(s_stage + lane * ShStage<DEG>::STRIDE_W) : sh;
+                emit_survivor<DEG, HALF, SHM>(s, c0 + s.local, slot0 + head + lane, shp, s_lut, sc, P, s_hist, rec, rec16, bin);
             }
             head += n_live;
             __syncwarp();
@@ -449,10 +487,10 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
 
 } // namespace
 
-static size_t project_smem_bytes(int n_m, int lcap)
+static size_t project_smem_bytes(int n_m, int lcap, bool staged = false)
 {
     return sizeof(uint32_t) * (size_t)((n_m + 3) & ~3) + sizeof(float) * (size_t)PROJ_WARPS * PROJ_QF * PROJ_QCAP + sizeof(uint32_t) * (size_t)lcap
-           + sizeof(float) * 1536;
+           + sizeof(float) * 1536 + (staged ? sizeof(uint32_t) * (size_t)PROJ_WARPS * SH_STAGE_WORDS_MAX : 0);
 }
 
 // list capacity of one partition CTA: four times its fair share of the chunks, so a CTA that fills its list and
@@ -470,20 +508,22 @@ int higs_part_grid(const higs_ctx* ctx, int64_t N)
 }
 
 int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, const float* scales, const float* quats,
-                   const float* opac, const float* sh, bool sh32, int64_t N, cudaStream_t st)
+                   const float* opac, const float* sh, int sh_mode, int64_t N, cudaStream_t st)
 {
     if (N <= 0) return HIGS_OK;
+    if (sh_mode == HIGS_SH_STAGED && !ctx->proj_staged_ok) return HIGS_E_ARG;
     const unsigned grid = (unsigned)higs_part_grid(ctx, N);
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, (int)grid);
-    const size_t smem = project_smem_bytes(P.n_m, lcap);
+    const size_t smem = project_smem_bytes(P.n_m, lcap, sh_mode == HIGS_SH_STAGED);
 #define HIGS_PROJ_(D, H, C) k_project<D, H, C><<<grid, PROJ_THREADS, smem, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
                                                                    ctx->rec16, ctx->bin, ctx->chunk_count, ctx->hist, ctx->mt_count, ctx->part_list, ctx->part_desc, lcap, ctx->hdr, sc)
-#define HIGS_PROJ(D) do { if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(D, true, false); else HIGS_PROJ_(D, false, false); } while (0)
+#define HIGS_PROJ(D) do { if (sh_mode == HIGS_SH_STAGED) { if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(D, true, SH_STAGED); else HIGS_PROJ_(D, false, SH_STAGED); } \
+                          else if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(D, true, SH_ROWS); else HIGS_PROJ_(D, false, SH_ROWS); } while (0)
     ShScales sc;
     memset(&sc, 0, sizeof(sc));
-    if (sh32) {                                                      // sh = the 32-byte codes of the resident scene (degree 3)
+    if (sh_mode == HIGS_SH_CODES) {                                  // sh = the 32-byte codes of the resident scene (degree 3)
         memcpy(sc.s, ctx->sh32_scales_host, sizeof(sc.s));
-        if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(3, true, true); else HIGS_PROJ_(3, false, true);
+        if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(3, true, SH_CODES); else HIGS_PROJ_(3, false, SH_CODES);
     } else switch (P.degree) {
         case 0: HIGS_PROJ(0); break;
         case 1: HIGS_PROJ(1); break;
@@ -502,12 +542,24 @@ int higs_project_smem_setup(higs_ctx* ctx)
     const int lcap_max = higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) > 6 * PROJ_WARPS ? higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) : 6 * PROJ_WARPS;
     const int bytes = (int)project_smem_bytes(ctx->max_nm, lcap_max);
 #define HIGS_ATTR(D, H, C) HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<D, H, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))
-    HIGS_ATTR(0, false, false); HIGS_ATTR(1, false, false); HIGS_ATTR(2, false, false); HIGS_ATTR(3, false, false);
-    HIGS_ATTR(0, true, false); HIGS_ATTR(1, true, false); HIGS_ATTR(2, true, false); HIGS_ATTR(3, true, false);
-    HIGS_ATTR(3, false, true); HIGS_ATTR(3, true, true);
+    HIGS_ATTR(0, false, SH_ROWS); HIGS_ATTR(1, false, SH_ROWS); HIGS_ATTR(2, false, SH_ROWS); HIGS_ATTR(3, false, SH_ROWS);
+    HIGS_ATTR(0, true, SH_ROWS); HIGS_ATTR(1, true, SH_ROWS); HIGS_ATTR(2, true, SH_ROWS); HIGS_ATTR(3, true, SH_ROWS);
+    HIGS_ATTR(3, false, SH_CODES); HIGS_ATTR(3, true, SH_CODES);
 #undef HIGS_ATTR
+    // the staged-row variants (mapped host memory) need room for the rows of 32 survivors per warp; without it
+    // higs_render_host keeps uploading the SH array
+    int optin = 0;
+    HIGS_CUDA(ctx, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->device));
+    const int bytes_staged = (int)project_smem_bytes(ctx->max_nm, lcap_max, true);
+    ctx->proj_staged_ok = bytes_staged <= optin;
+    if (ctx->proj_staged_ok) {
+#define HIGS_ATTR(D, H) HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<D, H, SH_STAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes_staged))
+        HIGS_ATTR(0, false); HIGS_ATTR(1, false); HIGS_ATTR(2, false); HIGS_ATTR(3, false);
+        HIGS_ATTR(0, true); HIGS_ATTR(1, true); HIGS_ATTR(2, true); HIGS_ATTR(3, true);
+#undef HIGS_ATTR
+    }
     int occ = 0;
-    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3, false, false>, PROJ_THREADS, (size_t)bytes));
+    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3, false, SH_ROWS>, PROJ_THREADS, (size_t)bytes));
     ctx->n_part_max = ctx->n_sm * (occ < 1 ? 1 : occ);
     return HIGS_OK;
 }

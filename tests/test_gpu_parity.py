@@ -224,9 +224,47 @@ def test_host_buffer_entry_points(hg):
     hg.higs_render_host(ctx, s.means, s.scales, s.quats, s.opacities, s.sh, 0, hg.make_camera(cam), cam.W, cam.H, out)
     ref = oracle.render(oracle.project(s, cam))
     assert np.abs(out - ref).max() <= PIX_TOL
+    import ctypes as C
+    # the host call borrows the resident scene's buffers: no resident scene afterwards
+    assert hg.load().higs_render_view_host(ctx, C.byref(hg.make_camera(cam)), cam.W, cam.H, C.c_void_p(out.ctypes.data)) == hg.HIGS_E_ARG
     out2 = np.zeros_like(out)
+    hg.higs_scene_upload(ctx, s.means, s.scales, s.quats, s.opacities, s.sh, 0)
     hg.higs_render_view_host(ctx, hg.make_camera(cam), cam.W, cam.H, out2)
     assert np.array_equal(out, out2) or np.abs(out - out2).max() < 5e-4
+    hg.higs_destroy(ctx)
+
+
+@pytest.mark.parametrize("degree", [0, 1, 2, 3])
+def test_host_call_reads_pinned_sh_rows_in_place(hg, degree):
+    """higs_render_host with a page-locked SH array: the projection kernel copies the survivors' rows from host memory
+    (whole warps, contiguous pieces) instead of uploading the array.  Same records, lists and image as with pageable
+    arrays, bit for bit; image against the oracle."""
+    import torch
+    s = hs.scene_cfg1()
+    K = (degree + 1) ** 2
+    sh = np.ascontiguousarray(s.sh[:, :K, :], dtype=np.float32)
+    s = hs.Scene(s.name + f"_deg{degree}", s.means, s.scales, s.quats, s.opacities, sh, degree, s.cameras)
+    cam = s.cameras[0]
+    ctx = hg.higs_create(0, s.N, cam.W, cam.H)
+    out_pageable = np.zeros((cam.H, cam.W, 3), np.float32)
+    hg.higs_render_host(ctx, s.means, s.scales, s.quats, s.opacities, sh, degree, hg.make_camera(cam), cam.W, cam.H, out_pageable)
+    rec_a, lists_a = hg.higs_get_records(ctx), hg.higs_get_lists(ctx)
+    pinned = torch.from_numpy(sh).pin_memory()
+    assert pinned.is_pinned()
+    out_pinned = torch.zeros((cam.H, cam.W, 3), dtype=torch.float32).pin_memory()
+    for flags in (0, hg.HIGS_FLAG_FP16):
+        hg.higs_set_flags(ctx, flags)
+        hg.higs_render_host(ctx, s.means, s.scales, s.quats, s.opacities, pinned, degree, hg.make_camera(cam), cam.W, cam.H, out_pinned)
+        if flags == 0:
+            rec_b, lists_b = hg.higs_get_records(ctx), hg.higs_get_lists(ctx)
+            assert np.array_equal(rec_a["valid"], rec_b["valid"]) and np.array_equal(rec_a["rec"], rec_b["rec"])
+            for k in ("mt_count", "mt_offset", "keys", "ids"):
+                assert np.array_equal(lists_a[k], lists_b[k]), k
+            assert np.abs(out_pinned.numpy() - out_pageable).max() <= 5e-4       # same records, same lists; the cut is scheduling dependent
+            ref = oracle.render(oracle.project(s, cam))
+            assert np.abs(out_pinned.numpy() - ref).max() <= PIX_TOL
+        else:
+            assert psnr(out_pinned.numpy(), out_pageable) >= PSNR_FP16
     hg.higs_destroy(ctx)
 
 
