@@ -155,8 +155,11 @@ __device__ __forceinline__ void sh32_colour(const uint4* __restrict__ codes, int
     r = fmaxf(r + 0.5f, 0.0f); g = fmaxf(g + 0.5f, 0.0f); b = fmaxf(b + 0.5f, 0.0f);
 }
 
-constexpr int PROJ_THREADS = 512;
-constexpr int PROJ_WARPS = PROJ_THREADS / 32;
+// Threads per CTA (two CTAs per SM).  The fp32-record kernel on fp32 SH rows is bound by DRAM and spills at 64 registers
+// (512 threads: 40 bytes of stack, 5 M local-memory warp accesses per frame that all travel to L2); 384 threads (80 registers)
+// has none: 0.268 -> 0.262 ms, DRAM traffic 1.36 -> 1.27 GB.  The other variants are bound by instruction issue and keep 32 warps per SM.
+__host__ __device__ constexpr int proj_threads(bool half, int shm) { return (!half && shm == 0) ? 384 : 512; }
+constexpr int PROJ_WARPS_MAX = 16;
 constexpr int PROJ_QCAP = 64;                              // per-warp survivor queue (entries), >= 31 + 32
 constexpr int PROJ_QF = 15;                                // words per queued survivor
 
@@ -180,6 +183,16 @@ constexpr int SH_STAGE_WORDS_MAX = 32 * ShStage<3>::STRIDE_W;               // p
 // bits 0-8 first macro-tile row r0, bits 9-10 rows-1 (<= 4 rows), then 13 bits per row:
 // first column m0 (9 bits, 511 = row not touched) and columns-1 (4 bits, <= 16 columns).
 #define HIGS_DESC_FALLBACK 0x8000000000000000ull
+
+// One 256-bit store (sm_100: STG.256).  A record written as 16-byte halves reaches L2 as partial-sector writes, and L2 answers a
+// partial write that misses with a fill read of the sector from DRAM: ncu counted 11.7 M write-miss sectors per frame in this
+// kernel and 0.2 GB of DRAM reads nobody asked for.  A whole 32-byte sector in one store needs no fill.  p: 32-byte aligned.
+__device__ __forceinline__ void st_global_256(void* p, uint4 lo, uint4 hi)
+{
+    asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                 :: "l"(__cvta_generic_to_global(p)), "r"(lo.x), "r"(lo.y), "r"(lo.z), "r"(lo.w), "r"(hi.x), "r"(hi.y), "r"(hi.z), "r"(hi.w) : "memory");
+}
+__device__ __forceinline__ uint4 f4_bits(float a, float b, float c, float d) { return make_uint4(__float_as_uint(a), __float_as_uint(b), __float_as_uint(c), __float_as_uint(d)); }
 
 // what phase A hands to phase B for a surviving gaussian
 struct Survivor { float mux, muy, a, b, c, A, B2, C, tau, zc, o, mx, my, mz; uint32_t local; };
@@ -287,7 +300,7 @@ __device__ __forceinline__ bool project_cull(const RawIn& in, const FrameParams&
 template <int DEG, bool HALF, int SHM>
 __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size_t slot, const float* __restrict__ sh, const float* __restrict__ lut, const ShScales& sc,
                                               const FrameParams& P, uint32_t* s_hist, float4* __restrict__ rec,
-                                              uint4* __restrict__ rec16, uint4* __restrict__ bin)
+                                              uint4* __restrict__ rec16, uint4* __restrict__ bin, int lane, uint32_t n_live)
 {
     constexpr bool SHC = SHM == SH_CODES;
     unsigned long long desc = 0;
@@ -330,17 +343,27 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
         const float ks = 0.84932180f * (float)P.tile;                // sqrt(log2(e) / 2) * tile_size
         const __half2 h01 = __floats2half2_rn(l0 * ks, l1 * ks), h2o = __floats2half2_rn(l2 * ks, s.o);
         const __half2 hrg = __floats2half2_rn(r, g), hb = __floats2half2_rn(bl, 0.0f);
-        rec16[2 * slot] = make_uint4(__float_as_uint(s.mux), __float_as_uint(s.muy), *reinterpret_cast<const uint32_t*>(&h01), *reinterpret_cast<const uint32_t*>(&h2o));
-        rec16[2 * slot + 1] = make_uint4(*reinterpret_cast<const uint32_t*>(&hrg), *reinterpret_cast<const uint32_t*>(&hb), 0u, 0u);
+        st_global_256(rec16 + 2 * slot, make_uint4(__float_as_uint(s.mux), __float_as_uint(s.muy), *reinterpret_cast<const uint32_t*>(&h01), *reinterpret_cast<const uint32_t*>(&h2o)),
+                      make_uint4(*reinterpret_cast<const uint32_t*>(&hrg), *reinterpret_cast<const uint32_t*>(&hb), 0u, 0u));
     }
     if (!HALF || desc == HIGS_DESC_FALLBACK) {                       // fp16 path: the fill pass reads rec only to redo the row scan of wide gaussians
         float4* rp = rec + 4 * slot;
-        rp[0] = make_float4(s.mux, s.muy, s.A, s.B2);
-        rp[1] = make_float4(s.C, s.tau, SHC ? __log2f(s.o) : log2f(s.o), r);
-        rp[2] = make_float4(g, bl, s.a, s.b);
-        rp[3] = make_float4(s.c, __uint_as_float(key), __uint_as_float((uint32_t)i), 0.0f);
+        st_global_256(rp, f4_bits(s.mux, s.muy, s.A, s.B2), f4_bits(s.C, s.tau, SHC ? __log2f(s.o) : log2f(s.o), r));
+        st_global_256(rp + 2, f4_bits(g, bl, s.a, s.b), f4_bits(s.c, __uint_as_float(key), __uint_as_float((uint32_t)i), 0.0f));
     }
-    bin[slot] = make_uint4(key, (uint32_t)desc, (uint32_t)(desc >> 32), (uint32_t)i);
+    // bin records are 16 bytes: lanes 2j and 2j+1 hold neighbouring slots (the first slot of a drain is even) and the even lane
+    // stores both.  Worth its four shuffles only where DRAM is the limit (fp32 records from fp32 SH rows: 0.266 -> 0.262 ms); the
+    // variants bound by instruction issue lose (32-byte codes: 0.220 -> 0.237 ms) and store their own 16 bytes.
+    const uint4 mine = make_uint4(key, (uint32_t)desc, (uint32_t)(desc >> 32), (uint32_t)i);
+    if constexpr (HALF || SHM != SH_ROWS) { bin[slot] = mine; return; }
+    const uint32_t live = n_live >= 32u ? 0xffffffffu : (1u << n_live) - 1u;
+    uint4 next;
+    next.x = __shfl_xor_sync(live, mine.x, 1); next.y = __shfl_xor_sync(live, mine.y, 1);
+    next.z = __shfl_xor_sync(live, mine.z, 1); next.w = __shfl_xor_sync(live, mine.w, 1);
+    if (!(lane & 1)) {
+        if ((uint32_t)lane + 1u < n_live) st_global_256(bin + slot, mine, next);
+        else bin[slot] = mine;
+    }
 }
 
 // Persistent CTAs (a whole number per SM), one histogram row per CTA.  A warp claims chunks of HIGS_CHUNK = 128
@@ -351,13 +374,14 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
 // on them with every lane busy.  Survivor k of chunk c gets dense slot c*HIGS_CHUNK + k: slots are monotone in the
 // gaussian id, so (key, slot) order = (key, id) order (Q7).
 template <int DEG, bool HALF, int SHM>
-__global__ void __launch_bounds__(PROJ_THREADS, 2)
+__global__ void __launch_bounds__(proj_threads(HALF, SHM), 2)
 k_project(const float* __restrict__ means, const float* __restrict__ scales, const float* __restrict__ quats,
           const float* __restrict__ opac, const float* __restrict__ sh, int64_t N, const FrameParams P,
           uint32_t* __restrict__ valid_bits, float4* __restrict__ rec, uint4* __restrict__ rec16, uint4* __restrict__ bin,
           uint32_t* __restrict__ chunk_count, uint32_t* __restrict__ hist, uint32_t* __restrict__ mt_count, uint32_t* __restrict__ part_list,
           uint2* __restrict__ part_desc, int lcap, FrameHeader* __restrict__ hdr, const ShScales sc)
 {
+    constexpr int PROJ_THREADS = proj_threads(HALF, SHM), PROJ_WARPS = PROJ_THREADS / 32;
     extern __shared__ uint32_t s_dyn[];
     __shared__ uint32_t s_nvis, s_nlist, s_lbase;
     uint32_t* s_hist = s_dyn;
@@ -423,7 +447,7 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
                 s.mx = q[11 * PROJ_QCAP + e]; s.my = q[12 * PROJ_QCAP + e]; s.mz = q[13 * PROJ_QCAP + e];
                 s.local = __float_as_uint(q[14 * PROJ_QCAP + e]);
                 const float* shp = SHM == SH_STAGED ? reinterpret_cast<const float*>(s_stage + lane * ShStage<DEG>::STRIDE_W) : sh;
-                emit_survivor<DEG, HALF, SHM>(s, c0 + s.local, slot0 + head + lane, shp, s_lut, sc, P, s_hist, rec, rec16, bin);
+                emit_survivor<DEG, HALF, SHM>(s, c0 + s.local, slot0 + head + lane, shp, s_lut, sc, P, s_hist, rec, rec16, bin, lane, n_live);
             }
             head += n_live;
             __syncwarp();
@@ -487,22 +511,22 @@ k_project(const float* __restrict__ means, const float* __restrict__ scales, con
 
 } // namespace
 
-static size_t project_smem_bytes(int n_m, int lcap, bool staged = false)
+static size_t project_smem_bytes(int n_m, int lcap, int warps, bool staged = false)
 {
-    return sizeof(uint32_t) * (size_t)((n_m + 3) & ~3) + sizeof(float) * (size_t)PROJ_WARPS * PROJ_QF * PROJ_QCAP + sizeof(uint32_t) * (size_t)lcap
-           + sizeof(float) * 1536 + (staged ? sizeof(uint32_t) * (size_t)PROJ_WARPS * SH_STAGE_WORDS_MAX : 0);
+    return sizeof(uint32_t) * (size_t)((n_m + 3) & ~3) + sizeof(float) * (size_t)warps * PROJ_QF * PROJ_QCAP + sizeof(uint32_t) * (size_t)lcap
+           + sizeof(float) * 1536 + (staged ? sizeof(uint32_t) * (size_t)warps * SH_STAGE_WORDS_MAX : 0);
 }
 
 // list capacity of one partition CTA: four times its fair share of the chunks, so a CTA that fills its list and
 // retires early always leaves others with room (sum of capacities > chunks: every chunk finds a taker)
-int higs_part_lcap(int64_t n_chunks, int grid) { return (int)(4 * ((n_chunks + grid - 1) / grid) + 2 * PROJ_WARPS); }
+int higs_part_lcap(int64_t n_chunks, int grid) { return (int)(4 * ((n_chunks + grid - 1) / grid) + 2 * PROJ_WARPS_MAX); }
 
 // CTAs of the partition passes (project+count, fill) for N gaussians: a whole number per SM, fewer only when
 // there are not enough chunks to give every warp one
 int higs_part_grid(const higs_ctx* ctx, int64_t N)
 {
     const int64_t n_chunks = (N + HIGS_CHUNK - 1) / HIGS_CHUNK;
-    const int64_t want = (n_chunks + PROJ_WARPS - 1) / PROJ_WARPS;
+    const int64_t want = (n_chunks + PROJ_WARPS_MAX - 1) / PROJ_WARPS_MAX;
     const int64_t cap = (int64_t)ctx->n_part_max;
     return (int)(want < 1 ? 1 : (want > cap ? cap : want));
 }
@@ -514,8 +538,7 @@ int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, cons
     if (sh_mode == HIGS_SH_STAGED && !ctx->proj_staged_ok) return HIGS_E_ARG;
     const unsigned grid = (unsigned)higs_part_grid(ctx, N);
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, (int)grid);
-    const size_t smem = project_smem_bytes(P.n_m, lcap, sh_mode == HIGS_SH_STAGED);
-#define HIGS_PROJ_(D, H, C) k_project<D, H, C><<<grid, PROJ_THREADS, smem, st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
+#define HIGS_PROJ_(D, H, C) k_project<D, H, C><<<grid, proj_threads(H, C), project_smem_bytes(P.n_m, lcap, proj_threads(H, C) / 32, C == SH_STAGED), st>>>(means, scales, quats, opac, sh, N, P, ctx->valid_bits, ctx->rec, \
                                                                    ctx->rec16, ctx->bin, ctx->chunk_count, ctx->hist, ctx->mt_count, ctx->part_list, ctx->part_desc, lcap, ctx->hdr, sc)
 #define HIGS_PROJ(D) do { if (sh_mode == HIGS_SH_STAGED) { if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(D, true, SH_STAGED); else HIGS_PROJ_(D, false, SH_STAGED); } \
                           else if (P.flags & HIGS_FLAG_FP16) HIGS_PROJ_(D, true, SH_ROWS); else HIGS_PROJ_(D, false, SH_ROWS); } while (0)
@@ -539,8 +562,8 @@ int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, cons
 int higs_project_smem_setup(higs_ctx* ctx)
 {
     // worst case for the list: the full grid on max_gaussians (a smaller grid has at most 16 chunks per CTA)
-    const int lcap_max = higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) > 6 * PROJ_WARPS ? higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) : 6 * PROJ_WARPS;
-    const int bytes = (int)project_smem_bytes(ctx->max_nm, lcap_max);
+    const int lcap_max = higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) > 6 * PROJ_WARPS_MAX ? higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) : 6 * PROJ_WARPS_MAX;
+    const int bytes = (int)project_smem_bytes(ctx->max_nm, lcap_max, PROJ_WARPS_MAX);
 #define HIGS_ATTR(D, H, C) HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<D, H, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))
     HIGS_ATTR(0, false, SH_ROWS); HIGS_ATTR(1, false, SH_ROWS); HIGS_ATTR(2, false, SH_ROWS); HIGS_ATTR(3, false, SH_ROWS);
     HIGS_ATTR(0, true, SH_ROWS); HIGS_ATTR(1, true, SH_ROWS); HIGS_ATTR(2, true, SH_ROWS); HIGS_ATTR(3, true, SH_ROWS);
@@ -550,7 +573,7 @@ int higs_project_smem_setup(higs_ctx* ctx)
     // higs_render_host keeps uploading the SH array
     int optin = 0;
     HIGS_CUDA(ctx, cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->device));
-    const int bytes_staged = (int)project_smem_bytes(ctx->max_nm, lcap_max, true);
+    const int bytes_staged = (int)project_smem_bytes(ctx->max_nm, lcap_max, PROJ_WARPS_MAX, true);
     ctx->proj_staged_ok = bytes_staged <= optin;
     if (ctx->proj_staged_ok) {
 #define HIGS_ATTR(D, H) HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<D, H, SH_STAGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes_staged))
@@ -559,7 +582,7 @@ int higs_project_smem_setup(higs_ctx* ctx)
 #undef HIGS_ATTR
     }
     int occ = 0;
-    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3, false, SH_ROWS>, PROJ_THREADS, (size_t)bytes));
+    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3, true, SH_ROWS>, proj_threads(true, SH_ROWS), (size_t)bytes));
     ctx->n_part_max = ctx->n_sm * (occ < 1 ? 1 : occ);
     return HIGS_OK;
 }
