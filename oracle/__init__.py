@@ -75,6 +75,10 @@ def lib():
         L.orc_bin_tile.argtypes = [C.c_int64, u8p, u32p, f32p, C.c_int, C.c_int, C.c_int, C.c_int, u32p, u32p, u32p, u32p, u32p, C.c_int64]
         L.orc_render_batched_tile.restype = None
         L.orc_render_batched_tile.argtypes = [u32p, u32p, f32p, f32p, f32p, f64p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, f64p]
+        L.orc_bin_grid.restype = C.c_int64
+        L.orc_bin_grid.argtypes = [C.c_int64, u8p, u32p, f32p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, u32p, u32p, u32p, u32p, u32p, C.c_int64]
+        L.orc_render_batched_grid.restype = None
+        L.orc_render_batched_grid.argtypes = [u32p, u32p, f32p, f32p, f32p, f64p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, f64p]
         L.orc_sh32_scales.restype = None; L.orc_sh32_scales.argtypes = [C.c_int64, f32p, f32p]
         L.orc_sh32_encode.restype = None; L.orc_sh32_encode.argtypes = [C.c_int64, f32p, f32p, u8p]
         L.orc_sh32_decode.restype = None; L.orc_sh32_decode.argtypes = [C.c_int64, u8p, f32p, f32p]
@@ -188,16 +192,18 @@ def scan(geo_row: np.ndarray, W: int, H: int, cw: int = MT_W, ch: int = MT_H) ->
     return out[:n].copy()
 
 
-def bin_lists(pr: Projected, B_r: int = B_R, tile: int = TILE) -> Lists:
-    """O-LIST.  tile = render-tile edge (8, or 16 for the variant of PAPER.md:286-299); macro-tile = 8 x 4 tiles."""
-    nmx, nmy = (pr.W + 8 * tile - 1) // (8 * tile), (pr.H + 4 * tile - 1) // (4 * tile)
+def bin_lists(pr: Projected, B_r: int = B_R, tile: int = TILE, mt: tuple = (8, 4)) -> Lists:
+    """O-LIST.  tile = render-tile edge (8, or 16 for the variant of PAPER.md:286-299); mt = render tiles per macro-tile
+    in x and y (the paper's 8 x 4; 4 x 8 and 16 x 2 for the shape sweep)."""
+    mw, mh = mt[0] * tile, mt[1] * tile
+    nmx, nmy = (pr.W + mw - 1) // mw, (pr.H + mh - 1) // mh
     NM = nmx * nmy
     mt_count = np.zeros(NM, np.uint32); mt_offset = np.zeros(NM + 1, np.uint32); batch_offset = np.zeros(NM + 1, np.uint32)
-    args = (pr.N, _p(pr.valid, C.c_uint8), _p(pr.key, C.c_uint32), _p(pr.geo, C.c_float), pr.W, pr.H, B_r, tile,
+    args = (pr.N, _p(pr.valid, C.c_uint8), _p(pr.key, C.c_uint32), _p(pr.geo, C.c_float), pr.W, pr.H, B_r, mw, mh,
             _p(mt_count, C.c_uint32), _p(mt_offset, C.c_uint32), _p(batch_offset, C.c_uint32))
-    npairs = int(lib().orc_bin_tile(*args, None, None, 0))
+    npairs = int(lib().orc_bin_grid(*args, None, None, 0))
     keys = np.zeros(max(npairs, 1), np.uint32); ids = np.zeros(max(npairs, 1), np.uint32)
-    lib().orc_bin_tile(*args, _p(keys, C.c_uint32), _p(ids, C.c_uint32), npairs)
+    lib().orc_bin_grid(*args, _p(keys, C.c_uint32), _p(ids, C.c_uint32), npairs)
     return Lists(npairs, int(batch_offset[NM]), mt_count, mt_offset, batch_offset, keys[:npairs], ids[:npairs])
 
 
@@ -222,13 +228,13 @@ def brute(pr: Projected, window=None, terminate: bool = True, threads: Optional[
     return _render(lib().orc_brute, pr, window, terminate, threads, want_T)
 
 
-def render_batched(pr: Projected, ls: Lists, B_r: int = B_R, terminate: bool = True, tile: int = TILE) -> np.ndarray:
+def render_batched(pr: Projected, ls: Lists, B_r: int = B_R, terminate: bool = True, tile: int = TILE, mt: tuple = (8, 4)) -> np.ndarray:
     """The method step by step: per-macro-tile lists, batches of B_r, Eq. (1) merge."""
     out = np.zeros((pr.H, pr.W, 3), np.float64)
     ids = ls.ids if ls.ids.size else np.zeros(1, np.uint32)
-    lib().orc_render_batched_tile(_p(ls.mt_offset, C.c_uint32), _p(ids, C.c_uint32), _p(pr.geo, C.c_float),
+    lib().orc_render_batched_grid(_p(ls.mt_offset, C.c_uint32), _p(ids, C.c_uint32), _p(pr.geo, C.c_float),
                                   _p(pr.conic, C.c_float), _p(pr.opac, C.c_float), _p(pr.rgb, C.c_double),
-                                  pr.W, pr.H, B_r, tile, int(terminate), _p(out, C.c_double))
+                                  pr.W, pr.H, B_r, mt[0] * tile, mt[1] * tile, int(terminate), _p(out, C.c_double))
     return out
 
 

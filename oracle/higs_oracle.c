@@ -351,14 +351,14 @@ static int cmp_u64(const void* pa, const void* pb)
     return a < b ? -1 : (a > b ? 1 : 0);
 }
 
-/* tile = render-tile edge in px: 8 or 16 (the variant of Table 2); the macro-tile is
- * always 8 x 4 render tiles, i.e. (8 tile) x (4 tile) px. */
-int64_t orc_bin_tile(int64_t N, const uint8_t* valid, const uint32_t* key, const float* geo,
-                     int W, int H, int B_r, int tile,
+/* Macro-tile of MT_W x MT_H pixels: the paper's is 8 x 4 render tiles of 8 x 8 px = 64 x 32; 128 x 64 in the
+ * 16 x 16-tile variant (Table 2); other groupings of 32 render tiles (4 x 8, 16 x 2) for the macro-tile
+ * shape sweep.  The lists depend on the macro-tile's extent in pixels only, not on how it is cut into render tiles. */
+int64_t orc_bin_grid(int64_t N, const uint8_t* valid, const uint32_t* key, const float* geo,
+                     int W, int H, int B_r, int MT_W, int MT_H,
                      uint32_t* mt_count, uint32_t* mt_offset, uint32_t* batch_offset,
                      uint32_t* keys, uint32_t* ids, int64_t cap)
 {
-    const int MT_W = 8 * tile, MT_H = 4 * tile;
     const int nmx = (W + MT_W - 1) / MT_W, nmy = (H + MT_H - 1) / MT_H, NM = nmx * nmy;
     int32_t* cells = (int32_t*)malloc(sizeof(int32_t) * (size_t)NM);
     memset(mt_count, 0, sizeof(uint32_t) * (size_t)NM);
@@ -391,6 +391,15 @@ int64_t orc_bin_tile(int64_t N, const uint8_t* valid, const uint32_t* key, const
     }
     free(cells);
     return npairs;
+}
+
+/* tile = render-tile edge in px (8 or 16), macro-tile = 8 x 4 render tiles */
+int64_t orc_bin_tile(int64_t N, const uint8_t* valid, const uint32_t* key, const float* geo,
+                     int W, int H, int B_r, int tile,
+                     uint32_t* mt_count, uint32_t* mt_offset, uint32_t* batch_offset,
+                     uint32_t* keys, uint32_t* ids, int64_t cap)
+{
+    return orc_bin_grid(N, valid, key, geo, W, H, B_r, 8 * tile, 4 * tile, mt_count, mt_offset, batch_offset, keys, ids, cap);
 }
 
 int64_t orc_bin(int64_t N, const uint8_t* valid, const uint32_t* key, const float* geo,
@@ -563,11 +572,10 @@ int64_t orc_brute(int64_t N, const uint8_t* valid, const uint32_t* key, const fl
  * terminate=1 stops a pixel once the running product of transmittances drops below 1e-4.
  * Full image only; pixel-major, slow: small scenes only.  out: H*W*3 fp64.
  * ------------------------------------------------------------------------------------- */
-void orc_render_batched_tile(const uint32_t* mt_offset, const uint32_t* ids, const float* geo,
+void orc_render_batched_grid(const uint32_t* mt_offset, const uint32_t* ids, const float* geo,
                              const float* conic, const float* opac, const double* rgb,
-                             int W, int H, int B_r, int tile, int terminate, double* out)
+                             int W, int H, int B_r, int MT_W, int MT_H, int terminate, double* out)
 {
-    const int MT_W = 8 * tile, MT_H = 4 * tile;
     const int nmx = (W + MT_W - 1) / MT_W, nmy = (H + MT_H - 1) / MT_H;
     for (int my = 0; my < nmy; ++my) for (int mx = 0; mx < nmx; ++mx) {
         const int m = my * nmx + mx;
@@ -595,6 +603,13 @@ void orc_render_batched_tile(const uint32_t* mt_offset, const uint32_t* ids, con
             out[3 * pix] = C[0]; out[3 * pix + 1] = C[1]; out[3 * pix + 2] = C[2];
         }
     }
+}
+
+void orc_render_batched_tile(const uint32_t* mt_offset, const uint32_t* ids, const float* geo,
+                             const float* conic, const float* opac, const double* rgb,
+                             int W, int H, int B_r, int tile, int terminate, double* out)
+{
+    orc_render_batched_grid(mt_offset, ids, geo, conic, opac, rgb, W, H, B_r, 8 * tile, 4 * tile, terminate, out);
 }
 
 void orc_render_batched(const uint32_t* mt_offset, const uint32_t* ids, const float* geo,
