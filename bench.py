@@ -469,6 +469,10 @@ def run_higs(args) -> int:
         run_variant("fp32_16x16", 0, frame, "PAPER.md:286-299 (Table 2): 16x16 render tiles, macro-tiles of 128x64 px")
         run_variant("fp16_16x16", hg.HIGS_FLAG_FP16, frame, "both")
         hg.higs_set_tile(ctx, 8)
+        for tx, ty in ((4, 8), (16, 2)):                                # macro-tile shape sweep: 32 render tiles grouped otherwise
+            hg.higs_set_macro_tile(ctx, tx, ty)
+            run_variant(f"fp32_8x8_mt{tx}x{ty}", 0, frame, f"macro-tiles of {tx} x {ty} render tiles = {8 * tx} x {8 * ty} px instead of 8 x 4 (PAPER.md:73)")
+        hg.higs_set_macro_tile(ctx, 8, 4)
         hg.higs_scene_upload(ctx, *[np.ascontiguousarray(a, dtype=np.float32) for a in (scene.means, scene.scales, scene.quats, scene.opacities, scene.sh)], scene.degree)
         hg.higs_scene_compress_sh(ctx)
         view = lambda i: hg.higs_render_view(ctx, ccams_1080[views_for_rank(i, rank, world, n_views)], 1920, 1080, img, stream.cuda_stream)

@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define HIGS_ABI_VERSION 2    /* 2: higs_lists.tile_load, higs_stats.tile, set_tile / scene_sort_spatial / scene_compress_sh / get_sh32 */
+#define HIGS_ABI_VERSION 3    /* 2: higs_lists.tile_load, higs_stats.tile, set_tile / scene_sort_spatial / scene_compress_sh / get_sh32; 3: set_macro_tile */
 
 #define HIGS_TILE        8      /* render tile edge, px  */
 #define HIGS_MT_W        64     /* macro-tile width,  px (8 tiles)  */
@@ -141,6 +141,11 @@ int higs_set_batch_cap(higs_ctx* ctx, int batch_cap);
  * stays 8 x 4 render tiles, i.e. 64 x 32 or 128 x 64 px, and m = my*ceil(W/(8 tile)) + mx.  Reallocates the per-unit
  * buffers (synchronises the device). */
 int higs_set_tile(higs_ctx* ctx, int tile);
+/* Macro-tile shape in render tiles (shape sweep): 8 x 4 (default), 4 x 8 or 16 x 2; always
+ * HIGS_MT_TILES = 32 tiles, m = my*ceil(W/(tiles_x tile)) + mx, tile t of a macro-tile at column t % tiles_x, row t / tiles_x.
+ * Shapes other than 8 x 4 exist on the fp32 path with 8 x 8 tiles only: HIGS_E_ARG with tile 16, and a frame rendered with
+ * HIGS_FLAG_FP16 set returns HIGS_E_ARG (the fp16 path's coordinate range is that of the 8 x 4 macro-tile). */
+int higs_set_macro_tile(higs_ctx* ctx, int tiles_x, int tiles_y);
 
 /* Render one frame.  All array arguments are DEVICE pointers:
  *   means [N][3], scales [N][3], quats [N][4], opacities [N], sh [N][(degree+1)^2][3],

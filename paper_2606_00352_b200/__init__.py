@@ -23,7 +23,7 @@ HIGS_FLAG_STAGE_TIMERS, HIGS_FLAG_COUNT_EVALS, HIGS_FLAG_NO_XBATCH_CUT, HIGS_FLA
 HIGS_TILE, HIGS_MT_W, HIGS_MT_H, HIGS_MT_TILES, HIGS_BATCH_CAP = 8, 64, 32, 32, 1024
 
 EXPORTS = ["higs_abi_version", "higs_strerror", "higs_last_error", "higs_create", "higs_destroy", "higs_set_flags",
-           "higs_set_batch_cap", "higs_set_tile", "higs_render", "higs_render_host", "higs_scene_upload", "higs_render_view_host",
+           "higs_set_batch_cap", "higs_set_tile", "higs_set_macro_tile", "higs_render", "higs_render_host", "higs_scene_upload", "higs_render_view_host",
            "higs_render_view", "higs_scene_sort_spatial", "higs_scene_compress_sh", "higs_get_sh32", "higs_get_stats", "higs_get_lists", "higs_get_records", "higs_sort_segments", "higs_download"]
 
 
@@ -81,6 +81,7 @@ def load() -> C.CDLL:
         L.higs_set_flags.restype = C.c_int; L.higs_set_flags.argtypes = [vp, C.c_uint32]
         L.higs_set_batch_cap.restype = C.c_int; L.higs_set_batch_cap.argtypes = [vp, C.c_int]
         L.higs_set_tile.restype = C.c_int; L.higs_set_tile.argtypes = [vp, C.c_int]
+        L.higs_set_macro_tile.restype = C.c_int; L.higs_set_macro_tile.argtypes = [vp, C.c_int, C.c_int]
         L.higs_render.restype = C.c_int
         L.higs_render.argtypes = [vp, f32p, f32p, f32p, f32p, f32p, C.c_int, C.c_int64, C.POINTER(higs_camera),
                                   C.c_int, C.c_int, f32p, vp]
@@ -163,6 +164,10 @@ def higs_set_batch_cap(ctx, batch_cap: int) -> None:
 
 def higs_set_tile(ctx, tile: int) -> None:
     _check(load().higs_set_tile(ctx, tile), "higs_set_tile", ctx)
+
+
+def higs_set_macro_tile(ctx, tiles_x: int, tiles_y: int) -> None:
+    _check(load().higs_set_macro_tile(ctx, tiles_x, tiles_y), "higs_set_macro_tile", ctx)
 
 
 def higs_render(ctx, means, scales, quats, opacities, sh, degree: int, cam: higs_camera, W: int, H: int, out_rgb,
@@ -274,11 +279,13 @@ class Renderer:
     """Owns a higs_ctx.  render(scene tensors on the device, camera) -> (H, W, 3) fp32 device tensor."""
 
     def __init__(self, max_gaussians: int, max_W: int, max_H: int, max_pairs: int = 0, device: int = 0,
-                 flags: int = 0, batch_cap: int = HIGS_BATCH_CAP, tile: int = HIGS_TILE):
+                 flags: int = 0, batch_cap: int = HIGS_BATCH_CAP, tile: int = HIGS_TILE, mt: tuple = (8, 4)):
         self.ctx = higs_create(device, max_gaussians, max_W, max_H, max_pairs)
         self.device = device
         if tile != HIGS_TILE:
             higs_set_tile(self.ctx, tile)
+        if tuple(mt) != (8, 4):
+            higs_set_macro_tile(self.ctx, int(mt[0]), int(mt[1]))
         if flags:
             higs_set_flags(self.ctx, flags)
         if batch_cap != HIGS_BATCH_CAP:

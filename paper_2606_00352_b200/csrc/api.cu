@@ -69,9 +69,11 @@ int render_impl(higs_ctx* ctx, const float* means, const float* scales, const fl
     P.fx = cam->fx; P.fy = cam->fy; P.cx = cam->cx; P.cy = cam->cy; P.near_z = cam->near_z;
     memcpy(P.cam, cam->cam_pos, sizeof(P.cam));
     P.W = W; P.H = H;
-    P.tile = ctx->tile;
+    P.tile = ctx->tile; P.mt_tx = ctx->mt_tx; P.mt_ty = ctx->mt_ty;
+    if (P.mt_tx != 8 && (P.tile != 8 || (ctx->flags & HIGS_FLAG_FP16))) return HIGS_E_ARG;   // other shapes: fp32 path, 8 x 8 tiles
     { const float tx = 0.65f * (float)W, ty = 0.65f * (float)H; P.limx = tx / P.fx; P.limy = ty / P.fy; }   // one rounding per op, as N-PROJ writes it
-    P.n_mx = (W + 8 * P.tile - 1) / (8 * P.tile); P.n_my = (H + 4 * P.tile - 1) / (4 * P.tile); P.n_m = P.n_mx * P.n_my;
+    P.n_mx = (W + P.mt_tx * P.tile - 1) / (P.mt_tx * P.tile); P.n_my = (H + P.mt_ty * P.tile - 1) / (P.mt_ty * P.tile); P.n_m = P.n_mx * P.n_my;
+    if (P.n_m > ctx->max_nm) return HIGS_E_ARG;
     P.degree = degree; P.batch_cap = ctx->batch_cap; P.flags = ctx->flags;
     P.max_pairs = (uint32_t)ctx->max_pairs; P.max_units = (uint32_t)ctx->max_units;
     const bool timers = (ctx->flags & HIGS_FLAG_STAGE_TIMERS) != 0;
@@ -167,13 +169,18 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     if (max_gaussians < 0 || max_gaussians > 0xfffffff0ll || max_W <= 0 || max_H <= 0) return HIGS_E_ARG;
     if (max_pairs <= 0) max_pairs = 4 * max_gaussians + 65536;
     if (max_pairs > 0x7fffffffll) return HIGS_E_ARG;
-    const int64_t nm = (int64_t)((max_W + HIGS_MT_W - 1) / HIGS_MT_W) * ((max_H + HIGS_MT_H - 1) / HIGS_MT_H);
+    int64_t nm = 0;                                                 // macro-tiles at max_W x max_H, the most over the supported shapes (8 x 8 px tiles)
+    for (int tx = 4; tx <= 16; tx *= 2) {
+        const int mw = tx * HIGS_TILE, mh = (HIGS_MT_TILES / tx) * HIGS_TILE;
+        const int64_t v = (int64_t)((max_W + mw - 1) / mw) * ((max_H + mh - 1) / mh);
+        if (v > nm) nm = v;
+    }
     if (nm > HIGS_MAX_NM) return HIGS_E_ARG;
     higs_ctx* ctx = new (std::nothrow) higs_ctx();
     if (!ctx) return HIGS_E_NOMEM;
     memset(ctx, 0, sizeof(*ctx));
     ctx->device = device; ctx->max_gaussians = max_gaussians; ctx->max_W = max_W; ctx->max_H = max_H;
-    ctx->max_nm = (int)nm; ctx->max_pairs = max_pairs; ctx->batch_cap = HIGS_BATCH_CAP; ctx->flags = 0; ctx->tile = HIGS_TILE;
+    ctx->max_nm = (int)nm; ctx->max_pairs = max_pairs; ctx->batch_cap = HIGS_BATCH_CAP; ctx->flags = 0; ctx->tile = HIGS_TILE; ctx->mt_tx = 8; ctx->mt_ty = 4;
     int rc = HIGS_OK;
     auto fail = [&](int code) { higs_destroy(ctx); return code; };
     if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return fail(HIGS_E_CUDA); }
@@ -278,12 +285,20 @@ int higs_set_batch_cap(higs_ctx* ctx, int batch_cap)
 
 int higs_set_tile(higs_ctx* ctx, int tile)
 {
-    if (!ctx || (tile != 8 && tile != 16)) return HIGS_E_ARG;
+    if (!ctx || (tile != 8 && tile != 16) || (tile != 8 && ctx->mt_tx != 8)) return HIGS_E_ARG;
     if (tile == ctx->tile) return HIGS_OK;
     HIGS_CUDA(ctx, cudaSetDevice(ctx->device));
     HIGS_CUDA(ctx, cudaDeviceSynchronize());
     ctx->tile = tile;
     return alloc_unit_buffers(ctx);
+}
+
+int higs_set_macro_tile(higs_ctx* ctx, int tiles_x, int tiles_y)
+{
+    if (!ctx || tiles_x * tiles_y != HIGS_MT_TILES || (tiles_x != 4 && tiles_x != 8 && tiles_x != 16)) return HIGS_E_ARG;
+    if (tiles_x != 8 && ctx->tile != 8) return HIGS_E_ARG;
+    ctx->mt_tx = tiles_x; ctx->mt_ty = tiles_y;
+    return HIGS_OK;
 }
 
 int higs_render(higs_ctx* ctx, const float* means, const float* scales, const float* quats, const float* opacities,

@@ -191,11 +191,11 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
         const float4 s0 = __ldcs(rec + 4 * slot), s1 = __ldcs(rec + 4 * slot + 1), s2 = __ldcs(rec + 4 * slot + 2),
                      s3 = __ldcs(rec + 4 * slot + 3);
         RowScan rs{};
-        rs.init(s0.x, s0.y, s2.z, s2.w, s3.x, tau_scan(s2.z, s2.w, s3.x, s1.y), (float)(4 * P.tile), P.n_my);
+        rs.init(s0.x, s0.y, s2.z, s2.w, s3.x, tau_scan(s2.z, s2.w, s3.x, s1.y), (float)(P.mt_ty * P.tile), P.n_my);
         const float fW = (float)P.W, fH = (float)P.H;
         for (int r = rs.r0; r <= rs.r1; ++r) {
             int m0, m1;
-            if (!rs.row(r, (float)(8 * P.tile), (float)(4 * P.tile), fW, fH, P.n_mx, m0, m1)) continue;
+            if (!rs.row(r, (float)(P.mt_tx * P.tile), (float)(P.mt_ty * P.tile), fW, fH, P.n_mx, m0, m1)) continue;
             for (int m = m0; m <= m1; ++m) {
                 const uint32_t at = atomicAdd(&s_cursor[r * P.n_mx + m], 1u);
                 HIGS_ASSERT(at >= mt_offset[r * P.n_mx + m] && at < mt_offset[r * P.n_mx + m + 1]);

@@ -55,7 +55,8 @@ struct FrameParams {
     int   n_mx, n_my, n_m;
     int   degree;
     int   batch_cap;
-    int   tile;                // render-tile edge, 8 or 16; macro-tile = 8 x 4 tiles
+    int   tile;                // render-tile edge, 8 or 16
+    int   mt_tx, mt_ty;        // render tiles per macro-tile in x and y: 8 x 4, or 4 x 8 / 16 x 2 (higs_set_macro_tile)
     float limx, limy;          // (0.65 W) / fx, (0.65 H) / fy: the clamp of the Jacobian (N-PROJ step 3), the same for every gaussian
     uint32_t flags;
     uint32_t max_pairs, max_units;
@@ -74,6 +75,7 @@ struct higs_ctx {
     uint32_t flags;
     int batch_cap;
     int tile;                  // render-tile edge in effect (8 or 16)
+    int mt_tx, mt_ty;          // macro-tile shape in render tiles (8 x 4 unless higs_set_macro_tile changed it)
     // scratch (device)
     uint32_t* valid_bits;      // [ceil(maxN/32)]
     float4*   rec;             // [slots][4]  mux,muy,A,B2 | C,tau,log2o,r | g,b,a,b | c,bits(key),id,-   (64 B; the rasterizer gathers the

@@ -306,14 +306,14 @@ __device__ __forceinline__ void emit_survivor(const Survivor& s, int64_t i, size
     unsigned long long desc = 0;
     {
         RowScan rs{};
-        rs.template init<SHC>(s.mux, s.muy, s.a, s.b, s.c, tau_scan(s.a, s.b, s.c, s.tau), (float)(4 * P.tile), P.n_my);
+        rs.template init<SHC>(s.mux, s.muy, s.a, s.b, s.c, tau_scan(s.a, s.b, s.c, s.tau), (float)(P.mt_ty * P.tile), P.n_my);
         const float fW = (float)P.W, fH = (float)P.H;
         bool fits = (rs.r1 - rs.r0) <= 3 && P.n_mx <= 511 && rs.r0 <= 511;
         desc = (unsigned long long)(uint32_t)rs.r0 | ((unsigned long long)(uint32_t)((rs.r1 - rs.r0) & 3) << 9);
         for (int r = rs.r0; r <= rs.r1; ++r) {
             int m0, m1;
             uint32_t field = 511u;
-            if (rs.template row<SHC>(r, (float)(8 * P.tile), (float)(4 * P.tile), fW, fH, P.n_mx, m0, m1)) {
+            if (rs.template row<SHC>(r, (float)(P.mt_tx * P.tile), (float)(P.mt_ty * P.tile), fW, fH, P.n_mx, m0, m1)) {
                 HIGS_ASSERT(r >= 0 && r < P.n_my && m0 >= 0 && m1 < P.n_mx);
                 for (int m = m0; m <= m1; ++m) atomicAdd(&s_hist[r * P.n_mx + m], 1u);
                 fits = fits && (m1 - m0) <= 15;

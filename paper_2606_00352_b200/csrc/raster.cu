@@ -103,10 +103,11 @@ __device__ __forceinline__ __half2 ex2_h2(__half2 x)
 
 // Conservative render-tile overlap mask of one gaussian inside a macro-tile (reading Q9: internal, never
 // compared with the oracle): N-SCAN on the covariance (a, b, c), det = a c - b^2 given by the caller from an identity
-// that does not cancel, threshold tau_m, over a grid of 8 x 4 cells of size `cell` whose origin is (X0, Y0); the image
+// that does not cancel, threshold tau_m, over a grid of MTX x (32 / MTX) cells of size `cell` whose origin is (X0, Y0); the image
 // ends at (fW, fH) in the same units.  Approximate rcp / sqrt: every extent is good to ~1e-6 relative; extents are widened
 // by `slack` on top (pixel centres sit half a pixel inside their tile) and a gaussian whose extent exceeds `huge` takes
 // every tile.
+template <int MTX>
 __device__ __forceinline__ uint32_t tile_mask_cov(float mux, float muy, float a, float b, float c, float det, float tau_m,
                                                   float X0, float Y0, float cell, float rcell, float fW, float fH, float slack, float huge)
 {
@@ -118,7 +119,7 @@ __device__ __forceinline__ uint32_t tile_mask_cov(float mux, float muy, float a,
     const float ytop = muy - hy, ybot = muy + hy;
     uint32_t mask = 0;
 #pragma unroll
-    for (int tr = 0; tr < 4; ++tr) {
+    for (int tr = 0; tr < 32 / MTX; ++tr) {
         const float y0 = Y0 + cell * tr;
         const float y1 = fminf(y0 + cell, fH);
         const float ylo = fmaxf(y0, ytop) - muy, yhi = fminf(y1, ybot) - muy;
@@ -128,10 +129,10 @@ __device__ __forceinline__ uint32_t tile_mask_cov(float mux, float muy, float a,
         float xmax = (ylo <= yR && yR <= yhi) ? hx : fmaxf(fmaf(boc, ylo, rlo), fmaf(boc, yhi, rhi)) + slack;
         float xmin = (ylo <= -yR && -yR <= yhi) ? -hx : fminf(fmaf(boc, ylo, -rlo), fmaf(boc, yhi, -rhi)) - slack;
         xmax = fminf(xmax + mux, fW) - X0; xmin = fmaxf(xmin + mux, X0) - X0;
-        if (!(xmax >= 0.0f) || !(xmin < 8.0f * cell) || !(xmax >= xmin)) continue;
-        const int c0 = max(0, (int)floorf(xmin * rcell)), c1 = min(7, (int)floorf(xmax * rcell));
+        if (!(xmax >= 0.0f) || !(xmin < (float)MTX * cell) || !(xmax >= xmin)) continue;
+        const int c0 = max(0, (int)floorf(xmin * rcell)), c1 = min(MTX - 1, (int)floorf(xmax * rcell));
         if (c0 > c1) continue;
-        mask |= ((2u << c1) - (1u << c0)) << (tr * 8);
+        mask |= ((2u << c1) - (1u << c0)) << (tr * MTX);
     }
     return mask;
 }
@@ -161,14 +162,17 @@ __device__ __forceinline__ int cut_prefix(unsigned long long* __restrict__ word,
     return sum;
 }
 
-template <int TILE> struct TileGeo {
-    static constexpr int MT_W = 8 * TILE, MT_H = 4 * TILE;
+// MTX x MTY render tiles per macro-tile: 8 x 4; 4 x 8 and 16 x 2 for the shape sweep (higs_set_macro_tile).  Tile t of a
+// macro-tile sits in column t % MTX, row t / MTX.
+template <int TILE, int MTX = 8> struct TileGeo {
+    static constexpr int MTY = 32 / MTX, MT_SH = MTX == 4 ? 2 : (MTX == 8 ? 3 : 4);
+    static constexpr int MT_W = MTX * TILE, MT_H = MTY * TILE;
     static constexpr int PPL = TILE * TILE / 32;   // pixels per lane
     static constexpr int NP = PPL / 2;             // pairs of pixels per lane
     static constexpr int RS = 32 / TILE;           // rows between consecutive pixels of a lane: lane -> column lane % TILE, rows lane / TILE + RS * i
 };
 
-template <bool COUNT, int TILE, bool HALF>
+template <bool COUNT, int TILE, bool HALF, int MTX = 8>
 __global__ void __launch_bounds__(RAS_THREADS, HALF ? 3 : (TILE == 8 ? 3 : 2))
 k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict__ rec, const uint4* __restrict__ rec16,
          const uint32_t* __restrict__ mt_offset, const uint32_t* __restrict__ mt_count,
@@ -178,7 +182,8 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
          float4* __restrict__ partial, uint32_t* __restrict__ unit_active,
          unsigned long long* __restrict__ cut_word, int* __restrict__ cut_term, uint32_t* __restrict__ tile_load)
 {
-    typedef TileGeo<TILE> G;
+    typedef TileGeo<TILE, MTX> G;
+    static_assert(MTX == 8 || (TILE == 8 && !HALF), "other macro-tile shapes: fp32 path, 8 x 8 tiles (the fp16 path's coordinate range is the 8 x 4 macro-tile's, PAPER.md:280)");
     constexpr int NP = G::NP;
     extern __shared__ __align__(16) unsigned char s_raw[];
     RasCtl& S = *reinterpret_cast<RasCtl*>(s_raw + RasLayout<HALF>::rec_bytes);
@@ -215,12 +220,12 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             const uint32_t u0c = batch_offset[mc];
             const uint32_t jc = uc - u0c;
             const int mtx = (int)(mc % (uint32_t)P.n_mx), mty = (int)(mc / (uint32_t)P.n_mx);
-            const int tiles_x = min(8, (P.W - mtx * G::MT_W + TILE - 1) / TILE);
-            const int tiles_y = min(4, (P.H - mty * G::MT_H + TILE - 1) / TILE);
+            const int tiles_x = min(MTX, (P.W - mtx * G::MT_W + TILE - 1) / TILE);
+            const int tiles_y = min(G::MTY, (P.H - mty * G::MT_H + TILE - 1) / TILE);
             bool saturated = false;
             if (use_cut && jc > 0)
                 saturated = cut_prefix(cut_word + (size_t)mc * HIGS_MT_TILES + lane, cut_term + (size_t)u0c * HIGS_MT_TILES + lane, jc) < LOGT_EPS;
-            const bool inb = (lane & 7) < tiles_x && (lane >> 3) < tiles_y;
+            const bool inb = (lane & (MTX - 1)) < tiles_x && (lane >> G::MT_SH) < tiles_y;
             const uint32_t cut = __ballot_sync(0xffffffffu, saturated || !inb);
             if (cut == 0xffffffffu) {                                 // nothing left to see behind the earlier batches
                 if (lane == 0) unit_active[uc] = 0;
@@ -310,7 +315,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
                     const float c = il2 * il2, det = c * il0 * il0;
                     const float a = (l01.y * l01.y + l2o.x * l2o.x) * det, b = -l01.y * il0 * c;
                     const float tau_m = 1.02f * (7.99435344f + __log2f(l2o.y)) + 0.05f;
-                    gm = tile_mask_cov(xt, yt, a, b, c, det, tau_m, -4.0f, -2.0f, 1.0f, 1.0f, (fW - (X0 + 0.5f * G::MT_W)) * (1.0f / TILE),
+                    gm = tile_mask_cov<8>(xt, yt, a, b, c, det, tau_m, -4.0f, -2.0f, 1.0f, 1.0f, (fW - (X0 + 0.5f * G::MT_W)) * (1.0f / TILE),
                                        (fH - (Y0 + 0.5f * G::MT_H)) * (1.0f / TILE), 0.05f, 3000.0f) & ~cut;
                 } else {
                     // c and det from the identities det = a / C, c = A det, cond = a c / det = A a (recomputing det from the
@@ -319,7 +324,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
                     const float4 q0 = s_rec[REC_F4 * i], q1 = s_rec[REC_F4 * i + 1], q2 = s_rec[REC_F4 * i + 2];
                     const float det = q2.z * rcp_approx(q1.x);
                     const float tau_m = q1.y * fmaf(q0.z * q2.z, 9.5367431640625e-07f, 1.002f);
-                    gm = tile_mask_cov(q0.x, q0.y, q2.z, q2.w, q0.z * det, det, tau_m, X0, Y0, (float)TILE, 1.0f / TILE, fW, fH, 0.25f, 3.0e4f) & ~cut;
+                    gm = tile_mask_cov<MTX>(q0.x, q0.y, q2.z, q2.w, q0.z * det, det, tau_m, X0, Y0, (float)TILE, 1.0f / TILE, fW, fH, 0.25f, 3.0e4f) & ~cut;
                 }
             }
             uint32_t mine = 0;
@@ -359,7 +364,7 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
             if (t >= n_tiles) break;
             t = __ffs(__ballot_sync(0xffffffffu, t_cnt != 0u && t_rank == (uint32_t)t)) - 1;
             const uint32_t mine = lane < RAS_MB ? S.masks[t * MASK_PITCH + lane] : 0u;   // lane k holds mini-batch k's word
-            const int col = (t & 7) * TILE + (lane % TILE), row0 = (t >> 3) * TILE + (lane / TILE);   // inside the macro-tile
+            const int col = (t & (MTX - 1)) * TILE + (lane % TILE), row0 = (t >> G::MT_SH) * TILE + (lane / TILE);   // inside the macro-tile
             uint32_t wr = 0, rd = 0, n_done = 0;
             bool sat = false;
             float tm;                                                 // largest transmittance left in the tile
@@ -537,13 +542,13 @@ k_raster(const unsigned long long* __restrict__ pairs, const float4* __restrict_
 }
 
 // a8: one warp per render tile; Eq. (1): C = C_0 + T_0 C_1 + T_0 T_1 C_2 + ...  fp32 accumulation on both paths.
-template <int TILE, bool HALF>
+template <int TILE, bool HALF, int MTX = 8>
 __global__ void __launch_bounds__(256)
 k_merge_image(const float4* __restrict__ partial, const uint32_t* __restrict__ unit_active,
               const uint32_t* __restrict__ batch_offset, const FrameParams P, const FrameHeader* __restrict__ hdr,
               float* __restrict__ out_rgb)
 {
-    typedef TileGeo<TILE> G;
+    typedef TileGeo<TILE, MTX> G;
     constexpr int PPL = G::PPL;
     const int lane = threadIdx.x & 31;
     pdl_wait();
@@ -551,9 +556,10 @@ k_merge_image(const float4* __restrict__ partial, const uint32_t* __restrict__ u
     const int m = gw >> 5, t = gw & 31;
     if (m >= P.n_m) return;
     const int mtx = m % P.n_mx, mty = m / P.n_mx;
-    const int x = mtx * G::MT_W + (t & 7) * TILE + (lane % TILE);
-    const int y0 = mty * G::MT_H + (t >> 3) * TILE + (lane / TILE);
-    if (mtx * G::MT_W + (t & 7) * TILE >= P.W || mty * G::MT_H + (t >> 3) * TILE >= P.H) return;
+    const int tcol = (t & (MTX - 1)) * TILE, trow = (t >> G::MT_SH) * TILE;
+    const int x = mtx * G::MT_W + tcol + (lane % TILE);
+    const int y0 = mty * G::MT_H + trow + (lane / TILE);
+    if (mtx * G::MT_W + tcol >= P.W || mty * G::MT_H + trow >= P.H) return;
     uint32_t u0 = 0, nb = 0;
     if (!hdr->overflow) { u0 = batch_offset[m]; nb = batch_offset[m + 1] - u0; }   // this macro-tile's units, in depth order
     float T[PPL], r[PPL], g[PPL], b[PPL];
@@ -594,24 +600,24 @@ k_merge_image(const float4* __restrict__ partial, const uint32_t* __restrict__ u
     }
 }
 
-template <bool COUNT, int TILE, bool HALF>
+template <bool COUNT, int TILE, bool HALF, int MTX = 8>
 int setup_one(higs_ctx* ctx, int* occ_out)
 {
     const int smem = (int)ras_smem_bytes<HALF>();
-    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_raster<COUNT, TILE, HALF>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    HIGS_CUDA(ctx, cudaFuncSetAttribute(k_raster<COUNT, TILE, HALF, MTX>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     if (occ_out) {
         int occ = 0;
-        HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_raster<COUNT, TILE, HALF>, RAS_THREADS, smem));
+        HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_raster<COUNT, TILE, HALF, MTX>, RAS_THREADS, smem));
         *occ_out = occ > 0 ? occ : 1;
     }
     return HIGS_OK;
 }
 
-template <bool COUNT, int TILE, bool HALF>
+template <bool COUNT, int TILE, bool HALF, int MTX = 8>
 void launch_one(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
 {
     const int grid = ctx->n_sm * ctx->raster_ctas_per_sm[TILE == 16][HALF];
-    k_raster<COUNT, TILE, HALF><<<grid, RAS_THREADS, ras_smem_bytes<HALF>(), st>>>(
+    k_raster<COUNT, TILE, HALF, MTX><<<grid, RAS_THREADS, ras_smem_bytes<HALF>(), st>>>(
         ctx->pairs, ctx->rec, ctx->rec16, ctx->mt_offset, ctx->mt_count, ctx->batch_offset, ctx->unit_mt, ctx->unit_order, P, ctx->hdr,
         ctx->partial, ctx->unit_active, ctx->cut_word, ctx->cut_term, ctx->tile_load);
 }
@@ -629,6 +635,10 @@ int higs_raster_setup(higs_ctx* ctx)
     if ((rc = setup_one<true, 16, false>(ctx, nullptr))) return rc;
     if ((rc = setup_one<false, 16, true>(ctx, &ctx->raster_ctas_per_sm[1][1]))) return rc;
     if ((rc = setup_one<true, 16, true>(ctx, nullptr))) return rc;
+    if ((rc = setup_one<false, 8, false, 4>(ctx, nullptr))) return rc;
+    if ((rc = setup_one<true, 8, false, 4>(ctx, nullptr))) return rc;
+    if ((rc = setup_one<false, 8, false, 16>(ctx, nullptr))) return rc;
+    if ((rc = setup_one<true, 8, false, 16>(ctx, nullptr))) return rc;
     return HIGS_OK;
 }
 
@@ -636,7 +646,12 @@ int launch_raster(higs_ctx* ctx, const FrameParams& P, cudaStream_t st)
 {
     const bool count = (P.flags & HIGS_FLAG_COUNT_EVALS) != 0, half = (P.flags & HIGS_FLAG_FP16) != 0;
 #define HIGS_RAS(T, H) do { if (count) launch_one<true, T, H>(ctx, P, st); else launch_one<false, T, H>(ctx, P, st); } while (0)
-    if (P.tile == 16) { if (half) HIGS_RAS(16, true); else HIGS_RAS(16, false); }
+    if (P.mt_tx != 8) {                                               // shape sweep: fp32 path, 8 x 8 tiles (render_impl checks the combination)
+        if (P.tile != 8 || half) return HIGS_E_ARG;
+        if (P.mt_tx == 4) { if (count) launch_one<true, 8, false, 4>(ctx, P, st); else launch_one<false, 8, false, 4>(ctx, P, st); }
+        else              { if (count) launch_one<true, 8, false, 16>(ctx, P, st); else launch_one<false, 8, false, 16>(ctx, P, st); }
+    }
+    else if (P.tile == 16) { if (half) HIGS_RAS(16, true); else HIGS_RAS(16, false); }
     else              { if (half) HIGS_RAS(8, true);  else HIGS_RAS(8, false); }
 #undef HIGS_RAS
     HIGS_LAUNCHED(ctx);
@@ -649,9 +664,14 @@ int launch_merge(higs_ctx* ctx, const FrameParams& P, float* out_rgb, cudaStream
     const bool half = (P.flags & HIGS_FLAG_FP16) != 0;
 #define HIGS_MRG(T, H) HIGS_CUDA(ctx, launch_pdl(k_merge_image<T, H>, dim3((warps + 7) / 8), dim3(256), 0, st, ctx->partial, ctx->unit_active, \
                                                  ctx->batch_offset, P, ctx->hdr, out_rgb))
-    if (P.tile == 16) { if (half) HIGS_MRG(16, true); else HIGS_MRG(16, false); }
+#define HIGS_MRG_MT(X) HIGS_CUDA(ctx, launch_pdl(k_merge_image<8, false, X>, dim3((warps + 7) / 8), dim3(256), 0, st, ctx->partial, ctx->unit_active, \
+                                                 ctx->batch_offset, P, ctx->hdr, out_rgb))
+    if (P.mt_tx == 4) HIGS_MRG_MT(4);
+    else if (P.mt_tx == 16) HIGS_MRG_MT(16);
+    else if (P.tile == 16) { if (half) HIGS_MRG(16, true); else HIGS_MRG(16, false); }
     else              { if (half) HIGS_MRG(8, true);  else HIGS_MRG(8, false); }
 #undef HIGS_MRG
+#undef HIGS_MRG_MT
     HIGS_LAUNCHED(ctx);
     return HIGS_OK;
 }

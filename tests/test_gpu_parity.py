@@ -22,9 +22,9 @@ def hg():
     return hg
 
 
-def _render(hg, scene, cam, flags=0, batch_cap=1024, max_pairs=0, tile=8):
+def _render(hg, scene, cam, flags=0, batch_cap=1024, max_pairs=0, tile=8, mt=(8, 4)):
     import torch
-    r = hg.Renderer(max(scene.N, 1), cam.W, cam.H, max_pairs=max_pairs, flags=flags, batch_cap=batch_cap, tile=tile)
+    r = hg.Renderer(max(scene.N, 1), cam.W, cam.H, max_pairs=max_pairs, flags=flags, batch_cap=batch_cap, tile=tile, mt=mt)
     dev = hg.scene_to_device(scene)
     img = r.render(*dev, scene.degree, cam)
     torch.cuda.synchronize()
@@ -68,12 +68,12 @@ def psnr(img, ref) -> float:
 PSNR_FP16 = 60.0        # acceptance of the fp16 data path against the fp32 oracle (paper: 67 dB)
 
 
-def _full_check(hg, scene, cam, flags=0, batch_cap=1024, image=True, tile=8, min_psnr=None):
+def _full_check(hg, scene, cam, flags=0, batch_cap=1024, image=True, tile=8, min_psnr=None, mt=(8, 4)):
     """Every output of one frame against the oracle.  With HIGS_FLAG_FP16 the integer lists are still bit-exact (the
     cull, the row scan and the sort are the same pinned fp32 code); the image is accepted by PSNR, records are not exported."""
-    r, img = _render(hg, scene, cam, flags=flags, batch_cap=batch_cap, tile=tile)
+    r, img = _render(hg, scene, cam, flags=flags, batch_cap=batch_cap, tile=tile, mt=mt)
     pr = oracle.project(scene, cam)
-    ols = oracle.bin_lists(pr, B_r=batch_cap, tile=tile)
+    ols = oracle.bin_lists(pr, B_r=batch_cap, tile=tile, mt=mt)
     st = r.stats()
     assert st["n_visible"] == pr.n_vis and st["n_pairs"] == ols.n_pairs and st["n_units"] == ols.n_units
     assert st["overflow"] == 0 and st["batch_cap"] == batch_cap and st["tile"] == tile
@@ -418,6 +418,29 @@ def test_tile16_variant_odd_sizes_and_full_size(hg, large_scene):
     pr = oracle.project(large_scene, cam)
     _check_lists(r.lists(), oracle.bin_lists(pr, tile=16))
     assert np.abs(img - oracle.render(pr)).max() <= PIX_TOL
+    r.close()
+
+
+@pytest.mark.parametrize("mt", [(4, 8), (16, 2)])
+def test_macro_tile_shapes(hg, mt, large_scene):
+    """Macro-tile shape sweep: 32 render tiles grouped 4 x 8 or 16 x 2 instead of 8 x 4.  Records
+    and lists bit-exact against the oracle's lists on that grid, whole image within 2e-3: small scenes, small batches, odd
+    sizes, BASELINE.json configs[3] at full size.  Unsupported combinations are refused."""
+    for s, bc in ((hs.scene_cfg0(), 1024), (hs.scene_cfg0(), 16), (hs.scene_cfg1(), 1024), (hs.scene_cfg1(), 48),
+                  (hs.scene_cfg0(N=800, W=129, H=70), 64)):
+        _full_check(hg, s, s.cameras[0], batch_cap=bc, mt=mt)
+    cam = large_scene.cameras[0]
+    r, img = _render(hg, large_scene, cam, mt=mt)
+    pr = oracle.project(large_scene, cam)
+    _check_lists(r.lists(), oracle.bin_lists(pr, mt=mt))
+    assert np.abs(img - oracle.render(pr)).max() <= PIX_TOL
+    L = hg.load()
+    assert L.higs_set_tile(r.ctx, 16) == hg.HIGS_E_ARG                     # other shapes: 8 x 8 tiles only
+    assert L.higs_set_macro_tile(r.ctx, 8, 8) == hg.HIGS_E_ARG and L.higs_set_macro_tile(r.ctx, 2, 16) == hg.HIGS_E_ARG
+    hg.higs_set_flags(r.ctx, hg.HIGS_FLAG_FP16)                            # ... and the fp32 path only
+    s0 = hs.scene_cfg0()
+    with pytest.raises(hg.HigsError):
+        r.render(*hg.scene_to_device(s0), s0.degree, s0.cameras[0])
     r.close()
 
 
