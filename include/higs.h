@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define HIGS_ABI_VERSION 3    /* 2: higs_lists.tile_load, higs_stats.tile, set_tile / scene_sort_spatial / scene_compress_sh / get_sh32; 3: set_macro_tile */
+#define HIGS_ABI_VERSION 3    /* 2: higs_lists.tile_load, higs_stats.tile, set_tile / scene_sort_spatial / scene_compress_sh / get_sh32; 3: set_macro_tile, sh32_encode_static */
 
 #define HIGS_TILE        8      /* render tile edge, px  */
 #define HIGS_MT_W        64     /* macro-tile width,  px (8 tiles)  */
@@ -189,6 +189,21 @@ int higs_scene_sort_spatial(higs_ctx* ctx, uint32_t* host_perm);
 int higs_scene_compress_sh(higs_ctx* ctx);
 /* Copies the codes ([N][32] bytes) and the scale table ([16][3] floats: Y, Co, Cg) to HOST memory (either may be NULL). */
 int higs_get_sh32(higs_ctx* ctx, uint8_t* host_codes, float* host_scales);
+
+/* The same encoder for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): no context, no cudaMalloc / cudaFree, no host synchronisation; it only enqueues kernels and one 192-byte
+ * device-to-device copy on cuda_stream, on the CURRENT device.  All pointers are DEVICE pointers owned by the caller:
+ *   d_sh     [N][16][3] fp32 degree-3 SH rows (input),
+ *   d_codes  [N][32] bytes (output, 16-byte aligned), d_scales [16][3] fp32 (output: Y, Co, Cg scale per basis).
+ * Bytes and scales are identical to higs_scene_compress_sh + higs_get_sh32 on the same rows.  N = 0 writes scales of 1.
+ * The work area of the percentile selection (49,920 bytes) is a file-scope device array inside the library: every GPU that
+ * loads the library holds it until the process exits.  It is SHARED by all calls and keeps the last call's contents (each
+ * call clears what must start at zero): calls that overlap on the GPU - two streams, two host threads - race; serialise them.
+ * Errors: HIGS_E_CAPACITY if N > HIGS_SH32_STATIC_MAX_N (the work area's counters are 32-bit), HIGS_E_ARG for null or
+ * misaligned pointers or N < 0, HIGS_E_CUDA; text of this thread's last failure: higs_sh32_encode_static_error(). */
+#define HIGS_SH32_STATIC_MAX_N 1073741824ll   /* 2^30 gaussians */
+int higs_sh32_encode_static(const float* d_sh, int64_t N, uint8_t* d_codes, float* d_scales, void* cuda_stream);
+const char* higs_sh32_encode_static_error(void);
 /* Resident-scene path with a DEVICE image (no download, no synchronisation). */
 int higs_render_view(higs_ctx* ctx, const higs_camera* cam, int W, int H, float* out_rgb, void* cuda_stream);
 

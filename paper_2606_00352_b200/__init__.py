@@ -23,7 +23,7 @@ HIGS_FLAG_STAGE_TIMERS, HIGS_FLAG_COUNT_EVALS, HIGS_FLAG_NO_XBATCH_CUT, HIGS_FLA
 HIGS_TILE, HIGS_MT_W, HIGS_MT_H, HIGS_MT_TILES, HIGS_BATCH_CAP = 8, 64, 32, 32, 1024
 
 EXPORTS = ["higs_abi_version", "higs_strerror", "higs_last_error", "higs_create", "higs_destroy", "higs_set_flags",
-           "higs_set_batch_cap", "higs_set_tile", "higs_set_macro_tile", "higs_render", "higs_render_host", "higs_scene_upload", "higs_render_view_host",
+           "higs_set_batch_cap", "higs_set_tile", "higs_set_macro_tile", "higs_sh32_encode_static", "higs_sh32_encode_static_error", "higs_render", "higs_render_host", "higs_scene_upload", "higs_render_view_host",
            "higs_render_view", "higs_scene_sort_spatial", "higs_scene_compress_sh", "higs_get_sh32", "higs_get_stats", "higs_get_lists", "higs_get_records", "higs_sort_segments", "higs_download"]
 
 
@@ -82,6 +82,9 @@ def load() -> C.CDLL:
         L.higs_set_batch_cap.restype = C.c_int; L.higs_set_batch_cap.argtypes = [vp, C.c_int]
         L.higs_set_tile.restype = C.c_int; L.higs_set_tile.argtypes = [vp, C.c_int]
         L.higs_set_macro_tile.restype = C.c_int; L.higs_set_macro_tile.argtypes = [vp, C.c_int, C.c_int]
+        L.higs_sh32_encode_static.restype = C.c_int
+        L.higs_sh32_encode_static.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.higs_sh32_encode_static_error.restype = C.c_char_p; L.higs_sh32_encode_static_error.argtypes = []
         L.higs_render.restype = C.c_int
         L.higs_render.argtypes = [vp, f32p, f32p, f32p, f32p, f32p, C.c_int, C.c_int64, C.POINTER(higs_camera),
                                   C.c_int, C.c_int, f32p, vp]
@@ -210,6 +213,22 @@ def higs_get_sh32(ctx, n: int):
     codes = np.zeros((n, 32), np.uint8); scales = np.zeros((16, 3), np.float32)
     _check(load().higs_get_sh32(ctx, C.c_void_p(codes.ctypes.data), C.c_void_p(scales.ctypes.data)), "higs_get_sh32", ctx)
     return codes, scales
+
+
+HIGS_SH32_STATIC_MAX_N = 1 << 30
+
+
+def higs_sh32_encode_static(d_sh, n: int, d_codes, d_scales, stream: Optional[int] = None) -> None:
+    """32-byte SH codes of n degree-3 rows without any allocation (include/higs.h): device tensors in and out, enqueue only."""
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream
+    L = load()
+    rc = L.higs_sh32_encode_static(C.c_void_p(d_sh.data_ptr() if d_sh is not None else None), int(n),
+                                   C.c_void_p(d_codes.data_ptr() if d_codes is not None else None),
+                                   C.c_void_p(d_scales.data_ptr() if d_scales is not None else None), C.c_void_p(stream))
+    if rc != HIGS_OK:
+        raise HigsError(rc, "higs_sh32_encode_static: " + L.higs_sh32_encode_static_error().decode())
 
 
 def higs_render_view_host(ctx, cam: higs_camera, W: int, H: int, out_rgb) -> None:

@@ -13,6 +13,8 @@
 // work: every arithmetic step is one correctly rounded fp32 op in the written order, so the bytes are identical to the
 // CPU oracle's.  The percentile is an exact selection: four 8-bit passes of a radix select on the bit patterns of |v|
 // (non-negative floats order like unsigned integers), 48 columns at a time.
+#include <pthread.h>
+#include <stdint.h>
 #include <stdio.h>
 #include <string.h>
 #include "higs_internal.cuh"
@@ -182,5 +184,85 @@ int launch_sh32_encode(higs_ctx* ctx, cudaStream_t st)
     }
     HIGS_CUDA(ctx, cudaMemcpyAsync(ctx->sh32_scales_host, work + W_SCALE, sizeof(float) * 48, cudaMemcpyDeviceToHost, st));
     HIGS_CUDA(ctx, cudaStreamSynchronize(st));
+    return HIGS_OK;
+}
+
+// ---- higs_sh32_encode_static: the encoder for callers that cannot allocate ------------------------------------------
+// (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc.)  Same kernels as above; the radix-select work
+// area (W_TOTAL words = 49,920 bytes: 48 x 256 counters, prefixes, ranks, scales) lives in a file-scope device array
+// instead of ctx->sh32_work, so the call needs no context and allocates nothing.  Every GPU that loads the library holds
+// these 49,920 bytes until the process exits.  The array is shared by all calls and keeps the last call's contents:
+// k_sh_select_init clears what must start at zero; calls that overlap on the GPU (two streams, two threads) race on it.
+static __device__ __align__(256) uint32_t g_sh32_static_work[W_TOTAL];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticDev { bool ready; uint32_t* work; int n_sm; };
+StaticDev g_static_dev[STATIC_MAX_DEVICES];                          // set up once per device (guarded by g_static_mutex)
+pthread_mutex_t g_static_mutex = PTHREAD_MUTEX_INITIALIZER;
+thread_local char g_static_err[256] = "";
+
+__global__ void k_sh_static_ones(float* __restrict__ scales) { if (threadIdx.x < 48) scales[threadIdx.x] = 1.0f; }   // N = 0: as launch_sh32_encode
+
+int static_fail(int code, const char* what, cudaError_t e = cudaSuccess)
+{
+    if (e != cudaSuccess) { snprintf(g_static_err, sizeof(g_static_err), "%s: %s", what, cudaGetErrorString(e)); cudaGetLastError(); }
+    else snprintf(g_static_err, sizeof(g_static_err), "%s", what);
+    return code;
+}
+} // namespace
+
+const char* higs_sh32_encode_static_error(void) { return g_static_err; }
+
+int higs_sh32_encode_static(const float* d_sh, int64_t N, uint8_t* d_codes, float* d_scales, void* cuda_stream)
+{
+    g_static_err[0] = 0;
+    if (N < 0) return static_fail(HIGS_E_ARG, "higs_sh32_encode_static: N < 0");
+    if (N > HIGS_SH32_STATIC_MAX_N) {
+        snprintf(g_static_err, sizeof(g_static_err), "higs_sh32_encode_static: N = %lld exceeds HIGS_SH32_STATIC_MAX_N = %lld (32-bit counters of the static work area)",
+                 (long long)N, (long long)HIGS_SH32_STATIC_MAX_N);
+        return HIGS_E_CAPACITY;
+    }
+    if (!d_scales || (N > 0 && (!d_sh || !d_codes))) return static_fail(HIGS_E_ARG, "higs_sh32_encode_static: null pointer");
+    if ((reinterpret_cast<uintptr_t>(d_sh) & 3u) || (reinterpret_cast<uintptr_t>(d_codes) & 15u))
+        return static_fail(HIGS_E_ARG, "higs_sh32_encode_static: d_sh must be 4-byte and d_codes 16-byte aligned");
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return static_fail(HIGS_E_CUDA, "cudaGetDevice", e);
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return static_fail(HIGS_E_ARG, "higs_sh32_encode_static: device index beyond 63");
+    const size_t hist_smem = sizeof(uint32_t) * (48 * 256 + 48);
+    pthread_mutex_lock(&g_static_mutex);
+    StaticDev sd = g_static_dev[dev];
+    if (!sd.ready) {
+        // once per device, with that device current: the array's name is a host-side stand-in here, not a device address
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_sh32_static_work);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_sh_select_hist, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)hist_smem);
+        int n_sm = 0;
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess || !p || n_sm <= 0) {
+            pthread_mutex_unlock(&g_static_mutex);
+            return static_fail(HIGS_E_CUDA, "higs_sh32_encode_static set-up (cudaGetSymbolAddress / attributes)", e);
+        }
+        sd.ready = true; sd.work = static_cast<uint32_t*>(p); sd.n_sm = n_sm;
+        g_static_dev[dev] = sd;
+    }
+    pthread_mutex_unlock(&g_static_mutex);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    uint32_t* work = sd.work;
+    if (N == 0) {
+        k_sh_static_ones<<<1, 64, 0, st>>>(d_scales);
+        if ((e = cudaGetLastError()) != cudaSuccess) return static_fail(HIGS_E_CUDA, "higs_sh32_encode_static launch", e);
+        return HIGS_OK;
+    }
+    k_sh_select_init<<<1, 256, 0, st>>>(work, N);                    // clears the counters and prefixes the last call left behind
+    for (int pass = 0; pass < 4; ++pass) {
+        k_sh_select_hist<<<sd.n_sm * 2, ENC_THREADS, hist_smem, st>>>(d_sh, N, pass, work);
+        k_sh_select_step<<<48, 32, 0, st>>>(work, pass);
+    }
+    k_sh_encode<<<(unsigned)((N + ENC_THREADS - 1) / ENC_THREADS), ENC_THREADS, 0, st>>>(d_sh, N, work, reinterpret_cast<uint4*>(d_codes));
+    if ((e = cudaGetLastError()) != cudaSuccess) return static_fail(HIGS_E_CUDA, "higs_sh32_encode_static launch", e);
+    if ((e = cudaMemcpyAsync(d_scales, work + W_SCALE, sizeof(float) * 48, cudaMemcpyDeviceToDevice, st)) != cudaSuccess)
+        return static_fail(HIGS_E_CUDA, "higs_sh32_encode_static scale copy", e);
     return HIGS_OK;
 }
