@@ -25,7 +25,8 @@ constexpr int BIN_THREADS = 1024;   // two CTAs per SM at 32 registers: the pass
 __global__ void __launch_bounds__(1024)
 k_plan(const FrameParams P,
        const uint32_t* __restrict__ mt_count, uint32_t* __restrict__ mt_offset, uint32_t* __restrict__ batch_offset,
-       SortJob* __restrict__ sort_jobs, size_t max_jobs, SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr)
+       SortJob* __restrict__ sort_jobs, size_t max_jobs, SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr,
+       uint4* __restrict__ pairs_touch)
 {
     __shared__ uint32_t s_warp[33 * 8];
     __shared__ uint32_t s_max;
@@ -33,6 +34,29 @@ k_plan(const FrameParams P,
     if (threadIdx.x == 0) { s_max = 0; s_total = 0ull; }
     pdl_wait(); pdl_trigger();
     __syncthreads();
+    // CTAs 1 .. gridDim.x - 1: beside the one CTA that plans, the rest of the GPU has nothing to do for these 13 us.  They write
+    // zeros over the part of the pair list the fill pass is about to fill.  The fill pass drops 8-byte items at scattered places:
+    // partial-sector writes, which L2 answers with a fill read of the sector from DRAM when the line is not resident (it never is:
+    // the list was last touched a frame ago) - ncu counted 47 MB of such reads, and the kernel ran at the pace of those fills,
+    // whatever its occupancy or instruction count (0.082 ms).  Whole lines written here are resident and dirty when the fill pass
+    // comes (41 MB, L2 holds 126 MB), its partial writes hit, and it runs 0.060 ms, as it does on a spatially ordered scene whose
+    // stores coalesce; this kernel grows from 0.013 to 0.019 ms (the zeros are 8 us of L2 write bandwidth).  Every item zeroed
+    // here is overwritten by the fill pass, which starts after this grid has completed.  (The same treatment of the alternate
+    // buffer the oversize split scatters into was measured and bought nothing.)
+    if (blockIdx.x > 0) {
+        unsigned long long tot = 0;
+        for (int m = threadIdx.x; m < P.n_m; m += 1024) tot += mt_count[m];
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, d);
+        if ((threadIdx.x & 31) == 0 && tot) atomicAdd(&s_total, tot);
+        __syncthreads();
+        if (s_total > (unsigned long long)P.max_pairs) return;
+        const size_t n16 = (size_t)s_total / 2;                       // whole 16-byte pieces (an odd last item stays a partial write)
+        const size_t per = (n16 + (gridDim.x - 1) - 1) / (gridDim.x - 1);
+        const size_t a = (size_t)(blockIdx.x - 1) * per, b = a + per < n16 ? a + per : n16;
+        for (size_t i = a + threadIdx.x; i < b; i += 1024) pairs_touch[i] = make_uint4(0u, 0u, 0u, 0u);
+        return;
+    }
     uint32_t carry[2] = {0, 0};
     unsigned long long my_total = 0;
     const uint32_t br = (uint32_t)P.batch_cap;
@@ -226,8 +250,9 @@ k_fill(const uint32_t* __restrict__ chunk_count, const uint32_t* __restrict__ pa
         }
     };
     // warps claim chunks (up to 128 dense survivor slots: four warp iterations) from a shared counter: no search for the
-    // slot of the k-th survivor of the batch (it was a third of the kernel's instructions; the kernel waits on memory, so the
-    // time did not move: 0.083 ms), tail of at most one chunk.  Requesting the next record ahead spills at 32 registers.
+    // slot of the k-th survivor of the batch (it was a third of the kernel's instructions and the time did not move; neither did it
+    // with half the warps, with the records requested four deep or prefetched: the kernel ran at the pace of L2's fill reads for
+    // its partial-sector stores, see k_plan), tail of at most one chunk.
     for (;;) {
         uint32_t q = 0;
         if (lane == 0) q = atomicAdd(&s_next, 1u);
@@ -287,8 +312,8 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
     const int lcap = higs_part_lcap((N + HIGS_CHUNK - 1) / HIGS_CHUNK, n_b);
     const size_t smem = sizeof(uint32_t) * ((size_t)P.n_m + 2 * (size_t)lcap + 1 + 2 * FILL_QCAP);
     if (ev_count) cudaEventRecord(ev_count, st);    // the count pass ran inside k_project: this stage is empty
-    HIGS_CUDA(ctx, launch_pdl(k_plan, dim3(1), dim3(1024), 0, st, P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->sort_jobs,
-                              (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr));
+    HIGS_CUDA(ctx, launch_pdl(k_plan, dim3(1 + ctx->n_sm), dim3(1024), 0, st, P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->sort_jobs,
+                              (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr, reinterpret_cast<uint4*>(ctx->pairs)));
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
     HIGS_CUDA(ctx, launch_pdl(k_fill, dim3(n_b), dim3(BIN_THREADS), smem, st, ctx->chunk_count, ctx->part_list, ctx->part_desc, lcap, ctx->bin,
