@@ -187,6 +187,7 @@ int higs_create(higs_ctx** out, int device, int64_t max_gaussians, int max_W, in
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return fail(HIGS_E_CUDA);
     ctx->n_sm = prop.multiProcessorCount;
+    ctx->touch_max_pairs = (uint32_t)((size_t)prop.l2CacheSize / 4 * 3 / 8);
     const int64_t n = max_gaussians > 0 ? max_gaussians : 1;
     ctx->n_chunks_max = (n + HIGS_CHUNK - 1) / HIGS_CHUNK;
     if ((rc = higs_project_smem_setup(ctx))) return fail(rc);       // also fixes n_part_max = n_sm x resident CTAs

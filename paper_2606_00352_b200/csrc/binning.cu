@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(1024)
 k_plan(const FrameParams P,
        const uint32_t* __restrict__ mt_count, uint32_t* __restrict__ mt_offset, uint32_t* __restrict__ batch_offset,
        SortJob* __restrict__ sort_jobs, size_t max_jobs, SplitSeg* __restrict__ split, FrameHeader* __restrict__ hdr,
-       uint4* __restrict__ pairs_touch)
+       uint4* __restrict__ pairs_touch, uint32_t touch_max_pairs)
 {
     __shared__ uint32_t s_warp[33 * 8];
     __shared__ uint32_t s_max;
@@ -50,7 +50,7 @@ k_plan(const FrameParams P,
         for (int d = 16; d > 0; d >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, d);
         if ((threadIdx.x & 31) == 0 && tot) atomicAdd(&s_total, tot);
         __syncthreads();
-        if (s_total > (unsigned long long)P.max_pairs) return;
+        if (s_total > (unsigned long long)P.max_pairs || s_total > (unsigned long long)touch_max_pairs) return;   // a list that does not fit in L2 gains nothing
         const size_t n16 = (size_t)s_total / 2;                       // whole 16-byte pieces (an odd last item stays a partial write)
         const size_t per = (n16 + (gridDim.x - 1) - 1) / (gridDim.x - 1);
         const size_t a = (size_t)(blockIdx.x - 1) * per, b = a + per < n16 ? a + per : n16;
@@ -313,7 +313,7 @@ int launch_binning(higs_ctx* ctx, const FrameParams& P, int64_t N, cudaStream_t 
     const size_t smem = sizeof(uint32_t) * ((size_t)P.n_m + 2 * (size_t)lcap + 1 + 2 * FILL_QCAP);
     if (ev_count) cudaEventRecord(ev_count, st);    // the count pass ran inside k_project: this stage is empty
     HIGS_CUDA(ctx, launch_pdl(k_plan, dim3(1 + ctx->n_sm), dim3(1024), 0, st, P, ctx->mt_count, ctx->mt_offset, ctx->batch_offset, ctx->sort_jobs,
-                              (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr, reinterpret_cast<uint4*>(ctx->pairs)));
+                              (size_t)ctx->max_jobs, ctx->split_segs, ctx->hdr, reinterpret_cast<uint4*>(ctx->pairs), ctx->touch_max_pairs));
     HIGS_LAUNCHED(ctx);
     if (ev_scan) cudaEventRecord(ev_scan, st);
     HIGS_CUDA(ctx, launch_pdl(k_fill, dim3(n_b), dim3(BIN_THREADS), smem, st, ctx->chunk_count, ctx->part_list, ctx->part_desc, lcap, ctx->bin,

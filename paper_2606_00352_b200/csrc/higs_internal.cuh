@@ -76,6 +76,7 @@ struct higs_ctx {
     int batch_cap;
     int tile;                  // render-tile edge in effect (8 or 16)
     int mt_tx, mt_ty;          // macro-tile shape in render tiles (8 x 4 unless higs_set_macro_tile changed it)
+    uint32_t touch_max_pairs;  // k_plan pre-writes the pair list when it has at most this many items (3/4 of L2)
     // scratch (device)
     uint32_t* valid_bits;      // [ceil(maxN/32)]
     float4*   rec;             // [slots][4]  mux,muy,A,B2 | C,tau,log2o,r | g,b,a,b | c,bits(key),id,-   (64 B; the rasterizer gathers the

@@ -561,8 +561,20 @@ int launch_project(higs_ctx* ctx, const FrameParams& P, const float* means, cons
 
 int higs_project_smem_setup(higs_ctx* ctx)
 {
-    // worst case for the list: the full grid on max_gaussians (a smaller grid has at most 16 chunks per CTA)
-    const int lcap_max = higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) > 6 * PROJ_WARPS_MAX ? higs_part_lcap(ctx->n_chunks_max, ctx->n_sm) : 6 * PROJ_WARPS_MAX;
+    // The chunk list of a CTA (four times its fair share of the chunks of max_gaussians) is part of its shared memory, and the
+    // fair share depends on how many CTAs the grid has: the largest number of CTAs per SM whose list still lets that many CTAs
+    // be resident (sizing the list for one CTA per SM made it so long at 75 M gaussians that only one fitted).  The 512-thread
+    // variants carry the largest queue: they decide.
+    int per_sm = 1, lcap_max = 0;
+    for (int c = 4; c >= 1; --c) {
+        lcap_max = higs_part_lcap(ctx->n_chunks_max, ctx->n_sm * c) > 6 * PROJ_WARPS_MAX ? higs_part_lcap(ctx->n_chunks_max, ctx->n_sm * c) : 6 * PROJ_WARPS_MAX;
+        const size_t b = project_smem_bytes(ctx->max_nm, lcap_max, PROJ_WARPS_MAX);
+        int occ = 0;
+        if (cudaFuncSetAttribute(k_project<3, true, SH_ROWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)b) != cudaSuccess) { cudaGetLastError(); continue; }
+        HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3, true, SH_ROWS>, proj_threads(true, SH_ROWS), b));
+        per_sm = c;
+        if (occ >= c) break;
+    }
     const int bytes = (int)project_smem_bytes(ctx->max_nm, lcap_max, PROJ_WARPS_MAX);
 #define HIGS_ATTR(D, H, C) HIGS_CUDA(ctx, cudaFuncSetAttribute(k_project<D, H, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes))
     HIGS_ATTR(0, false, SH_ROWS); HIGS_ATTR(1, false, SH_ROWS); HIGS_ATTR(2, false, SH_ROWS); HIGS_ATTR(3, false, SH_ROWS);
@@ -581,8 +593,6 @@ int higs_project_smem_setup(higs_ctx* ctx)
         HIGS_ATTR(0, true); HIGS_ATTR(1, true); HIGS_ATTR(2, true); HIGS_ATTR(3, true);
 #undef HIGS_ATTR
     }
-    int occ = 0;
-    HIGS_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_project<3, true, SH_ROWS>, proj_threads(true, SH_ROWS), (size_t)bytes));
-    ctx->n_part_max = ctx->n_sm * (occ < 1 ? 1 : occ);
+    ctx->n_part_max = ctx->n_sm * per_sm;
     return HIGS_OK;
 }
